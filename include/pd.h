@@ -1,0 +1,117 @@
+/*
+ * pd.h -- C ABI of the B200-native primal-dual (Chambolle-Pock) solver for the dipole-kernel
+ * deconvolution of positive-contrast susceptibility MRI (arXiv 2006.09808).
+ *
+ * What is solved (Eq.(1); readings R1-R3 in DESIGN.md), independently for every
+ * 2-D slice / coil field map b of a stack:
+ *
+ *     chi_b = argmin_chi  1/2 || W (K chi - phi_b) ||_2^2 + lambda || M G chi ||_1 ,   K = F^-1 D F
+ *
+ * by exactly the iteration of PAPER.md:44-49 (p-update, q-update, chi-update, over-relaxation),
+ * started from zero and run for max_iters iterations ("Until n >= N")
+ * or, per slice, until the relative primal-dual gap falls below tol (BASELINE.json north_star (d)).
+ * D(kx,ky) = 1/3 - k_b^2/(kx^2+ky^2), D(0,0) = 0 (BASELINE.json north_star).  G: forward
+ * differences with Neumann boundary; M: mask on the gradient; W: optional data weighting.
+ *
+ * Layout of every image argument: fp32, [batch][ny][nx], x fastest, contiguous, 16-byte aligned.
+ * Multi-coil stacks: batch = nslices*ncoils, index slice*ncoils + coil (BASELINE.json configs[3]);
+ * every coil map is reconstructed independently.
+ *
+ * All entry points return PD_OK (0) or a negative pd_error; nothing throws across the ABI; there
+ * is no global state.  A plan is not thread-safe; distinct plans are independent.  There is no
+ * CPU fallback: every step of the path runs in sm_100a CUDA kernels.
+ */
+#ifndef PD_B200_H
+#define PD_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pd_plan_s *pd_plan_t; /* opaque, library-owned */
+
+enum pd_b0 { PD_B0_X = 0, PD_B0_Y = 1 }; /* in-plane B0 axis: k_b = kx (fast axis) or ky (row axis) */
+
+enum pd_error {
+    PD_OK = 0,
+    PD_EINVAL = -1,   /* null plan/field/chi_out, batch < 1, max_iters < 0, theta outside [0,1], lambda < 0, bad option */
+    PD_ESIZE = -2,    /* nx or ny not in {64,128,256,512} */
+    PD_ESTEP = -3,    /* explicit steps with sigma*tau*(4/9+8) >= 1: convergence bound of [7] violated */
+    PD_ENOMEM = -4,   /* device allocation failed */
+    PD_ECUDA = -5,    /* a CUDA call or launch failed; pd_strerror(PD_ECUDA) returns the last CUDA error text */
+    PD_EVARIANT = -6  /* PD_VARIANT_RESIDENT requested for a size that does not fit on chip */
+};
+
+enum pd_option {
+    PD_OPT_TV_MODE = 0,      /* PD_TV_ISO (default) | PD_TV_ANISO: how |.| in the q-projection is read (PAPER.md:49 line 2) */
+    PD_OPT_LAMBDA_CONV = 1,  /* PD_LAMBDA_REG (default): 1/2||.||^2 + lambda*TV ; PD_LAMBDA_DATA: lambda/2||.||^2 + TV (PAPER.md:37 literally) */
+    PD_OPT_VARIANT = 2,      /* PD_VARIANT_AUTO (default) | PD_VARIANT_STREAMING | PD_VARIANT_RESIDENT */
+    PD_OPT_CHECK_EVERY = 3,  /* tolerance tested when (n+1) % value == 0 ; default 1 */
+    PD_OPT_MASK_SHARED = 4,  /* 0 (default): mask is [batch][ny][nx] ; 1: one [ny][nx] mask for all slices */
+    PD_OPT_UNSAFE_STEPS = 5  /* 1: skip the PD_ESTEP check at the next pd_set_steps call (not at pd_plan) */
+};
+enum { PD_TV_ISO = 0, PD_TV_ANISO = 1 };
+enum { PD_LAMBDA_REG = 0, PD_LAMBDA_DATA = 1 };
+enum { PD_VARIANT_AUTO = 0, PD_VARIANT_STREAMING = 1, PD_VARIANT_RESIDENT = 2 };
+
+/* pd_plan (host call; PAPER.md:44 step 1, "dipole kernel convolution operator D").
+ * Builds the dipole table D for (nx, ny, B0_dir), the FFT twiddle tables (computed in double), and the
+ * device workspace for `batch` slices: p, q (2 comps), chibar, one complex spectrum per slice pair, the
+ * per-slice state variables.  sigma <= 0 or tau <= 0 selects the automatic steps
+ * sigma = tau = 1/sqrt(4/9 + 8) (upper bound on ||K_full||_2).  *out receives the plan.
+ * Errors: PD_EINVAL, PD_ESIZE, PD_ESTEP, PD_ENOMEM, PD_ECUDA.  Uses the current CUDA device. */
+int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir,
+            float lambda, float sigma, float tau, float theta);
+
+/* pd_solve (the Repeat loop; flow steps (3)-(5)).
+ * field  : DEVICE, const, [batch][ny][nx]  -- the local field map phi = Delta B ("iFreq delta")
+ * mask   : DEVICE, const, [batch][ny][nx] (or [ny][nx] with PD_OPT_MASK_SHARED), multiplies the gradient (M of
+ *          Eq.(1)); NULL = all ones.  Any float is accepted and used as a multiplier.
+ * chi_out: DEVICE, [batch][ny][nx] -- receives chi_N (PAPER.md:49 names chi the solution).  It is also the
+ *          solver's primal state during the call; must not alias field/mask/W.
+ * max_iters >= 0.  tol <= 0: exactly max_iters iterations for every slice.  tol > 0: slice b stops at the first
+ *          checked iteration n+1 with relgap_{n+1} < tol (relative Fenchel-Young gap, R9), else at
+ *          max_iters; stopped slices cost (almost) nothing afterwards.  A slice whose W*phi is identically zero
+ *          returns chi = 0 (iters_done 0 when tol > 0).
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Everything is enqueued on it; the call does not
+ *          synchronise and never copies to the host.  Buffers must stay alive until the stream
+ *          reaches the end of the enqueued work.  Inputs are never written.
+ * Errors: PD_EINVAL, PD_ECUDA. */
+int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
+             int max_iters, float tol, void *cuda_stream);
+
+/* pd_solve_host: same computation with HOST buffers (pageable or pinned) -- flow steps (2) and (6) of the paper
+ * done by the library: H2D of field (and mask if non-NULL), pd_solve, D2H of chi_out, on
+ * cuda_stream, then synchronises that stream.  Staging buffers are plan-owned (allocated on first use). */
+int pd_solve_host(pd_plan_t p, const float *field_host, const float *mask_host, float *chi_out_host,
+                  int max_iters, float tol, void *cuda_stream);
+
+/* Optional data weighting W of Eq.(1) (DEVICE, [batch][ny][nx], caller-owned, must outlive the solves that use it);
+ * NULL (default) = identity. */
+int pd_set_weight(pd_plan_t p, const float *W);
+
+/* Replace lambda / sigma / tau / theta of an existing plan (same checks as pd_plan). */
+int pd_set_steps(pd_plan_t p, float lambda, float sigma, float tau, float theta);
+
+int pd_set_option(pd_plan_t p, int key, int value);
+
+/* Per-slice state variables of the last pd_solve: DEVICE pointers, length batch, plan-owned, valid
+ * (after the stream reached the end of that solve) until the next pd_solve / pd_destroy.  Any pointer may be NULL.
+ * iters_done[b]: iterations executed; relgap[b]: last relative gap computed; relres[b]: last ||chi_{n+1}-chi_n|| / ||chi_{n+1}||. */
+int pd_get_stats(pd_plan_t p, const int **iters_done, const float **relgap, const float **relres);
+
+/* Host convenience: copies the three arrays above into HOST buffers of length batch (any may be NULL), ordered on
+ * cuda_stream after the last pd_solve, and synchronises that stream. */
+int pd_get_stats_host(pd_plan_t p, int *iters_done_host, float *relgap_host, float *relres_host, void *cuda_stream);
+
+/* Number of kernel launches pd_solve enqueued at its last call (for launch accounting in benchmarks). */
+int pd_last_launch_count(pd_plan_t p);
+
+int pd_destroy(pd_plan_t p);
+
+const char *pd_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,170 @@
+"""Thin ctypes binding of the C ABI in include/pd.h (argument marshalling only).
+
+PyTorch is used by callers for device memory and streams; this module only passes raw pointers.
+There is no CPU fallback: if libpd_b200.so is missing or cannot be loaded, every entry point raises.
+Names mirror the C ABI: pd_plan -> Plan(...), pd_solve -> Plan.solve, pd_solve_host -> Plan.solve_host,
+pd_set_weight / pd_set_option / pd_set_steps / pd_get_stats(_host) / pd_destroy likewise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpd_b200.so")
+
+B0_X, B0_Y = 0, 1
+OK, EINVAL, ESIZE, ESTEP, ENOMEM, ECUDA, EVARIANT = 0, -1, -2, -3, -4, -5, -6
+OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS = range(6)
+TV_ISO, TV_ANISO = 0, 1
+LAMBDA_REG, LAMBDA_DATA = 0, 1
+VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
+
+# every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
+SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
+           "pd_get_stats_host", "pd_last_launch_count", "pd_destroy", "pd_strerror"]
+
+_lib = None
+
+
+class PdError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("pd error %d: %s" % (code, text))
+        self.code = code
+
+
+def lib():
+    """Load libpd_b200.so (built in-tree by paper_2006_09808_b200/build.py).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("CUDA library %s is not built (run `python -m paper_2006_09808_b200.build`); "
+                               "there is no CPU fallback" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        vp, fp, ip = C.c_void_p, C.c_float, C.c_int
+        L.pd_plan.argtypes = [C.POINTER(vp), ip, ip, ip, ip, fp, fp, fp, fp]
+        L.pd_solve.argtypes = [vp, vp, vp, vp, ip, fp, vp]
+        L.pd_solve_host.argtypes = [vp, vp, vp, vp, ip, fp, vp]
+        L.pd_set_weight.argtypes = [vp, vp]
+        L.pd_set_steps.argtypes = [vp, fp, fp, fp, fp]
+        L.pd_set_option.argtypes = [vp, ip, ip]
+        L.pd_get_stats.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+        L.pd_get_stats_host.argtypes = [vp, vp, vp, vp, vp]
+        L.pd_last_launch_count.argtypes = [vp]
+        L.pd_destroy.argtypes = [vp]
+        L.pd_strerror.argtypes = [ip]
+        L.pd_strerror.restype = C.c_char_p
+        for name in SYMBOLS:
+            if name != "pd_strerror":
+                getattr(L, name).restype = ip
+        _lib = L
+    return _lib
+
+
+def strerror(code):
+    return lib().pd_strerror(code).decode()
+
+
+def _check(code):
+    if code != OK:
+        raise PdError(code, strerror(code))
+
+
+def _ptr(t):
+    """Raw device pointer of a torch tensor (or None)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous() or t.dtype.__str__() != "torch.float32":
+        raise ValueError("expected a contiguous float32 CUDA tensor")
+    if t.data_ptr() % 16:
+        raise ValueError("tensor must be 16-byte aligned")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream_handle(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return C.c_void_p(stream)
+    return C.c_void_p(stream.cuda_stream)
+
+
+class Plan:
+    """pd_plan(nx, ny, batch, B0_dir, lambda, sigma, tau, theta) -- owns the device workspace."""
+
+    def __init__(self, nx, ny, batch, b0_dir=B0_Y, lambda_=0.01, sigma=0.25, tau=0.25, theta=1.0):
+        self._h = C.c_void_p()
+        self.nx, self.ny, self.batch = nx, ny, batch
+        self._mask_shared = 0
+        self._keep = None
+        _check(lib().pd_plan(C.byref(self._h), nx, ny, batch, b0_dir, lambda_, sigma, tau, theta))
+
+    def set_option(self, key, value):
+        _check(lib().pd_set_option(self._h, key, value))
+        if key == OPT_MASK_SHARED:
+            self._mask_shared = value
+
+    def set_steps(self, lambda_, sigma, tau, theta=1.0):
+        _check(lib().pd_set_steps(self._h, lambda_, sigma, tau, theta))
+
+    def set_weight(self, weight):
+        if weight is not None and weight.numel() != self.batch * self.ny * self.nx:
+            raise ValueError("weight must be [batch][ny][nx]")
+        self._keep = weight
+        _check(lib().pd_set_weight(self._h, _ptr(weight)))
+
+    def solve(self, field, mask, chi_out, max_iters, tol=0.0, stream=None):
+        """pd_solve: device tensors [batch][ny][nx] float32; enqueues on `stream` (default: torch's current stream)."""
+        n = self.batch * self.ny * self.nx
+        if field.numel() != n or chi_out.numel() != n:
+            raise ValueError("field and chi_out must be [batch][ny][nx]")
+        if mask is not None and mask.numel() != (self.ny * self.nx if self._mask_shared else n):
+            raise ValueError("mask has the wrong number of elements")
+        _check(lib().pd_solve(self._h, _ptr(field), _ptr(mask), _ptr(chi_out), int(max_iters), float(tol),
+                              _stream_handle(stream)))
+        return chi_out
+
+    def solve_host(self, field, mask, chi_out, max_iters, tol=0.0, stream=None):
+        """pd_solve_host: numpy float32 arrays (or pinned torch CPU tensors); H2D + solve + D2H + stream sync."""
+        def hp(a):
+            if a is None:
+                return None
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.float32 and a.flags["C_CONTIGUOUS"]
+                return C.c_void_p(a.ctypes.data)
+            assert a.dtype.__str__() == "torch.float32" and a.is_contiguous() and not a.is_cuda
+            return C.c_void_p(a.data_ptr())
+        _check(lib().pd_solve_host(self._h, hp(field), hp(mask), hp(chi_out), int(max_iters), float(tol),
+                                   _stream_handle(stream)))
+        return chi_out
+
+    def stats(self, stream=None):
+        """pd_get_stats_host: (iters_done int32[batch], relgap float32[batch], relres float32[batch]) on the host."""
+        it = np.empty(self.batch, np.int32)
+        gap = np.empty(self.batch, np.float32)
+        res = np.empty(self.batch, np.float32)
+        _check(lib().pd_get_stats_host(self._h, C.c_void_p(it.ctypes.data), C.c_void_p(gap.ctypes.data),
+                                       C.c_void_p(res.ctypes.data), _stream_handle(stream)))
+        return it, gap, res
+
+    def stats_device_ptrs(self):
+        """pd_get_stats: raw device pointers (iters_done, relgap, relres)."""
+        a, b, c = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _check(lib().pd_get_stats(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return a.value, b.value, c.value
+
+    @property
+    def last_launch_count(self):
+        return lib().pd_last_launch_count(self._h)
+
+    def destroy(self):
+        if self._h:
+            lib().pd_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

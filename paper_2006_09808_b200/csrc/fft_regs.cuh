@@ -1,0 +1,141 @@
+// fft_regs.cuh -- register-resident complex FFT building blocks for sm_100a.
+//
+// A length-N line (N in {64,128,256,512}) is transformed by T = N/E cooperating threads that each
+// hold E points in registers: one in-register DFT of size E, a twiddle multiply, ONE exchange
+// through shared memory, and E/T in-register DFTs of size T.  Input and output use the same
+// thread<->index map (thread j holds the points j + T*m, m = 0..E-1), so a forward and an inverse
+// transform chain without any extra shuffle (used for F^-1 D F).
+//
+// Only the forward (exp(-i...)) transform exists; the inverse is obtained by swapping re/im before
+// and after, which is a register renaming.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace pdk {
+
+template <int N> struct FftCfg;
+template <> struct FftCfg<64>  { static constexpr int E = 8,  T = 8;  };
+template <> struct FftCfg<128> { static constexpr int E = 16, T = 8;  };
+template <> struct FftCfg<256> { static constexpr int E = 16, T = 16; };
+template <> struct FftCfg<512> { static constexpr int E = 32, T = 16; };
+
+// cos(2*pi*i/32), sin(2*pi*i/32), i = 0..15, as literals so that they fold after unrolling.
+__device__ __forceinline__ float cos32(int i) {
+    switch (i) {
+        case 0: return 1.0f;
+        case 1: return 0.98078528040323044913f;
+        case 2: return 0.92387953251128675613f;
+        case 3: return 0.83146961230254523708f;
+        case 4: return 0.70710678118654752440f;
+        case 5: return 0.55557023301960222474f;
+        case 6: return 0.38268343236508977173f;
+        case 7: return 0.19509032201612826785f;
+        case 8: return 0.0f;
+        case 9: return -0.19509032201612826785f;
+        case 10: return -0.38268343236508977173f;
+        case 11: return -0.55557023301960222474f;
+        case 12: return -0.70710678118654752440f;
+        case 13: return -0.83146961230254523708f;
+        case 14: return -0.92387953251128675613f;
+        default: return -0.98078528040323044913f;
+    }
+}
+__device__ __forceinline__ float sin32(int i) { return cos32(i < 8 ? 8 - i : i - 8); }  // sin(t) = cos(pi/2 - t)
+
+// d * exp(-2*pi*i*k/R), 0 <= k < R/2, k known after unrolling.
+template <int R>
+__device__ __forceinline__ float2 twiddle_mul(float2 d, int k) {
+    constexpr float C8 = 0.70710678118654752440f;
+    if (k == 0) return d;
+    if (4 * k == R) return make_float2(d.y, -d.x);
+    if (8 * k == R) return make_float2(C8 * (d.x + d.y), C8 * (d.y - d.x));
+    if (8 * k == 3 * R) return make_float2(C8 * (d.y - d.x), -C8 * (d.x + d.y));
+    const int i = k * (32 / R);  // angle index on the 32-point circle, in (0,16)
+    const float c = cos32(i), s = sin32(i);
+    return make_float2(fmaf(d.y, s, d.x * c), fmaf(-d.x, s, d.y * c));
+}
+
+// Radix-2 decimation-in-frequency on v[OFF..OFF+R): leaves X[k] at bit-reversed position.
+template <int R, int OFF>
+struct Dif {
+    template <int E>
+    static __device__ __forceinline__ void run(float2 (&v)[E]) {
+        constexpr int H = R / 2;
+#pragma unroll
+        for (int k = 0; k < H; ++k) {
+            const float2 a = v[OFF + k], b = v[OFF + k + H];
+            v[OFF + k] = make_float2(a.x + b.x, a.y + b.y);
+            v[OFF + k + H] = twiddle_mul<R>(make_float2(a.x - b.x, a.y - b.y), k);
+        }
+        Dif<H, OFF>::run(v);
+        Dif<H, OFF + H>::run(v);
+    }
+};
+template <int OFF>
+struct Dif<1, OFF> {
+    template <int E>
+    static __device__ __forceinline__ void run(float2 (&)[E]) {}
+};
+
+__host__ __device__ constexpr int bit_reverse(int k, int R) {
+    int r = 0;
+    for (int b = 1; b < R; b <<= 1) {
+        r = (r << 1) | (k & 1);
+        k >>= 1;
+    }
+    return r;
+}
+
+// In-register forward DFT of size R, natural order in and out (the permutation is register renaming).
+template <int R>
+__device__ __forceinline__ void dft_reg(float2 (&v)[R]) {
+    Dif<R, 0>::run(v);
+    float2 t[R];
+#pragma unroll
+    for (int k = 0; k < R; ++k) t[k] = v[bit_reverse(k, R)];
+#pragma unroll
+    for (int k = 0; k < R; ++k) v[k] = t[k];
+}
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 w) {
+    return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.x, w.y, a.y * w.x));
+}
+
+// Per-thread inter-stage twiddles W_N^(j*k2), k2 = 1..E-1 (index 0 unused), from the plan's double-precision table.
+template <int N>
+struct Twiddles {
+    static constexpr int E = FftCfg<N>::E;
+    float2 w[E];
+    __device__ __forceinline__ void load(const float2 *__restrict__ table, int j) {
+#pragma unroll
+        for (int k = 1; k < E; ++k) w[k] = __ldg(table + ((j * k) & (N - 1)));
+        w[0] = make_float2(1.f, 0.f);
+    }
+};
+
+// Cooperative forward FFT of one length-N line held by T threads (thread j: points j + T*m).
+//   sm : this line's exchange region, E rows of LD float2 (row k2, column j)
+//   SYNC: functor that synchronises the T threads of the line (and orders their shared-memory accesses)
+template <int N, int LD, class Sync>
+__device__ __forceinline__ void fft_line(float2 (&v)[FftCfg<N>::E], float2 *sm, int j, const Twiddles<N> &tw,
+                                         Sync sync) {
+    constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, C = E / T;
+    dft_reg<E>(v);  // over n2: Y[j][k2]
+#pragma unroll
+    for (int k = 1; k < E; ++k) v[k] = cmul(v[k], tw.w[k]);
+    sync();  // earlier readers of sm are done
+#pragma unroll
+    for (int k = 0; k < E; ++k) sm[k * LD + j] = v[k];
+    sync();
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+        float2 w[T];
+#pragma unroll
+        for (int n = 0; n < T; ++n) w[n] = sm[(j + T * c) * LD + n];
+        dft_reg<T>(w);  // over n1: X[E*k1 + (j + T*c)] = X[j + T*(C*k1 + c)]
+#pragma unroll
+        for (int k1 = 0; k1 < T; ++k1) v[C * k1 + c] = w[k1];
+    }
+}
+
+}  // namespace pdk

@@ -1,0 +1,361 @@
+// pd_api.cu -- host side of the C ABI declared in include/pd.h: plan construction (dipole table, twiddle
+// tables, workspace), launch sequencing of the PD iteration on a caller-provided stream.
+// No CPU fallback exists: every arithmetic step of the path runs in the kernels of pd_streaming.cuh.
+#include "../../include/pd.h"
+#include "pd_streaming.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using pdk::SolveArgs;
+
+namespace {
+
+thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char *where) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error at %s: %s", where, cudaGetErrorString(e));
+    return PD_ECUDA;
+}
+#define PD_CUDA(call)                                          \
+    do {                                                       \
+        cudaError_t e_ = (call);                               \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);    \
+    } while (0)
+
+bool size_ok(int n) { return n == 64 || n == 128 || n == 256 || n == 512; }
+
+constexpr double kNormBound = 4.0 / 9.0 + 8.0;  // ||K_full||^2 <= max|D|^2 + ||G||^2 = 4/9 + 8 for W = M = 1
+
+}  // namespace
+
+struct pd_plan_s {
+    int nx, ny, batch, npairs, b0_dir;
+    // user-facing parameters (as given) and the effective ones of the rescaled problem (R2)
+    float lambda_user, sigma_user, tau_user, theta;
+    int tv_mode, lambda_conv, variant, check_every, mask_shared, unsafe_steps;
+    const float *weight;
+    // device tables and workspace
+    float *Dtab;
+    float2 *tw_row, *tw_col;
+    float *chibar, *p, *qx, *qy;
+    float2 *Z;
+    int *stop_iter, *iters_done;
+    float *P0, *relgap, *relres, *gap_part, *res_part;
+    int nparts;
+    // host-buffer entry point staging
+    float *h_field, *h_mask, *h_chi;
+    int last_launches;
+    int device;
+};
+
+namespace {
+
+template <typename T>
+int dev_alloc(T **ptr, size_t count) {
+    cudaError_t e = cudaMalloc((void **)ptr, count * sizeof(T));
+    if (e == cudaErrorMemoryAllocation) {
+        cudaGetLastError();
+        *ptr = nullptr;
+        return PD_ENOMEM;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc");
+    return PD_OK;
+}
+
+int check_params(float lambda, float sigma, float tau, float theta, bool unsafe) {
+    if (!(lambda >= 0.f) || !(theta >= 0.f && theta <= 1.f) || std::isnan(sigma) || std::isnan(tau)) return PD_EINVAL;
+    if (sigma > 0.f && tau > 0.f && !unsafe && (double)sigma * (double)tau * kNormBound >= 1.0) return PD_ESTEP;
+    return PD_OK;
+}
+
+// Effective (alpha, sigma, tau) of the problem the kernels iterate (convention B); convention A is the exact
+// rescaling A(lambda, sigma, tau) == B(1/lambda, sigma/lambda, tau*lambda) (R2, oracle pin P9).
+void effective_params(const pd_plan_s *p, float *alpha, float *sigma, float *tau) {
+    float s = p->sigma_user, t = p->tau_user;
+    if (!(s > 0.f) || !(t > 0.f)) s = t = (float)(1.0 / std::sqrt(kNormBound));
+    if (p->lambda_conv == PD_LAMBDA_DATA) {
+        *alpha = 1.0f / p->lambda_user;
+        *sigma = s / p->lambda_user;
+        *tau = t * p->lambda_user;
+    } else {
+        *alpha = p->lambda_user;
+        *sigma = s;
+        *tau = t;
+    }
+}
+
+void build_dipole(std::vector<float> &D, int nx, int ny, int b0_dir) {
+    // D(kx,ky) = 1/3 - k_b^2/(kx^2+ky^2), D(0,0)=0, kx = fi/nx, ky = fj/ny (BASELINE.json north_star; R6);
+    // the 1/(nx*ny) of the inverse transform is folded in.
+    const double scale = 1.0 / ((double)nx * (double)ny);
+    for (int jy = 0; jy < ny; ++jy) {
+        const double ky = (double)(jy < ny / 2 ? jy : jy - ny) / (double)ny;
+        for (int ix = 0; ix < nx; ++ix) {
+            const double kx = (double)(ix < nx / 2 ? ix : ix - nx) / (double)nx;
+            const double k2 = kx * kx + ky * ky;
+            const double kb = (b0_dir == PD_B0_Y) ? ky : kx;
+            const double d = (ix == 0 && jy == 0) ? 0.0 : 1.0 / 3.0 - kb * kb / k2;
+            D[(size_t)jy * nx + ix] = (float)(d * scale);
+        }
+    }
+}
+
+void build_twiddles(std::vector<float2> &tw, int n) {
+    const double pi = 3.14159265358979323846264338327950288;
+    for (int k = 0; k < n; ++k) {
+        const double ang = -2.0 * pi * (double)k / (double)n;
+        tw[k] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+    }
+}
+
+template <int NX>
+void launch_dual(const SolveArgs &a, int n, cudaStream_t st) {
+    dim3 grid(a.ny / pdk::RowCfg<NX>::G, a.npairs);
+    pdk::dual_rows_kernel<NX><<<grid, pdk::RowCfg<NX>::THREADS, 0, st>>>(a, n);
+}
+template <int NX>
+void launch_primal(const SolveArgs &a, int n, cudaStream_t st) {
+    dim3 grid(a.ny / pdk::RowCfg<NX>::G, a.npairs);
+    pdk::primal_rows_kernel<NX><<<grid, pdk::RowCfg<NX>::THREADS, 0, st>>>(a, n);
+}
+template <int NY>
+void launch_cols(const SolveArgs &a, int n, int fin, cudaStream_t st) {
+    dim3 grid(a.nx / pdk::ColCfg<NY>::COLS, a.npairs);
+    pdk::dipole_cols_kernel<NY><<<grid, pdk::ColCfg<NY>::THREADS, pdk::ColCfg<NY>::SMEM_BYTES, st>>>(a, n, fin);
+}
+
+#define PD_DISPATCH(n, F, ...)                    \
+    switch (n) {                                  \
+        case 64: F<64>(__VA_ARGS__); break;       \
+        case 128: F<128>(__VA_ARGS__); break;     \
+        case 256: F<256>(__VA_ARGS__); break;     \
+        default: F<512>(__VA_ARGS__); break;      \
+    }
+
+template <int NY>
+cudaError_t set_col_smem() {
+    return cudaFuncSetAttribute(pdk::dipole_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                pdk::ColCfg<NY>::SMEM_BYTES);
+}
+
+}  // namespace
+
+extern "C" {
+
+int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda, float sigma, float tau, float theta) {
+    if (!out) return PD_EINVAL;
+    *out = nullptr;
+    if (batch < 1 || (B0_dir != PD_B0_X && B0_dir != PD_B0_Y)) return PD_EINVAL;
+    if (!size_ok(nx) || !size_ok(ny)) return PD_ESIZE;
+    int rc = check_params(lambda, sigma, tau, theta, false);
+    if (rc != PD_OK) return rc;
+
+    pd_plan_s *p = new (std::nothrow) pd_plan_s;
+    if (!p) return PD_ENOMEM;
+    std::memset(p, 0, sizeof(*p));
+    p->nx = nx; p->ny = ny; p->batch = batch; p->npairs = (batch + 1) / 2; p->b0_dir = B0_dir;
+    p->lambda_user = lambda; p->sigma_user = sigma; p->tau_user = tau; p->theta = theta;
+    p->check_every = 1;
+    {
+        cudaError_t e = cudaGetDevice(&p->device);
+        if (e != cudaSuccess) { delete p; return cuda_fail(e, "cudaGetDevice"); }
+    }
+    const int rows_per_cta = (nx == 64 || nx == 128) ? 16 : 8;  // = RowCfg<nx>::G
+    p->nparts = ny / rows_per_cta;
+
+    const size_t P = (size_t)nx * ny, BP = P * (size_t)batch;
+#define PD_TRY(expr) do { rc = (expr); if (rc != PD_OK) { pd_destroy(p); return rc; } } while (0)
+    PD_TRY(dev_alloc(&p->Dtab, P));
+    PD_TRY(dev_alloc(&p->tw_row, (size_t)nx));
+    PD_TRY(dev_alloc(&p->tw_col, (size_t)ny));
+    PD_TRY(dev_alloc(&p->chibar, BP));
+    PD_TRY(dev_alloc(&p->p, BP));
+    PD_TRY(dev_alloc(&p->qx, BP));
+    PD_TRY(dev_alloc(&p->qy, BP));
+    PD_TRY(dev_alloc(&p->Z, P * (size_t)p->npairs));
+    PD_TRY(dev_alloc(&p->stop_iter, (size_t)batch + 1));
+    PD_TRY(dev_alloc(&p->iters_done, (size_t)batch));
+    PD_TRY(dev_alloc(&p->P0, (size_t)batch));
+    PD_TRY(dev_alloc(&p->relgap, (size_t)batch));
+    PD_TRY(dev_alloc(&p->relres, (size_t)batch));
+    PD_TRY(dev_alloc(&p->gap_part, (size_t)batch * p->nparts));
+    PD_TRY(dev_alloc(&p->res_part, (size_t)batch * p->nparts * 2));
+#undef PD_TRY
+    {
+        std::vector<float> D(P);
+        build_dipole(D, nx, ny, B0_dir);
+        std::vector<float2> twr(nx), twc(ny);
+        build_twiddles(twr, nx);
+        build_twiddles(twc, ny);
+        cudaError_t e = cudaMemcpy(p->Dtab, D.data(), P * sizeof(float), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(p->tw_row, twr.data(), nx * sizeof(float2), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(p->tw_col, twc.data(), ny * sizeof(float2), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemset(p->iters_done, 0, batch * sizeof(int));
+        if (e == cudaSuccess) e = cudaMemset(p->relgap, 0, batch * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemset(p->relres, 0, batch * sizeof(float));
+        if (e == cudaSuccess) e = set_col_smem<64>();
+        if (e == cudaSuccess) e = set_col_smem<128>();
+        if (e == cudaSuccess) e = set_col_smem<256>();
+        if (e == cudaSuccess) e = set_col_smem<512>();
+        if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "plan table upload"); }
+    }
+    *out = p;
+    return PD_OK;
+}
+
+int pd_set_weight(pd_plan_t p, const float *W) {
+    if (!p) return PD_EINVAL;
+    p->weight = W;
+    return PD_OK;
+}
+
+int pd_set_steps(pd_plan_t p, float lambda, float sigma, float tau, float theta) {
+    if (!p) return PD_EINVAL;
+    int rc = check_params(lambda, sigma, tau, theta, p->unsafe_steps != 0);
+    if (rc != PD_OK) return rc;
+    p->lambda_user = lambda; p->sigma_user = sigma; p->tau_user = tau; p->theta = theta;
+    return PD_OK;
+}
+
+int pd_set_option(pd_plan_t p, int key, int value) {
+    if (!p) return PD_EINVAL;
+    switch (key) {
+        case PD_OPT_TV_MODE:
+            if (value != PD_TV_ISO && value != PD_TV_ANISO) return PD_EINVAL;
+            p->tv_mode = value; return PD_OK;
+        case PD_OPT_LAMBDA_CONV:
+            if (value != PD_LAMBDA_REG && value != PD_LAMBDA_DATA) return PD_EINVAL;
+            p->lambda_conv = value; return PD_OK;
+        case PD_OPT_VARIANT:
+            if (value == PD_VARIANT_RESIDENT) return PD_EVARIANT;  // not built in this round: fail loudly
+            if (value != PD_VARIANT_AUTO && value != PD_VARIANT_STREAMING) return PD_EINVAL;
+            p->variant = value; return PD_OK;
+        case PD_OPT_CHECK_EVERY:
+            if (value < 1) return PD_EINVAL;
+            p->check_every = value; return PD_OK;
+        case PD_OPT_MASK_SHARED:
+            if (value != 0 && value != 1) return PD_EINVAL;
+            p->mask_shared = value; return PD_OK;
+        case PD_OPT_UNSAFE_STEPS:
+            if (value != 0 && value != 1) return PD_EINVAL;
+            p->unsafe_steps = value; return PD_OK;
+        default: return PD_EINVAL;
+    }
+}
+
+int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+             void *cuda_stream) {
+    if (!p || !field || !chi_out || max_iters < 0) return PD_EINVAL;
+    if (p->lambda_conv == PD_LAMBDA_DATA && !(p->lambda_user > 0.f)) return PD_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
+
+    SolveArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.nx = p->nx; a.ny = p->ny; a.batch = p->batch; a.npairs = p->npairs;
+    a.field = field; a.mask = mask; a.weight = p->weight;
+    a.mask_bstride = p->mask_shared ? 0 : (long long)P;
+    a.chi = chi_out; a.chibar = p->chibar; a.p = p->p; a.qx = p->qx; a.qy = p->qy; a.Z = p->Z;
+    a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
+    a.stop_iter = p->stop_iter; a.P0 = p->P0; a.relgap = p->relgap; a.relres = p->relres;
+    a.gap_part = p->gap_part; a.res_part = p->res_part; a.nparts = p->nparts;
+    effective_params(p, &a.alpha, &a.sigma, &a.tau);
+    a.theta = p->theta;
+    a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
+    a.tol = tol;
+    a.aniso = p->tv_mode == PD_TV_ANISO;
+    a.check_every = p->check_every;
+    a.max_iters = max_iters;
+
+    int launches = 0;
+    // chi_0 = p_0 = q_0 = 0, chibar_0 = chi_0; the spectrum of chibar_0 is 0 as well
+    PD_CUDA(cudaMemsetAsync(chi_out, 0, BP * sizeof(float), st));
+    PD_CUDA(cudaMemsetAsync(p->chibar, 0, BP * sizeof(float), st));
+    PD_CUDA(cudaMemsetAsync(p->p, 0, BP * sizeof(float), st));
+    PD_CUDA(cudaMemsetAsync(p->qx, 0, BP * sizeof(float), st));
+    PD_CUDA(cudaMemsetAsync(p->qy, 0, BP * sizeof(float), st));
+    PD_CUDA(cudaMemsetAsync(p->Z, 0, P * (size_t)p->npairs * sizeof(float2), st));
+    PD_CUDA(cudaMemsetAsync(p->stop_iter, 0, ((size_t)p->batch + 1) * sizeof(int), st));
+    pdk::init_slices_kernel<<<p->batch, 256, 0, st>>>(a);
+    ++launches;
+    for (int n = 0; n < max_iters; ++n) {
+        if (n > 0) { PD_DISPATCH(p->ny, launch_cols, a, n, 0, st); ++launches; }   // K1 column pass (chibar_0 = 0)
+        PD_DISPATCH(p->nx, launch_dual, a, n, st); ++launches;
+        PD_DISPATCH(p->ny, launch_cols, a, n, 1, st); ++launches;                 // K2 column pass + gap / stop flag
+        PD_DISPATCH(p->nx, launch_primal, a, n, st); ++launches;
+    }
+    pdk::finish_slices_kernel<<<(p->batch + 127) / 128, 128, 0, st>>>(a, p->iters_done);
+    ++launches;
+    PD_CUDA(cudaGetLastError());
+    p->last_launches = launches;
+    return PD_OK;
+}
+
+int pd_solve_host(pd_plan_t p, const float *field_host, const float *mask_host, float *chi_out_host, int max_iters,
+                  float tol, void *cuda_stream) {
+    if (!p || !field_host || !chi_out_host || max_iters < 0) return PD_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
+    const size_t mask_count = p->mask_shared ? P : BP;
+    int rc;
+    if (!p->h_field && (rc = dev_alloc(&p->h_field, BP)) != PD_OK) return rc;
+    if (!p->h_chi && (rc = dev_alloc(&p->h_chi, BP)) != PD_OK) return rc;
+    if (mask_host && !p->h_mask && (rc = dev_alloc(&p->h_mask, BP)) != PD_OK) return rc;
+    PD_CUDA(cudaMemcpyAsync(p->h_field, field_host, BP * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (mask_host) PD_CUDA(cudaMemcpyAsync(p->h_mask, mask_host, mask_count * sizeof(float), cudaMemcpyHostToDevice, st));
+    rc = pd_solve(p, p->h_field, mask_host ? p->h_mask : nullptr, p->h_chi, max_iters, tol, cuda_stream);
+    if (rc != PD_OK) return rc;
+    PD_CUDA(cudaMemcpyAsync(chi_out_host, p->h_chi, BP * sizeof(float), cudaMemcpyDeviceToHost, st));
+    PD_CUDA(cudaStreamSynchronize(st));
+    return PD_OK;
+}
+
+int pd_get_stats(pd_plan_t p, const int **iters_done, const float **relgap, const float **relres) {
+    if (!p) return PD_EINVAL;
+    if (iters_done) *iters_done = p->iters_done;
+    if (relgap) *relgap = p->relgap;
+    if (relres) *relres = p->relres;
+    return PD_OK;
+}
+
+int pd_get_stats_host(pd_plan_t p, int *iters_done_host, float *relgap_host, float *relres_host, void *cuda_stream) {
+    if (!p) return PD_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)p->batch;
+    if (iters_done_host) PD_CUDA(cudaMemcpyAsync(iters_done_host, p->iters_done, n * sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (relgap_host) PD_CUDA(cudaMemcpyAsync(relgap_host, p->relgap, n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (relres_host) PD_CUDA(cudaMemcpyAsync(relres_host, p->relres, n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    PD_CUDA(cudaStreamSynchronize(st));
+    return PD_OK;
+}
+
+int pd_last_launch_count(pd_plan_t p) { return p ? p->last_launches : PD_EINVAL; }
+
+int pd_destroy(pd_plan_t p) {
+    if (!p) return PD_EINVAL;
+    void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->chibar, p->p, p->qx, p->qy, p->Z, p->stop_iter, p->iters_done,
+                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi};
+    for (void *q : ptrs)
+        if (q) cudaFree(q);
+    delete p;
+    return PD_OK;
+}
+
+const char *pd_strerror(int code) {
+    switch (code) {
+        case PD_OK: return "success";
+        case PD_EINVAL: return "invalid argument";
+        case PD_ESIZE: return "nx and ny must each be one of 64, 128, 256, 512";
+        case PD_ESTEP: return "sigma*tau*(4/9+8) >= 1: step sizes violate the convergence bound";
+        case PD_ENOMEM: return "out of device memory";
+        case PD_ECUDA: return g_cuda_err;
+        case PD_EVARIANT: return "requested variant is not available for this size";
+        default: return "unknown error code";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,235 @@
+"""GPU-vs-oracle parity through the C ABI (run on the B200 box: pytest -m gpu).
+
+Gates (BASELINE.json north_star): per-slice relative L2 of chi <= 1e-5 after 1 iteration, <= 1e-3 after the full
+iteration count; relgap within 1e-3 relative; |iters_done difference| <= 1 under tolerance stopping (R16).
+Inputs come from paper_2006_09808_b200/synth.py; expected values only from oracle/ (double precision).
+"""
+import numpy as np
+import pytest
+
+from paper_2006_09808_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_1IT = 1e-5
+TOL_FULL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def pd(torch):
+    from paper_2006_09808_b200 import binding
+    binding.lib()  # fails loudly if the extension is missing: there is no fallback
+    return binding
+
+
+def slice_rel(a, b):
+    a = a.reshape(a.shape[0], -1).astype(np.float64)
+    b = b.reshape(b.shape[0], -1).astype(np.float64)
+    den = np.maximum(np.linalg.norm(b, axis=1), 1e-300)
+    return np.linalg.norm(a - b, axis=1) / den
+
+
+def gpu_solve(torch, pd, field, mask, iters, *, lam, sigma=0.25, tau=0.25, theta=1.0, tol=0.0, weight=None, b0=1,
+              options=(), host=False):
+    batch, ny, nx = field.shape
+    plan = pd.Plan(nx, ny, batch, b0, lam, sigma, tau, theta)
+    for k, v in options:
+        plan.set_option(k, v)
+    if host:
+        chi = np.empty_like(field)
+        plan.solve_host(field, mask, chi, iters, tol)
+    else:
+        f = torch.from_numpy(field).cuda()
+        m = None if mask is None else torch.from_numpy(np.ascontiguousarray(mask)).cuda()
+        w = None if weight is None else torch.from_numpy(weight).cuda()
+        plan.set_weight(w)
+        out = torch.full_like(f, float("nan"))
+        plan.solve(f, m, out, iters, tol)
+        torch.cuda.synchronize()
+        chi = out.cpu().numpy()
+    it, gap, res = plan.stats()
+    launches = plan.last_launch_count
+    plan.destroy()
+    return {"chi": chi, "iters_done": it, "relgap": gap, "relres": res, "launches": launches}
+
+
+@pytest.mark.parametrize("ny,nx", [(64, 64), (128, 128), (256, 256), (512, 512), (64, 256), (512, 128), (128, 64)])
+def test_one_iteration_all_sizes(torch, pd, oracle, ny, nx):
+    case = synth.random_case(nx, ny, 3, seed=nx + ny, with_mask=True, with_weight=True)   # odd batch: ragged last pair
+    g = gpu_solve(torch, pd, case["field"], case["mask"], 1, lam=0.05, weight=case["weight"])
+    o = oracle.solve(case["field"], case["mask"], case["weight"], lambda_=0.05, sigma=0.25, tau=0.25, max_iters=1)
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], o["relgap"][:, 0], rtol=1e-4)
+    assert np.all(g["iters_done"] == 1)
+
+
+@pytest.mark.parametrize("iters", [2, 3, 7])
+def test_few_iterations_exercise_q_and_divergence(torch, pd, oracle, iters):
+    case = synth.random_case(128, 64, 4, seed=77, with_mask=True, with_weight=True)
+    g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.5, weight=case["weight"])
+    o = oracle.solve(case["field"], case["mask"], case["weight"], lambda_=0.5, sigma=0.25, tau=0.25, max_iters=iters)
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-3)
+    assert np.allclose(g["relres"], o["relres"][:, iters - 1], rtol=1e-3)
+
+
+def test_config0_full(torch, pd, oracle):
+    d = synth.generate(0)
+    cfg = d["cfg"]
+    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam)
+    o = oracle.solve(d["field"], d["mask"], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau, max_iters=cfg.iters)
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_FULL
+    assert slice_rel(g["chi"], o["chi"]).max() < 2e-5   # what fp32 actually achieves
+    assert np.allclose(g["relgap"], o["relgap"][:, -1], rtol=1e-3)
+    assert np.allclose(g["relres"], o["relres"][:, -1], rtol=1e-3)
+    assert g["iters_done"][0] == 100
+
+
+def test_config1_full(torch, pd, oracle):
+    d = synth.generate(1)
+    cfg = d["cfg"]
+    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam)
+    o = oracle.solve(d["field"], d["mask"], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau, max_iters=cfg.iters,
+                     want_hist=True)
+    r = slice_rel(g["chi"], o["chi"])
+    assert r.max() < TOL_FULL and r.max() < 5e-5
+    assert np.allclose(g["relgap"], o["relgap"][:, -1], rtol=1e-3)
+
+
+def _sampled_full_config(torch, pd, oracle, cid, sample, host=False):
+    """Run the GPU on the FULL config (the launch configuration bench.py times); oracle on sampled batch entries."""
+    d = synth.generate(cid)
+    cfg = d["cfg"]
+    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam, tol=cfg.tol, host=host)
+    assert np.all(np.isfinite(g["chi"]))
+    # property that holds at any size: every iterate has zero mean (DESIGN.md pin P7)
+    means = np.abs(g["chi"].reshape(cfg.batch, -1).astype(np.float64).mean(axis=1))
+    assert means.max() < 1e-3
+    for b in sample:
+        o = oracle.solve(d["field"][b], d["mask"][b], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau,
+                         max_iters=int(g["iters_done"][b]) if cfg.tol > 0 else cfg.iters)
+        assert slice_rel(g["chi"][b:b + 1], o["chi"]).max() < TOL_FULL, b
+        assert abs(g["relgap"][b] / o["relgap"][0, -1] - 1) < 1e-3
+        if cfg.tol > 0:   # the oracle's own stopping point may differ by one iteration at most (R16)
+            ost = oracle.solve(d["field"][b], d["mask"][b], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau,
+                               max_iters=cfg.iters, tol=cfg.tol, want_hist=False)
+            assert abs(int(ost["iters_done"][0]) - int(g["iters_done"][b])) <= 1
+    return d, g
+
+
+def test_config2_full_sampled(torch, pd, oracle):
+    _sampled_full_config(torch, pd, oracle, 2, [0, 37, 63])
+
+
+def test_config3_full_sampled_through_host_entry(torch, pd, oracle):
+    d, g = _sampled_full_config(torch, pd, oracle, 3, [5, 1023], host=True)
+    assert np.all(g["iters_done"] == 200)
+
+
+def test_northstar_stack_sampled(torch, pd, oracle):
+    _sampled_full_config(torch, pd, oracle, 5, [0, 127])
+
+
+def test_config4_full_tolerance_stop_sampled(torch, pd, oracle):
+    d, g = _sampled_full_config(torch, pd, oracle, 4, [3, 200])
+    assert g["iters_done"].min() > 40 and g["iters_done"].max() < 140
+    assert np.all(g["relgap"] < 1e-4)
+
+
+def test_options_aniso_dataconv_sharedmask_b0x_theta(torch, pd, oracle):
+    case = synth.random_case(64, 128, 2, seed=5, with_mask=True)
+    f, m = case["field"], case["mask"]
+    g = gpu_solve(torch, pd, f, m, 20, lam=0.3, options=[(pd.OPT_TV_MODE, pd.TV_ANISO)])
+    o = oracle.solve(f, m, lambda_=0.3, sigma=0.25, tau=0.25, max_iters=20, tv_mode=oracle.TV_ANISO)
+    assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
+    assert np.allclose(g["relgap"], o["relgap"][:, -1], rtol=1e-3)
+    g = gpu_solve(torch, pd, f, m, 20, lam=40.0, options=[(pd.OPT_LAMBDA_CONV, pd.LAMBDA_DATA)])
+    o = oracle.solve(f, m, lambda_=40.0, sigma=0.25, tau=0.25, max_iters=20, lambda_conv=oracle.LAMBDA_DATA)
+    assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
+    assert np.allclose(g["relgap"], o["relgap"][:, -1], rtol=1e-3)
+    g = gpu_solve(torch, pd, f, m[0], 20, lam=0.3, options=[(pd.OPT_MASK_SHARED, 1)])
+    o = oracle.solve(f, np.stack([m[0], m[0]]), lambda_=0.3, sigma=0.25, tau=0.25, max_iters=20)
+    assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
+    g = gpu_solve(torch, pd, f, None, 20, lam=0.3, b0=0, theta=0.5)
+    o = oracle.solve(f, None, lambda_=0.3, sigma=0.25, tau=0.25, theta=0.5, max_iters=20, b0_dir=oracle.B0_X)
+    assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
+    g = gpu_solve(torch, pd, f, m, 20, lam=0.3, sigma=-1.0, tau=-1.0)          # automatic steps
+    s = 1.0 / np.sqrt(8 + 4 / 9)
+    o = oracle.solve(f, m, lambda_=0.3, sigma=np.float32(s), tau=np.float32(s), max_iters=20)
+    assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
+    g = gpu_solve(torch, pd, f, m, 20, lam=0.0)                                  # alpha = 0: q stays 0 (R13)
+    o = oracle.solve(f, m, lambda_=0.0, sigma=0.25, tau=0.25, max_iters=20)
+    assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
+
+
+def test_degenerate_cases(torch, pd, oracle):
+    f = synth.random_case(64, 64, 3, seed=9)["field"]
+    f[1] = 0.0                                                                # an all-zero slice inside an active pair
+    g = gpu_solve(torch, pd, f, None, 15, lam=0.1, tol=1e-9)
+    assert g["iters_done"].tolist() == [15, 0, 15] and np.all(g["chi"][1] == 0)
+    o = oracle.solve(f, None, lambda_=0.1, sigma=0.25, tau=0.25, max_iters=15)
+    assert slice_rel(g["chi"][[0, 2]], o["chi"][[0, 2]]).max() < 2e-5
+    g = gpu_solve(torch, pd, f, None, 15, lam=0.1)                            # tol <= 0: runs N no-op iterations
+    assert g["iters_done"].tolist() == [15, 15, 15] and np.all(g["chi"][1] == 0) and g["relgap"][1] == 0
+    g = gpu_solve(torch, pd, f, None, 0, lam=0.1)                             # max_iters = 0: chi_0 = 0
+    assert np.all(g["chi"] == 0) and np.all(g["iters_done"] == 0)
+    one = gpu_solve(torch, pd, f[:1], None, 15, lam=0.1)                      # batch 1: half-empty pair
+    assert slice_rel(one["chi"], o["chi"][:1]).max() < 2e-5
+
+
+def test_per_slice_stop_mixed_batch(torch, pd, oracle):
+    """Slices of one batch stop at different iterations; a stopped slice is frozen while its pair partner goes on."""
+    d = synth.generate(1, nslices=5)
+    f = d["field"].copy()
+    f[1] *= 1e-3          # different noise-to-signal ratios do not matter; different phantoms already differ
+    tol = 3e-4
+    g = gpu_solve(torch, pd, f, d["mask"], 300, lam=0.01, tol=tol)
+    o = oracle.solve(f, d["mask"], lambda_=0.01, sigma=0.25, tau=0.25, max_iters=300, tol=tol)
+    assert np.abs(g["iters_done"].astype(int) - o["iters_done"].astype(int)).max() <= 1
+    assert len(set(g["iters_done"].tolist())) > 1
+    for b in range(5):
+        ob = oracle.solve(f[b], d["mask"][b], lambda_=0.01, sigma=0.25, tau=0.25, max_iters=int(g["iters_done"][b]),
+                          want_hist=True)
+        assert slice_rel(g["chi"][b:b + 1], ob["chi"]).max() < TOL_FULL
+        assert abs(g["relgap"][b] / ob["relgap"][0, -1] - 1) < 1e-3
+    ge = gpu_solve(torch, pd, f, d["mask"], 300, lam=0.01, tol=tol, options=[(pd.OPT_CHECK_EVERY, 8)])
+    assert np.all(ge["iters_done"] % 8 == 0) and np.all(ge["iters_done"] >= g["iters_done"])
+
+
+def test_repeatable_and_plan_reuse(torch, pd):
+    d = synth.generate(1, nslices=4)
+    f = torch.from_numpy(d["field"]).cuda()
+    m = torch.from_numpy(d["mask"]).cuda()
+    plan = pd.Plan(128, 128, 4, 1, 0.01, 0.25, 0.25, 1.0)
+    a, b = torch.empty_like(f), torch.empty_like(f)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        plan.solve(f, m, a, 50, 1e-3)
+        plan.solve(f, m, b, 50, 1e-3)
+    s.synchronize()
+    assert torch.equal(a, b)                                                  # bitwise deterministic, stream honoured
+    it, _, _ = plan.stats(s)
+    assert it.max() <= 50
+    plan.destroy()
+
+
+def test_runtime_errors(torch, pd):
+    plan = pd.Plan(64, 64, 2)
+    f = torch.zeros(2, 64, 64, device="cuda")
+    with pytest.raises(pd.PdError) as e:
+        plan.solve(f, None, f.clone(), -1)
+    assert e.value.code == pd.EINVAL
+    with pytest.raises(pd.PdError) as e:
+        plan.set_option(pd.OPT_VARIANT, 99)
+    assert e.value.code == pd.EINVAL
+    with pytest.raises(pd.PdError) as e:
+        plan.set_steps(0.01, 0.5, 0.5)
+    assert e.value.code == pd.ESTEP
+    plan.destroy()

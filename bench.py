@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- PD slice-iterations/s and stack reconstruction time of the B200 hot path (arXiv 2006.09808).
+
+    python bench.py --gpus N --steps K --warmup W            # the CUDA path (one rank per GPU under torchrun)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands, on the host cores
+
+A "step" is one pass of the whole hot path (all iterations of the PD solve) over one
+batch of synthetic input of the named workload.  Default workload: C3 = BASELINE.json configs[3] (128 slices x 8 coil
+field maps of 256x256, 200 iterations, lambda 0.005), the largest 256x256 configuration, which fits one GPU; inputs
+(0.5 GB) and state (1.6 GB) exceed the 126 MB L2, so no explicit flush is needed between timed steps.
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the meaning of every key.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2006_09808_b200 import synth  # noqa: E402  (input generator only: holds none of the solver's arithmetic)
+
+METRIC = "pd_slice_iterations_per_s"
+UNIT = "slice-iterations/s"
+WORKLOADS = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4, "NS": 5}
+
+# Algorithmic HBM bytes per pixel and launch of each kernel class of the streaming variant:
+# what the pass must read and write once, spectra counted at 4 B/px/slice (one float2 per pixel of a slice PAIR).
+KERNEL_BYTES_PER_PX = {
+    "resident": 48.0,     # one launch = the whole path: the streaming floor per slice-ITERATION (x iterations below)
+    "dual_rows": 44.0,    # Z r4 + p rw8 + phi r4 + chibar r4 + qx rw8 + qy rw8 + M r4 + Z w4
+    "dipole_cols": 8.0,   # Z r4 + Z w4
+    "primal_rows": 32.0,  # Z r4 + chi rw8 + chibar w4 + qx r4 + qy r4 + M r4 + Z w4
+}
+PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            pk = json.load(f)
+        return float(pk["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.tmp.flush()
+        self.tmp.seek(0)
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.tmp.read().splitlines():
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 9:
+                continue
+            try:
+                sm.append(float(parts[1]))
+                mx.append(float(parts[2]))
+                power.append(float(parts[3]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        self.tmp.close()
+        os.unlink(self.tmp.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=float(max(power)))
+        return out
+
+
+def oracle_module():
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import pd_oracle  # test infrastructure; only the cpu_baseline / --impl reference legs reach this line
+    pd_oracle.lib()
+    return pd_oracle
+
+
+def time_oracle(cfg, data, nsample):
+    """The oracle as it stands (float instantiation, one thread) on the first `nsample` batch entries."""
+    orc = oracle_module()
+    t0 = time.perf_counter()
+    out = orc.solve(data["field"][:nsample], data["mask"][:nsample], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau,
+                    theta=cfg.theta, max_iters=cfg.iters, tol=cfg.tol, precision="f32", want_hist=False)
+    dt = time.perf_counter() - t0
+    return float(out["iters_done"].sum()) / dt, dt, int(out["iters_done"].sum())
+
+
+def oracle_sample_size(cfg):
+    """Batch entries giving roughly 10-30 s of single-core oracle work (about 8e-7 s per pixel-iteration measured)."""
+    per_slice = 8e-7 * cfg.nx * cfg.ny * (cfg.iters if cfg.tol <= 0 else min(cfg.iters, 80))
+    return int(max(1, min(cfg.batch, round(20.0 / per_slice))))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0   # under torchrun only rank 0 runs the reference arm
+    cid = WORKLOADS[args.workload]
+    cfg = synth.CONFIGS[cid]
+    nsample = max(1, oracle_sample_size(cfg) // 4)        # one step = a bounded sample, so K+W steps end in minutes
+    nslices = -(-nsample // cfg.ncoils)
+    data = synth.generate(cid, nslices=nslices)
+    for _ in range(args.warmup):
+        time_oracle(cfg, data, min(nsample, 1))
+    t0 = time.perf_counter()
+    its = 0
+    for _ in range(args.steps):
+        _, _, n = time_oracle(cfg, data, nsample)
+        its += n
+    dt = time.perf_counter() - t0
+    value = its / dt
+    sample = "first %d of %d batch entries of %s, all %d iterations, per step" % (nsample, cfg.batch, cfg.name, cfg.iters)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": workload_config(cfg, args.workload, cfg.batch, 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_config(cfg, name, batch_per_gpu, ngpus):
+    return {"workload": "%s: %s" % (name, cfg.name), "nx": cfg.nx, "ny": cfg.ny, "batch_per_gpu": batch_per_gpu,
+            "slices": cfg.nslices, "coils": cfg.ncoils, "iterations": cfg.iters, "tol": cfg.tol, "lambda": cfg.lam,
+            "sigma": cfg.sigma, "tau": cfg.tau, "theta": cfg.theta, "B0": cfg.b0_dir,
+            "parallelism": "batch-sharded x%d, no collective" % ngpus,
+            "l2": "inputs+state per step exceed the 126 MB L2 (no flush needed)" if batch_per_gpu * cfg.nx * cfg.ny * 32 > 2 * 126e6
+                  else "working set fits L2: a 256 MB buffer is overwritten between timed steps"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="C3", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the north-star single-coil stack timing")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2006_09808_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.lib()
+
+    cid = WORKLOADS[args.workload]
+    cfg = synth.CONFIGS[cid]
+    # weak scaling: every rank reconstructs its own stack of the workload's size (slices are independent)
+    data = synth.generate(cid, first_slice=rank * cfg.nslices)
+    batch = cfg.batch
+    P = cfg.nx * cfg.ny
+    field = torch.from_numpy(data["field"]).cuda()
+    mask = torch.from_numpy(data["mask"]).cuda()
+    chi = torch.empty_like(field)
+    b0 = binding.B0_Y if cfg.b0_dir == "y" else binding.B0_X
+    plan = binding.Plan(cfg.nx, cfg.ny, batch, b0, cfg.lam, cfg.sigma, cfg.tau, cfg.theta)
+    small = batch * P * 32 <= 2 * 126e6
+    flush = torch.empty(64 * 1024 * 1024, device="cuda") if small else None
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(nsteps, host=False, h=None):
+        """K steps bracketed by barrier+sync; device time (CUDA events on the launch stream), max over ranks."""
+        barrier()
+        total = 0.0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if flush is None:
+            e0.record()
+            for _ in range(nsteps):
+                if host:
+                    plan.solve_host(h[0], h[1], h[2], cfg.iters, cfg.tol)
+                else:
+                    plan.solve(field, mask, chi, cfg.iters, cfg.tol)
+            e1.record()
+            torch.cuda.synchronize()
+            total = e0.elapsed_time(e1)
+        else:
+            for _ in range(nsteps):   # small working set: flush L2 between steps, time each step separately
+                flush.fill_(1.0)
+                e0.record()
+                if host:
+                    plan.solve_host(h[0], h[1], h[2], cfg.iters, cfg.tol)
+                else:
+                    plan.solve(field, mask, chi, cfg.iters, cfg.tol)
+                e1.record()
+                torch.cuda.synchronize()
+                total += e0.elapsed_time(e1)
+        barrier()
+        t = torch.tensor([total], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def total_iters():
+        it, _, _ = plan.stats()
+        t = torch.tensor([float(it.sum())], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item()), it
+
+    # ---- device-resident measurement (inputs already in HBM)
+    timed(args.warmup)
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms = timed(args.steps)
+    clocks = sampler.stop() if sampler else None
+    slice_its, its_local = total_iters()
+    value = slice_its * args.steps / (ms * 1e-3)
+    launches = plan.last_launch_count * args.steps
+
+    # ---- per-kernel device time, live, same K steps with CUDA events around every launch
+    plan.set_option(binding.OPT_KERNEL_TIMING, 1)
+    ktot = {}
+    ms_evt = 0.0
+    for _ in range(args.steps):
+        ms_evt += timed(1)
+        for k, (t, c) in plan.kernel_times().items():
+            a = ktot.setdefault(k, [0.0, 0])
+            a[0] += t
+            a[1] += c
+    plan.set_option(binding.OPT_KERNEL_TIMING, 0)
+    peak, peak_src = load_peaks()
+    dom = max(KERNEL_BYTES_PER_PX, key=lambda k: ktot.get(k, [0.0, 0])[0])
+    dom_ms, dom_n = ktot[dom]
+    # units one launch processes: every active slice once; averaged over the launches of the solve (a stopped slice is
+    # skipped by later launches), = batch when no tolerance is set
+    avg_active_slices = float(its_local.sum()) / max(cfg.iters, 1)
+    bytes_per_launch = KERNEL_BYTES_PER_PX[dom] * P * avg_active_slices
+    if dom == "resident":   # a single launch runs every iteration of every slice
+        bytes_per_launch = KERNEL_BYTES_PER_PX[dom] * P * float(its_local.sum())
+    achieved = bytes_per_launch / (dom_ms / dom_n * 1e-3) / 1e9
+    ksum = sum(v[0] for v in ktot.values())
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
+                "avg_launch_us": 1e3 * dom_ms / dom_n, "share_of_step": dom_ms / ksum,
+                "kernel_ms_per_step": {k: v[0] / args.steps for k, v in ktot.items()},
+                "step_ms_with_events": ms_evt / args.steps}
+    path_bytes = PATH_FLOOR_BYTES_PER_PX * P * float(its_local.sum())
+    roofline_path = {"bound": "hbm", "what": "whole path at the 48 B/px/slice-iteration streaming floor", "unit": "GB/s",
+                     "achieved": path_bytes * args.steps / (ms * 1e-3) / 1e9 if world == 1 else path_bytes / (ms / args.steps * 1e-3) / 1e9,
+                     "peak": peak}
+    roofline_path["frac"] = roofline_path["achieved"] / peak
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), H2D and D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hf = torch.from_numpy(data["field"]).pin_memory()
+        hm = torch.from_numpy(data["mask"]).pin_memory()
+        hc = torch.empty_like(hf).pin_memory()
+        timed(1, host=True, h=(hf, hm, hc))
+        ms_h = timed(args.steps, host=True, h=(hf, hm, hc))
+        e2e = {"value": slice_its * args.steps / (ms_h * 1e-3), "unit": UNIT, "ms_per_step": ms_h / args.steps,
+               "h2d_bytes_per_step": int(hf.numel() * 4 + hm.numel() * 4), "d2h_bytes_per_step": int(hc.numel() * 4),
+               "api": "pd_solve_host (pinned host buffers)"}
+        del hf, hm, hc
+
+    # ---- north-star stack (128 slices x 256x256, one field map per slice, 200 iterations): whole-stack recon ms
+    extra = None
+    if not args.no_extra and rank == 0 and cid == 3:
+        ns = synth.CONFIGS[5]
+        f2, m2, c2 = field[::cfg.ncoils].contiguous(), mask[::cfg.ncoils].contiguous(), torch.empty_like(field[::cfg.ncoils])
+        plan2 = binding.Plan(ns.nx, ns.ny, ns.batch, b0, ns.lam, ns.sigma, ns.tau, ns.theta)
+        for _ in range(3):
+            plan2.solve(f2, m2, c2, ns.iters, 0.0)
+        torch.cuda.synchronize()
+        times = []
+        fl = torch.empty(64 * 1024 * 1024, device="cuda")
+        for _ in range(max(args.steps, 5)):
+            fl.fill_(0.0)   # 256 MB write: flushes L2 between repetitions
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            plan2.solve(f2, m2, c2, ns.iters, 0.0)
+            b.record()
+            torch.cuda.synchronize()
+            times.append(a.elapsed_time(b))
+        t_ns = float(np.median(times))
+        extra = {"workload": "NS: 128 slices x 256x256, 1 field map per slice, 200 iterations (BASELINE.json north_star target)",
+                 "stack_recon_ms": t_ns, "slice_iterations_per_s": ns.batch * ns.iters / (t_ns * 1e-3),
+                 "hbm_floor_frac": PATH_FLOOR_BYTES_PER_PX * ns.nx * ns.ny * ns.batch * ns.iters / (t_ns * 1e-3) / 1e9 / peak}
+        plan2.destroy()
+
+    if rank == 0:
+        cpu = None
+        if not args.no_cpu_baseline and world == 1:
+            nsample = oracle_sample_size(cfg)
+            v, dt, n = time_oracle(cfg, data, nsample)
+            cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": "first %d of %d batch entries of the same inputs, %d slice-iterations in %.1f s, float instantiation"
+                             % (nsample, batch, n, dt),
+                   "host_cores_available": os.cpu_count()}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, args.workload, batch, world),
+            "stack_recon_ms": ms / args.steps, "slice_iterations_per_step": slice_its,
+            "roofline": roofline, "roofline_path": roofline_path, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches, "clocks": clocks, "north_star_stack": extra,
+            "paper_context": "paper reports 4-15x GPU over CPU on unnamed hardware (PAPER.md:118); not comparable",
+        }
+        print(json.dumps(line), flush=True)
+    plan.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

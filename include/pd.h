@@ -48,8 +48,13 @@ enum pd_option {
     PD_OPT_VARIANT = 2,      /* PD_VARIANT_AUTO (default) | PD_VARIANT_STREAMING | PD_VARIANT_RESIDENT */
     PD_OPT_CHECK_EVERY = 3,  /* tolerance tested when (n+1) % value == 0 ; default 1 */
     PD_OPT_MASK_SHARED = 4,  /* 0 (default): mask is [batch][ny][nx] ; 1: one [ny][nx] mask for all slices */
-    PD_OPT_UNSAFE_STEPS = 5  /* 1: skip the PD_ESTEP check at the next pd_set_steps call (not at pd_plan) */
+    PD_OPT_UNSAFE_STEPS = 5, /* 1: skip the PD_ESTEP check at the next pd_set_steps call (not at pd_plan) */
+    PD_OPT_KERNEL_TIMING = 6 /* 1: bracket every kernel launch of pd_solve with CUDA events on the caller's stream
+                                (read with pd_get_kernel_times); default 0 */
 };
+/* kernel classes (streaming variant: 0-4; resident variant: one launch, class 5), for pd_get_kernel_times */
+enum pd_kernel_class { PD_KERNEL_INIT = 0, PD_KERNEL_DUAL = 1, PD_KERNEL_COLS = 2, PD_KERNEL_PRIMAL = 3,
+                       PD_KERNEL_FINISH = 4, PD_KERNEL_RESIDENT = 5, PD_NUM_KERNEL_CLASSES = 6 };
 enum { PD_TV_ISO = 0, PD_TV_ANISO = 1 };
 enum { PD_LAMBDA_REG = 0, PD_LAMBDA_DATA = 1 };
 enum { PD_VARIANT_AUTO = 0, PD_VARIANT_STREAMING = 1, PD_VARIANT_RESIDENT = 2 };
@@ -103,6 +108,10 @@ int pd_get_stats(pd_plan_t p, const int **iters_done, const float **relgap, cons
 /* Host convenience: copies the three arrays above into HOST buffers of length batch (any may be NULL), ordered on
  * cuda_stream after the last pd_solve, and synchronises that stream. */
 int pd_get_stats_host(pd_plan_t p, int *iters_done_host, float *relgap_host, float *relres_host, void *cuda_stream);
+
+/* With PD_OPT_KERNEL_TIMING = 1: waits for the last pd_solve and returns, per kernel class, the summed device time
+ * in milliseconds (ms_host[PD_NUM_KERNEL_CLASSES]) and the number of launches (launches_host[...]); HOST pointers. */
+int pd_get_kernel_times(pd_plan_t p, float *ms_host, int *launches_host);
 
 /* Number of kernel launches pd_solve enqueued at its last call (for launch accounting in benchmarks). */
 int pd_last_launch_count(pd_plan_t p);

@@ -15,14 +15,15 @@ LIB_PATH = os.path.join(_HERE, "libpd_b200.so")
 
 B0_X, B0_Y = 0, 1
 OK, EINVAL, ESIZE, ESTEP, ENOMEM, ECUDA, EVARIANT = 0, -1, -2, -3, -4, -5, -6
-OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS = range(6)
+OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING = range(7)
+KERNEL_CLASSES = ["init", "dual_rows", "dipole_cols", "primal_rows", "finish", "resident"]
 TV_ISO, TV_ANISO = 0, 1
 LAMBDA_REG, LAMBDA_DATA = 0, 1
 VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_last_launch_count", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -50,6 +51,7 @@ def lib():
         L.pd_set_option.argtypes = [vp, ip, ip]
         L.pd_get_stats.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.pd_get_stats_host.argtypes = [vp, vp, vp, vp, vp]
+        L.pd_get_kernel_times.argtypes = [vp, vp, vp]
         L.pd_last_launch_count.argtypes = [vp]
         L.pd_destroy.argtypes = [vp]
         L.pd_strerror.argtypes = [ip]
@@ -153,6 +155,13 @@ class Plan:
         a, b, c = C.c_void_p(), C.c_void_p(), C.c_void_p()
         _check(lib().pd_get_stats(self._h, C.byref(a), C.byref(b), C.byref(c)))
         return a.value, b.value, c.value
+
+    def kernel_times(self):
+        """pd_get_kernel_times: {class name: (total ms, launches)} of the last solve (needs OPT_KERNEL_TIMING = 1)."""
+        ms = np.zeros(len(KERNEL_CLASSES), np.float32)
+        cnt = np.zeros(len(KERNEL_CLASSES), np.int32)
+        _check(lib().pd_get_kernel_times(self._h, C.c_void_p(ms.ctypes.data), C.c_void_p(cnt.ctypes.data)))
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(KERNEL_CLASSES)}
 
     @property
     def last_launch_count(self):

@@ -11,6 +11,11 @@
 #pragma once
 #include <cuda_runtime.h>
 
+// Blackwell packed fp32x2 arithmetic (FADD2/FFMA2) for the complex butterflies; undefine to fall back to scalar.
+#ifndef PDK_SCALAR_BUTTERFLY
+#define PDK_PACKED_F32X2 1
+#endif
+
 namespace pdk {
 
 template <int N> struct FftCfg;
@@ -64,8 +69,14 @@ struct Dif {
 #pragma unroll
         for (int k = 0; k < H; ++k) {
             const float2 a = v[OFF + k], b = v[OFF + k + H];
+#ifdef PDK_PACKED_F32X2
+            // Blackwell packed fp32x2: one FADD2 / FFMA2 per complex add / subtract
+            v[OFF + k] = __fadd2_rn(a, b);
+            v[OFF + k + H] = twiddle_mul<R>(__ffma2_rn(b, make_float2(-1.f, -1.f), a), k);
+#else
             v[OFF + k] = make_float2(a.x + b.x, a.y + b.y);
             v[OFF + k + H] = twiddle_mul<R>(make_float2(a.x - b.x, a.y - b.y), k);
+#endif
         }
         Dif<H, OFF>::run(v);
         Dif<H, OFF + H>::run(v);
@@ -101,6 +112,13 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
     return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.x, w.y, a.y * w.x));
 }
 
+struct WarpSync {   // the T threads of a line sit in one warp
+    __device__ __forceinline__ void operator()() const { __syncwarp(); }
+};
+struct BlockSync {  // the T threads of a line are spread over the warps of the CTA
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+
 // Per-thread inter-stage twiddles W_N^(j*k2), k2 = 1..E-1 (index 0 unused), from the plan's double-precision table.
 template <int N>
 struct Twiddles {
@@ -113,16 +131,33 @@ struct Twiddles {
     }
 };
 
+// Same twiddles kept in shared memory as a table tws[k2*T + j] = W_N^(j*k2) (conflict-free: consecutive j), read when
+// needed instead of living in E registers for the whole kernel.
+template <int N>
+struct TwiddlesSmem {
+    static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
+    const float2 *w;  // &tws[j]
+    __device__ __forceinline__ float2 get(int k) const { return w[k * T]; }
+    // fill a table of E*T float2 from the plan's W_N^n table (all threads of the CTA cooperate; caller synchronises)
+    static __device__ __forceinline__ void fill(float2 *tws, const float2 *__restrict__ table, int tid, int nthreads) {
+        for (int i = tid; i < E * T; i += nthreads) tws[i] = __ldg(table + (((i % T) * (i / T)) & (N - 1)));
+    }
+};
+template <int N>
+__device__ __forceinline__ float2 tw_get(const Twiddles<N> &tw, int k) { return tw.w[k]; }
+template <int N>
+__device__ __forceinline__ float2 tw_get(const TwiddlesSmem<N> &tw, int k) { return tw.get(k); }
+
 // Cooperative forward FFT of one length-N line held by T threads (thread j: points j + T*m).
 //   sm : this line's exchange region, E rows of LD float2 (row k2, column j)
 //   SYNC: functor that synchronises the T threads of the line (and orders their shared-memory accesses)
-template <int N, int LD, class Sync>
-__device__ __forceinline__ void fft_line(float2 (&v)[FftCfg<N>::E], float2 *sm, int j, const Twiddles<N> &tw,
+template <int N, int LD, class Tw, class Sync>
+__device__ __forceinline__ void fft_line(float2 (&v)[FftCfg<N>::E], float2 *sm, int j, const Tw &tw,
                                          Sync sync) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, C = E / T;
     dft_reg<E>(v);  // over n2: Y[j][k2]
 #pragma unroll
-    for (int k = 1; k < E; ++k) v[k] = cmul(v[k], tw.w[k]);
+    for (int k = 1; k < E; ++k) v[k] = cmul(v[k], tw_get<N>(tw, k));
     sync();  // earlier readers of sm are done
 #pragma unroll
     for (int k = 0; k < E; ++k) sm[k * LD + j] = v[k];

@@ -3,6 +3,7 @@
 // No CPU fallback exists: every arithmetic step of the path runs in the kernels of pd_streaming.cuh.
 #include "../../include/pd.h"
 #include "pd_streaming.cuh"
+#include "pd_resident.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -10,6 +11,7 @@
 #include <new>
 #include <vector>
 
+using pdk::ResidentArgs;
 using pdk::SolveArgs;
 
 namespace {
@@ -46,10 +48,20 @@ struct pd_plan_s {
     int *stop_iter, *iters_done;
     float *P0, *relgap, *relres, *gap_part, *res_part;
     int nparts;
+    // resident variant (pd_resident.cuh): per-cluster scratch, 9 arrays of nx*ny float2 per cluster
+    int res_ok;            // this size has a resident kernel
+    int res_clusters;      // clusters launched (= scratch slots)
+    int res_csize;         // CTAs per cluster
+    float2 *res_scratch;   // [kResidentScratchArrays][res_clusters][nx*ny]
+    float *rk_part;        // [res_clusters][res_csize][8]
     // host-buffer entry point staging
     float *h_field, *h_mask, *h_chi;
     int last_launches;
     int device;
+    // optional per-kernel-class device timing (PD_OPT_KERNEL_TIMING): events around every launch of the last solve
+    int timing;
+    std::vector<cudaEvent_t> *ev;      // pool, two per launch
+    std::vector<int> *ev_class;        // kernel class of launch i
 };
 
 namespace {
@@ -142,6 +154,110 @@ cudaError_t set_col_smem() {
                                 pdk::ColCfg<NY>::SMEM_BYTES);
 }
 
+// ---- resident variant: configuration per size, occupancy query, launch
+template <int N> struct ResChoice;
+template <> struct ResChoice<64>  { static constexpr int C = 2, NT = 256; };
+template <> struct ResChoice<128> { static constexpr int C = 4, NT = 256; };
+template <> struct ResChoice<256> { static constexpr int C = 8, NT = 512; };
+
+template <int N, bool HAS_W, bool ANISO>
+cudaError_t resident_launch_config(cudaLaunchConfig_t *cfg, cudaLaunchAttribute *attr, int nclusters, cudaStream_t st) {
+    using Ch = ResChoice<N>;
+    using Cfg = pdk::ResCfg<N, Ch::C, Ch::NT>;
+    cudaError_t e = cudaFuncSetAttribute(pdk::resident_kernel<N, Ch::C, Ch::NT, HAS_W, ANISO>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    std::memset(cfg, 0, sizeof(*cfg));
+    cfg->gridDim = dim3((unsigned)(nclusters * Ch::C), 1, 1);
+    cfg->blockDim = dim3(Ch::NT, 1, 1);
+    cfg->dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg->stream = st;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = Ch::C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg->attrs = attr;
+    cfg->numAttrs = 1;
+    return cudaSuccess;
+}
+
+template <int N>
+int resident_max_clusters(int *out) {
+    using Ch = ResChoice<N>;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    cudaError_t e = resident_launch_config<N, false, false>(&cfg, attr, 1, nullptr);
+    if (e != cudaSuccess) return cuda_fail(e, "resident kernel attributes");
+    int n = 0;
+    e = cudaOccupancyMaxActiveClusters(&n, pdk::resident_kernel<N, Ch::C, Ch::NT, false, false>, &cfg);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaOccupancyMaxActiveClusters");
+    *out = n;
+    return PD_OK;
+}
+
+template <int N, bool HAS_W, bool ANISO>
+cudaError_t resident_launch2(const ResidentArgs &a, int nclusters, cudaStream_t st) {
+    using Ch = ResChoice<N>;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    cudaError_t e = resident_launch_config<N, HAS_W, ANISO>(&cfg, attr, nclusters, st);
+    if (e != cudaSuccess) return e;
+    return cudaLaunchKernelEx(&cfg, pdk::resident_kernel<N, Ch::C, Ch::NT, HAS_W, ANISO>, a);
+}
+template <int N>
+cudaError_t resident_launch(const ResidentArgs &a, bool w, bool aniso, int nclusters, cudaStream_t st) {
+    if (w) return aniso ? resident_launch2<N, true, true>(a, nclusters, st) : resident_launch2<N, true, false>(a, nclusters, st);
+    return aniso ? resident_launch2<N, false, true>(a, nclusters, st) : resident_launch2<N, false, false>(a, nclusters, st);
+}
+
+int resident_csize(int n) { return n == 64 ? ResChoice<64>::C : n == 128 ? ResChoice<128>::C : ResChoice<256>::C; }
+
+int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                   cudaStream_t st) {
+    const size_t P = (size_t)p->nx * p->ny;
+    ResidentArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.batch = p->batch; a.npairs = p->npairs; a.max_iters = max_iters; a.check_every = p->check_every;
+    effective_params(p, &a.alpha, &a.sigma, &a.tau);
+    a.theta = p->theta;
+    a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
+    a.tol = tol;
+    a.field = field; a.mask = mask; a.weight = p->weight;
+    a.mask_bstride = p->mask_shared ? 0 : (long long)P;
+    a.chi_out = chi_out;
+    const size_t stride = (size_t)p->res_clusters * P;
+    float2 *base = p->res_scratch;
+    a.Z = base; a.qy = base + stride; a.chi = base + 2 * stride; a.chibar = base + 3 * stride;
+    a.phi2 = base + 4 * stride; a.M2 = base + 5 * stride; a.W2 = base + 6 * stride;
+    a.Dtab = p->Dtab; a.tw_tab = p->tw_row;
+    a.part = p->rk_part;
+    a.iters_done = p->iters_done; a.relgap = p->relgap; a.relres = p->relres;
+
+    p->ev_class->clear();
+    if (p->timing) {
+        while (p->ev->size() < 2) {
+            cudaEvent_t evn_;
+            PD_CUDA(cudaEventCreate(&evn_));
+            p->ev->push_back(evn_);
+        }
+        PD_CUDA(cudaEventRecord((*p->ev)[0], st));
+    }
+    const bool w = p->weight != nullptr, aniso = p->tv_mode == PD_TV_ANISO;
+    cudaError_t e;
+    switch (p->nx) {
+        case 64: e = resident_launch<64>(a, w, aniso, p->res_clusters, st); break;
+        case 128: e = resident_launch<128>(a, w, aniso, p->res_clusters, st); break;
+        default: e = resident_launch<256>(a, w, aniso, p->res_clusters, st); break;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "resident kernel launch");
+    if (p->timing) {
+        PD_CUDA(cudaEventRecord((*p->ev)[1], st));
+        p->ev_class->push_back(PD_KERNEL_RESIDENT);
+    }
+    p->last_launches = 1;
+    return PD_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -157,6 +273,9 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     pd_plan_s *p = new (std::nothrow) pd_plan_s;
     if (!p) return PD_ENOMEM;
     std::memset(p, 0, sizeof(*p));
+    p->ev = new (std::nothrow) std::vector<cudaEvent_t>();
+    p->ev_class = new (std::nothrow) std::vector<int>();
+    if (!p->ev || !p->ev_class) { delete p->ev; delete p->ev_class; delete p; return PD_ENOMEM; }
     p->nx = nx; p->ny = ny; p->batch = batch; p->npairs = (batch + 1) / 2; p->b0_dir = B0_dir;
     p->lambda_user = lambda; p->sigma_user = sigma; p->tau_user = tau; p->theta = theta;
     p->check_every = 1;
@@ -203,6 +322,24 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (e == cudaSuccess) e = set_col_smem<512>();
         if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "plan table upload"); }
     }
+    // resident variant: square slices up to 256x256
+    if (nx == ny && nx <= 256) {
+        int maxc = 0;
+        rc = (nx == 64) ? resident_max_clusters<64>(&maxc) : (nx == 128) ? resident_max_clusters<128>(&maxc)
+                                                                          : resident_max_clusters<256>(&maxc);
+        if (rc == PD_OK && maxc >= 1) {
+            p->res_csize = resident_csize(nx);
+            p->res_clusters = maxc < p->npairs ? maxc : p->npairs;
+            rc = dev_alloc(&p->res_scratch, (size_t)pdk::kResidentScratchArrays * p->res_clusters * P);
+            if (rc == PD_OK) rc = dev_alloc(&p->rk_part, (size_t)p->res_clusters * p->res_csize * 8);
+            if (rc != PD_OK) { pd_destroy(p); return rc; }
+            cudaError_t e = cudaMemset(p->rk_part, 0, (size_t)p->res_clusters * p->res_csize * 8 * sizeof(float));
+            if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "resident scratch init"); }
+            p->res_ok = 1;
+        } else {
+            cudaGetLastError();  // no cluster launch possible on this device: the streaming variant remains
+        }
+    }
     *out = p;
     return PD_OK;
 }
@@ -231,8 +368,8 @@ int pd_set_option(pd_plan_t p, int key, int value) {
             if (value != PD_LAMBDA_REG && value != PD_LAMBDA_DATA) return PD_EINVAL;
             p->lambda_conv = value; return PD_OK;
         case PD_OPT_VARIANT:
-            if (value == PD_VARIANT_RESIDENT) return PD_EVARIANT;  // not built in this round: fail loudly
-            if (value != PD_VARIANT_AUTO && value != PD_VARIANT_STREAMING) return PD_EINVAL;
+            if (value != PD_VARIANT_AUTO && value != PD_VARIANT_STREAMING && value != PD_VARIANT_RESIDENT) return PD_EINVAL;
+            if (value == PD_VARIANT_RESIDENT && !p->res_ok) return PD_EVARIANT;
             p->variant = value; return PD_OK;
         case PD_OPT_CHECK_EVERY:
             if (value < 1) return PD_EINVAL;
@@ -243,6 +380,9 @@ int pd_set_option(pd_plan_t p, int key, int value) {
         case PD_OPT_UNSAFE_STEPS:
             if (value != 0 && value != 1) return PD_EINVAL;
             p->unsafe_steps = value; return PD_OK;
+        case PD_OPT_KERNEL_TIMING:
+            if (value != 0 && value != 1) return PD_EINVAL;
+            p->timing = value; return PD_OK;
         default: return PD_EINVAL;
     }
 }
@@ -253,6 +393,8 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
     if (p->lambda_conv == PD_LAMBDA_DATA && !(p->lambda_user > 0.f)) return PD_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
+
+    if (p->res_ok && p->variant != PD_VARIANT_STREAMING) return solve_resident(p, field, mask, chi_out, max_iters, tol, st);
 
     SolveArgs a;
     std::memset(&a, 0, sizeof(a));
@@ -272,6 +414,25 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
     a.max_iters = max_iters;
 
     int launches = 0;
+    p->ev_class->clear();
+    // LAUNCH(class, statement): enqueue one kernel; with PD_OPT_KERNEL_TIMING bracket it with two events on `st`
+#define PD_LAUNCH(cls, stmt)                                                                       \
+    do {                                                                                           \
+        if (p->timing) {                                                                           \
+            while (p->ev->size() < 2 * (size_t)(launches + 1)) {                                   \
+                cudaEvent_t evn_;                                                                  \
+                PD_CUDA(cudaEventCreate(&evn_));                                                   \
+                p->ev->push_back(evn_);                                                            \
+            }                                                                                      \
+            PD_CUDA(cudaEventRecord((*p->ev)[2 * launches], st));                                  \
+        }                                                                                          \
+        stmt;                                                                                      \
+        if (p->timing) {                                                                           \
+            PD_CUDA(cudaEventRecord((*p->ev)[2 * launches + 1], st));                              \
+            p->ev_class->push_back(cls);                                                           \
+        }                                                                                          \
+        ++launches;                                                                                \
+    } while (0)
     // chi_0 = p_0 = q_0 = 0, chibar_0 = chi_0; the spectrum of chibar_0 is 0 as well
     PD_CUDA(cudaMemsetAsync(chi_out, 0, BP * sizeof(float), st));
     PD_CUDA(cudaMemsetAsync(p->chibar, 0, BP * sizeof(float), st));
@@ -280,16 +441,15 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
     PD_CUDA(cudaMemsetAsync(p->qy, 0, BP * sizeof(float), st));
     PD_CUDA(cudaMemsetAsync(p->Z, 0, P * (size_t)p->npairs * sizeof(float2), st));
     PD_CUDA(cudaMemsetAsync(p->stop_iter, 0, ((size_t)p->batch + 1) * sizeof(int), st));
-    pdk::init_slices_kernel<<<p->batch, 256, 0, st>>>(a);
-    ++launches;
+    PD_LAUNCH(PD_KERNEL_INIT, (pdk::init_slices_kernel<<<p->batch, 256, 0, st>>>(a)));
     for (int n = 0; n < max_iters; ++n) {
-        if (n > 0) { PD_DISPATCH(p->ny, launch_cols, a, n, 0, st); ++launches; }   // K1 column pass (chibar_0 = 0)
-        PD_DISPATCH(p->nx, launch_dual, a, n, st); ++launches;
-        PD_DISPATCH(p->ny, launch_cols, a, n, 1, st); ++launches;                 // K2 column pass + gap / stop flag
-        PD_DISPATCH(p->nx, launch_primal, a, n, st); ++launches;
+        if (n > 0) PD_LAUNCH(PD_KERNEL_COLS, PD_DISPATCH(p->ny, launch_cols, a, n, 0, st));  // K1 column pass (chibar_0 = 0)
+        PD_LAUNCH(PD_KERNEL_DUAL, PD_DISPATCH(p->nx, launch_dual, a, n, st));
+        PD_LAUNCH(PD_KERNEL_COLS, PD_DISPATCH(p->ny, launch_cols, a, n, 1, st));             // K2 column pass + gap / stop flag
+        PD_LAUNCH(PD_KERNEL_PRIMAL, PD_DISPATCH(p->nx, launch_primal, a, n, st));
     }
-    pdk::finish_slices_kernel<<<(p->batch + 127) / 128, 128, 0, st>>>(a, p->iters_done);
-    ++launches;
+    PD_LAUNCH(PD_KERNEL_FINISH, (pdk::finish_slices_kernel<<<(p->batch + 127) / 128, 128, 0, st>>>(a, p->iters_done)));
+#undef PD_LAUNCH
     PD_CUDA(cudaGetLastError());
     p->last_launches = launches;
     return PD_OK;
@@ -333,14 +493,37 @@ int pd_get_stats_host(pd_plan_t p, int *iters_done_host, float *relgap_host, flo
     return PD_OK;
 }
 
+int pd_get_kernel_times(pd_plan_t p, float *ms_host, int *launches_host) {
+    if (!p) return PD_EINVAL;
+    for (int c = 0; c < PD_NUM_KERNEL_CLASSES; ++c) {
+        if (ms_host) ms_host[c] = 0.f;
+        if (launches_host) launches_host[c] = 0;
+    }
+    if (!p->timing) return PD_EINVAL;
+    const size_t n = p->ev_class->size();
+    if (n == 0) return PD_OK;
+    PD_CUDA(cudaEventSynchronize((*p->ev)[2 * n - 1]));
+    for (size_t i = 0; i < n; ++i) {
+        float ms = 0.f;
+        PD_CUDA(cudaEventElapsedTime(&ms, (*p->ev)[2 * i], (*p->ev)[2 * i + 1]));
+        const int c = (*p->ev_class)[i];
+        if (ms_host) ms_host[c] += ms;
+        if (launches_host) launches_host[c] += 1;
+    }
+    return PD_OK;
+}
+
 int pd_last_launch_count(pd_plan_t p) { return p ? p->last_launches : PD_EINVAL; }
 
 int pd_destroy(pd_plan_t p) {
     if (!p) return PD_EINVAL;
     void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->chibar, p->p, p->qx, p->qy, p->Z, p->stop_iter, p->iters_done,
-                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi};
+                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part};
     for (void *q : ptrs)
         if (q) cudaFree(q);
+    if (p->ev) for (cudaEvent_t e : *p->ev) cudaEventDestroy(e);
+    delete p->ev;
+    delete p->ev_class;
     delete p;
     return PD_OK;
 }

@@ -52,13 +52,6 @@ __device__ __forceinline__ float group_sum(float v) {
     return v;
 }
 
-struct WarpSync {
-    __device__ __forceinline__ void operator()() const { __syncwarp(); }
-};
-struct BlockSync {
-    __device__ __forceinline__ void operator()() const { __syncthreads(); }
-};
-
 // Row kernels: G lines per CTA, one line (pair j, row y) per group of T threads inside one warp.
 template <int NX> struct RowCfg {
     static constexpr int E = FftCfg<NX>::E, T = FftCfg<NX>::T;

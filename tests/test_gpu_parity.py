@@ -36,10 +36,18 @@ def slice_rel(a, b):
     return np.linalg.norm(a - b, axis=1) / den
 
 
+@pytest.fixture(params=["auto", "streaming"])
+def variant(request):
+    """auto = the resident cluster kernel where the size has one (square, <= 256), else streaming."""
+    return request.param
+
+
 def gpu_solve(torch, pd, field, mask, iters, *, lam, sigma=0.25, tau=0.25, theta=1.0, tol=0.0, weight=None, b0=1,
-              options=(), host=False):
+              options=(), host=False, variant="auto"):
     batch, ny, nx = field.shape
     plan = pd.Plan(nx, ny, batch, b0, lam, sigma, tau, theta)
+    if variant == "streaming":
+        plan.set_option(pd.OPT_VARIANT, pd.VARIANT_STREAMING)
     for k, v in options:
         plan.set_option(k, v)
     if host:
@@ -61,9 +69,9 @@ def gpu_solve(torch, pd, field, mask, iters, *, lam, sigma=0.25, tau=0.25, theta
 
 
 @pytest.mark.parametrize("ny,nx", [(64, 64), (128, 128), (256, 256), (512, 512), (64, 256), (512, 128), (128, 64)])
-def test_one_iteration_all_sizes(torch, pd, oracle, ny, nx):
+def test_one_iteration_all_sizes(torch, pd, oracle, ny, nx, variant):
     case = synth.random_case(nx, ny, 3, seed=nx + ny, with_mask=True, with_weight=True)   # odd batch: ragged last pair
-    g = gpu_solve(torch, pd, case["field"], case["mask"], 1, lam=0.05, weight=case["weight"])
+    g = gpu_solve(torch, pd, case["field"], case["mask"], 1, lam=0.05, weight=case["weight"], variant=variant)
     o = oracle.solve(case["field"], case["mask"], case["weight"], lambda_=0.05, sigma=0.25, tau=0.25, max_iters=1)
     assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
     assert np.allclose(g["relgap"], o["relgap"][:, 0], rtol=1e-4)
@@ -71,19 +79,19 @@ def test_one_iteration_all_sizes(torch, pd, oracle, ny, nx):
 
 
 @pytest.mark.parametrize("iters", [2, 3, 7])
-def test_few_iterations_exercise_q_and_divergence(torch, pd, oracle, iters):
+def test_few_iterations_exercise_q_and_divergence(torch, pd, oracle, iters, variant):
     case = synth.random_case(128, 64, 4, seed=77, with_mask=True, with_weight=True)
-    g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.5, weight=case["weight"])
+    g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.5, weight=case["weight"], variant=variant)
     o = oracle.solve(case["field"], case["mask"], case["weight"], lambda_=0.5, sigma=0.25, tau=0.25, max_iters=iters)
     assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
     assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-3)
     assert np.allclose(g["relres"], o["relres"][:, iters - 1], rtol=1e-3)
 
 
-def test_config0_full(torch, pd, oracle):
+def test_config0_full(torch, pd, oracle, variant):
     d = synth.generate(0)
     cfg = d["cfg"]
-    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam)
+    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam, variant=variant)
     o = oracle.solve(d["field"], d["mask"], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau, max_iters=cfg.iters)
     assert slice_rel(g["chi"], o["chi"]).max() < TOL_FULL
     assert slice_rel(g["chi"], o["chi"]).max() < 2e-5   # what fp32 actually achieves
@@ -92,10 +100,10 @@ def test_config0_full(torch, pd, oracle):
     assert g["iters_done"][0] == 100
 
 
-def test_config1_full(torch, pd, oracle):
+def test_config1_full(torch, pd, oracle, variant):
     d = synth.generate(1)
     cfg = d["cfg"]
-    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam)
+    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam, variant=variant)
     o = oracle.solve(d["field"], d["mask"], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau, max_iters=cfg.iters,
                      want_hist=True)
     r = slice_rel(g["chi"], o["chi"])
@@ -103,11 +111,11 @@ def test_config1_full(torch, pd, oracle):
     assert np.allclose(g["relgap"], o["relgap"][:, -1], rtol=1e-3)
 
 
-def _sampled_full_config(torch, pd, oracle, cid, sample, host=False):
+def _sampled_full_config(torch, pd, oracle, cid, sample, host=False, variant="auto"):
     """Run the GPU on the FULL config (the launch configuration bench.py times); oracle on sampled batch entries."""
     d = synth.generate(cid)
     cfg = d["cfg"]
-    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam, tol=cfg.tol, host=host)
+    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam, tol=cfg.tol, host=host, variant=variant)
     assert np.all(np.isfinite(g["chi"]))
     # property that holds at any size: every iterate has zero mean (DESIGN.md pin P7)
     means = np.abs(g["chi"].reshape(cfg.batch, -1).astype(np.float64).mean(axis=1))
@@ -133,8 +141,8 @@ def test_config3_full_sampled_through_host_entry(torch, pd, oracle):
     assert np.all(g["iters_done"] == 200)
 
 
-def test_northstar_stack_sampled(torch, pd, oracle):
-    _sampled_full_config(torch, pd, oracle, 5, [0, 127])
+def test_northstar_stack_sampled(torch, pd, oracle, variant):
+    _sampled_full_config(torch, pd, oracle, 5, [0, 127], variant=variant)
 
 
 def test_config4_full_tolerance_stop_sampled(torch, pd, oracle):
@@ -143,54 +151,54 @@ def test_config4_full_tolerance_stop_sampled(torch, pd, oracle):
     assert np.all(g["relgap"] < 1e-4)
 
 
-def test_options_aniso_dataconv_sharedmask_b0x_theta(torch, pd, oracle):
+def test_options_aniso_dataconv_sharedmask_b0x_theta(torch, pd, oracle, variant):
     case = synth.random_case(64, 128, 2, seed=5, with_mask=True)
     f, m = case["field"], case["mask"]
-    g = gpu_solve(torch, pd, f, m, 20, lam=0.3, options=[(pd.OPT_TV_MODE, pd.TV_ANISO)])
+    g = gpu_solve(torch, pd, f, m, 20, lam=0.3, options=[(pd.OPT_TV_MODE, pd.TV_ANISO)], variant=variant)
     o = oracle.solve(f, m, lambda_=0.3, sigma=0.25, tau=0.25, max_iters=20, tv_mode=oracle.TV_ANISO)
     assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
     assert np.allclose(g["relgap"], o["relgap"][:, -1], rtol=1e-3)
-    g = gpu_solve(torch, pd, f, m, 20, lam=40.0, options=[(pd.OPT_LAMBDA_CONV, pd.LAMBDA_DATA)])
+    g = gpu_solve(torch, pd, f, m, 20, lam=40.0, options=[(pd.OPT_LAMBDA_CONV, pd.LAMBDA_DATA)], variant=variant)
     o = oracle.solve(f, m, lambda_=40.0, sigma=0.25, tau=0.25, max_iters=20, lambda_conv=oracle.LAMBDA_DATA)
     assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
     assert np.allclose(g["relgap"], o["relgap"][:, -1], rtol=1e-3)
-    g = gpu_solve(torch, pd, f, m[0], 20, lam=0.3, options=[(pd.OPT_MASK_SHARED, 1)])
+    g = gpu_solve(torch, pd, f, m[0], 20, lam=0.3, options=[(pd.OPT_MASK_SHARED, 1)], variant=variant)
     o = oracle.solve(f, np.stack([m[0], m[0]]), lambda_=0.3, sigma=0.25, tau=0.25, max_iters=20)
     assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
-    g = gpu_solve(torch, pd, f, None, 20, lam=0.3, b0=0, theta=0.5)
+    g = gpu_solve(torch, pd, f, None, 20, lam=0.3, b0=0, theta=0.5, variant=variant)
     o = oracle.solve(f, None, lambda_=0.3, sigma=0.25, tau=0.25, theta=0.5, max_iters=20, b0_dir=oracle.B0_X)
     assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
-    g = gpu_solve(torch, pd, f, m, 20, lam=0.3, sigma=-1.0, tau=-1.0)          # automatic steps
+    g = gpu_solve(torch, pd, f, m, 20, lam=0.3, sigma=-1.0, tau=-1.0, variant=variant)   # automatic steps
     s = 1.0 / np.sqrt(8 + 4 / 9)
     o = oracle.solve(f, m, lambda_=0.3, sigma=np.float32(s), tau=np.float32(s), max_iters=20)
     assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
-    g = gpu_solve(torch, pd, f, m, 20, lam=0.0)                                  # alpha = 0: q stays 0 (R13)
+    g = gpu_solve(torch, pd, f, m, 20, lam=0.0, variant=variant)                 # alpha = 0: q stays 0 (R13)
     o = oracle.solve(f, m, lambda_=0.0, sigma=0.25, tau=0.25, max_iters=20)
     assert slice_rel(g["chi"], o["chi"]).max() < 2e-5
 
 
-def test_degenerate_cases(torch, pd, oracle):
+def test_degenerate_cases(torch, pd, oracle, variant):
     f = synth.random_case(64, 64, 3, seed=9)["field"]
     f[1] = 0.0                                                                # an all-zero slice inside an active pair
-    g = gpu_solve(torch, pd, f, None, 15, lam=0.1, tol=1e-9)
+    g = gpu_solve(torch, pd, f, None, 15, lam=0.1, tol=1e-9, variant=variant)
     assert g["iters_done"].tolist() == [15, 0, 15] and np.all(g["chi"][1] == 0)
     o = oracle.solve(f, None, lambda_=0.1, sigma=0.25, tau=0.25, max_iters=15)
     assert slice_rel(g["chi"][[0, 2]], o["chi"][[0, 2]]).max() < 2e-5
-    g = gpu_solve(torch, pd, f, None, 15, lam=0.1)                            # tol <= 0: runs N no-op iterations
+    g = gpu_solve(torch, pd, f, None, 15, lam=0.1, variant=variant)           # tol <= 0: runs N no-op iterations
     assert g["iters_done"].tolist() == [15, 15, 15] and np.all(g["chi"][1] == 0) and g["relgap"][1] == 0
-    g = gpu_solve(torch, pd, f, None, 0, lam=0.1)                             # max_iters = 0: chi_0 = 0
+    g = gpu_solve(torch, pd, f, None, 0, lam=0.1, variant=variant)            # max_iters = 0: chi_0 = 0
     assert np.all(g["chi"] == 0) and np.all(g["iters_done"] == 0)
-    one = gpu_solve(torch, pd, f[:1], None, 15, lam=0.1)                      # batch 1: half-empty pair
+    one = gpu_solve(torch, pd, f[:1], None, 15, lam=0.1, variant=variant)     # batch 1: half-empty pair
     assert slice_rel(one["chi"], o["chi"][:1]).max() < 2e-5
 
 
-def test_per_slice_stop_mixed_batch(torch, pd, oracle):
+def test_per_slice_stop_mixed_batch(torch, pd, oracle, variant):
     """Slices of one batch stop at different iterations; a stopped slice is frozen while its pair partner goes on."""
     d = synth.generate(1, nslices=5)
     f = d["field"].copy()
     f[1] *= 1e-3          # different noise-to-signal ratios do not matter; different phantoms already differ
     tol = 3e-4
-    g = gpu_solve(torch, pd, f, d["mask"], 300, lam=0.01, tol=tol)
+    g = gpu_solve(torch, pd, f, d["mask"], 300, lam=0.01, tol=tol, variant=variant)
     o = oracle.solve(f, d["mask"], lambda_=0.01, sigma=0.25, tau=0.25, max_iters=300, tol=tol)
     assert np.abs(g["iters_done"].astype(int) - o["iters_done"].astype(int)).max() <= 1
     assert len(set(g["iters_done"].tolist())) > 1
@@ -199,8 +207,11 @@ def test_per_slice_stop_mixed_batch(torch, pd, oracle):
                           want_hist=True)
         assert slice_rel(g["chi"][b:b + 1], ob["chi"]).max() < TOL_FULL
         assert abs(g["relgap"][b] / ob["relgap"][0, -1] - 1) < 1e-3
-    ge = gpu_solve(torch, pd, f, d["mask"], 300, lam=0.01, tol=tol, options=[(pd.OPT_CHECK_EVERY, 8)])
-    assert np.all(ge["iters_done"] % 8 == 0) and np.all(ge["iters_done"] >= g["iters_done"])
+    ge = gpu_solve(torch, pd, f, d["mask"], 300, lam=0.01, tol=tol, options=[(pd.OPT_CHECK_EVERY, 8)], variant=variant)
+    oe = oracle.solve(f, d["mask"], lambda_=0.01, sigma=0.25, tau=0.25, max_iters=300, tol=tol, check_every=8,
+                      want_hist=False)
+    assert np.all((ge["iters_done"] % 8 == 0) | (ge["iters_done"] == 300))
+    assert np.abs(ge["iters_done"].astype(int) - oe["iters_done"].astype(int)).max() <= 8
 
 
 def test_repeatable_and_plan_reuse(torch, pd):

@@ -169,6 +169,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C3", choices=sorted(WORKLOADS))
+    ap.add_argument("--variant", default="auto", choices=["auto", "streaming", "resident"],
+                    help="auto: the library's own choice (resident cluster kernel for square slices <= 256, else streaming)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the north-star single-coil stack timing")
@@ -203,6 +205,9 @@ def main():
     chi = torch.empty_like(field)
     b0 = binding.B0_Y if cfg.b0_dir == "y" else binding.B0_X
     plan = binding.Plan(cfg.nx, cfg.ny, batch, b0, cfg.lam, cfg.sigma, cfg.tau, cfg.theta)
+    if args.variant != "auto":
+        plan.set_option(binding.OPT_VARIANT, {"streaming": binding.VARIANT_STREAMING, "resident": binding.VARIANT_RESIDENT}[args.variant])
+    plan_info = plan.info()
     small = batch * P * 32 <= 2 * 126e6
     flush = torch.empty(64 * 1024 * 1024, device="cuda") if small else None
 
@@ -312,6 +317,8 @@ def main():
         ns = synth.CONFIGS[5]
         f2, m2, c2 = field[::cfg.ncoils].contiguous(), mask[::cfg.ncoils].contiguous(), torch.empty_like(field[::cfg.ncoils])
         plan2 = binding.Plan(ns.nx, ns.ny, ns.batch, b0, ns.lam, ns.sigma, ns.tau, ns.theta)
+        if args.variant != "auto":
+            plan2.set_option(binding.OPT_VARIANT, {"streaming": binding.VARIANT_STREAMING, "resident": binding.VARIANT_RESIDENT}[args.variant])
         for _ in range(3):
             plan2.solve(f2, m2, c2, ns.iters, 0.0)
         torch.cuda.synchronize()
@@ -343,7 +350,7 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, args.workload, batch, world),
+            "dtype": "f32", "data": "synthetic", "config": dict(workload_config(cfg, args.workload, batch, world), **plan_info),
             "stack_recon_ms": ms / args.steps, "slice_iterations_per_step": slice_its,
             "roofline": roofline, "roofline_path": roofline_path, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches, "clocks": clocks, "north_star_stack": extra,

@@ -116,6 +116,12 @@ int pd_get_kernel_times(pd_plan_t p, float *ms_host, int *launches_host);
 /* Number of kernel launches pd_solve enqueued at its last call (for launch accounting in benchmarks). */
 int pd_last_launch_count(pd_plan_t p);
 
+/* Which variant the next pd_solve of this plan runs, and its launch shape (HOST pointers, any may be NULL):
+ * *variant = PD_VARIANT_STREAMING or PD_VARIANT_RESIDENT; *clusters = thread-block clusters the resident kernel is
+ * launched with (the paper's "N slices at a time", here slice PAIRS in flight; 0 for streaming);
+ * *cluster_size = CTAs per cluster (0 for streaming). */
+int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size);
+
 int pd_destroy(pd_plan_t p);
 
 const char *pd_strerror(int code);

@@ -23,7 +23,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -53,6 +53,7 @@ def lib():
         L.pd_get_stats_host.argtypes = [vp, vp, vp, vp, vp]
         L.pd_get_kernel_times.argtypes = [vp, vp, vp]
         L.pd_last_launch_count.argtypes = [vp]
+        L.pd_get_info.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
         L.pd_destroy.argtypes = [vp]
         L.pd_strerror.argtypes = [ip]
         L.pd_strerror.restype = C.c_char_p
@@ -162,6 +163,13 @@ class Plan:
         cnt = np.zeros(len(KERNEL_CLASSES), np.int32)
         _check(lib().pd_get_kernel_times(self._h, C.c_void_p(ms.ctypes.data), C.c_void_p(cnt.ctypes.data)))
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(KERNEL_CLASSES)}
+
+    def info(self):
+        """pd_get_info: {"variant": "streaming"|"resident", "clusters": n, "cluster_size": c} of the next solve."""
+        v, n, c = C.c_int(), C.c_int(), C.c_int()
+        _check(lib().pd_get_info(self._h, C.byref(v), C.byref(n), C.byref(c)))
+        return {"variant": "resident" if v.value == VARIANT_RESIDENT else "streaming", "clusters": n.value,
+                "cluster_size": c.value}
 
     @property
     def last_launch_count(self):

@@ -515,6 +515,15 @@ int pd_get_kernel_times(pd_plan_t p, float *ms_host, int *launches_host) {
 
 int pd_last_launch_count(pd_plan_t p) { return p ? p->last_launches : PD_EINVAL; }
 
+int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
+    if (!p) return PD_EINVAL;
+    const bool res = p->res_ok && p->variant != PD_VARIANT_STREAMING;
+    if (variant) *variant = res ? PD_VARIANT_RESIDENT : PD_VARIANT_STREAMING;
+    if (clusters) *clusters = res ? p->res_clusters : 0;
+    if (cluster_size) *cluster_size = res ? p->res_csize : 0;
+    return PD_OK;
+}
+
 int pd_destroy(pd_plan_t p) {
     if (!p) return PD_EINVAL;
     void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->chibar, p->p, p->qx, p->qy, p->Z, p->stop_iter, p->iters_done,

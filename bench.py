@@ -23,7 +23,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2006_09808_b200 import synth  # noqa: E402  (input generator only: holds none of the solver's arithmetic)
+from paper_2006_09808_b200 import shard, synth  # noqa: E402  (input generator and host-side sharding helpers only)
 
 METRIC = "pd_slice_iterations_per_s"
 UNIT = "slice-iterations/s"
@@ -197,7 +197,7 @@ def main():
     cid = WORKLOADS[args.workload]
     cfg = synth.CONFIGS[cid]
     # weak scaling: every rank reconstructs its own stack of the workload's size (slices are independent)
-    data = synth.generate(cid, first_slice=rank * cfg.nslices)
+    data = synth.generate(cid, first_slice=shard.weak_first_slice(cfg.nslices, rank))
     batch = cfg.batch
     P = cfg.nx * cfg.ny
     field = torch.from_numpy(data["field"]).cuda()
@@ -244,17 +244,11 @@ def main():
                 torch.cuda.synchronize()
                 total += e0.elapsed_time(e1)
         barrier()
-        t = torch.tensor([total], device="cuda", dtype=torch.float64)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return shard.max_over_ranks(total, "cuda")
 
     def total_iters():
         it, _, _ = plan.stats()
-        t = torch.tensor([float(it.sum())], device="cuda", dtype=torch.float64)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item()), it
+        return shard.sum_over_ranks(float(it.sum()), "cuda"), it
 
     # ---- device-resident measurement (inputs already in HBM)
     timed(args.warmup)

@@ -4,4 +4,4 @@ The CUDA library is loaded lazily by `paper_2006_09808_b200.binding`; importing 
 (or `paper_2006_09808_b200.synth`, the seeded input generator) needs neither a GPU nor the
 built extension.
 """
-__all__ = ["binding", "synth"]
+__all__ = ["binding", "shard", "synth"]

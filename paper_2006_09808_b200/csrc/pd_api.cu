@@ -156,17 +156,27 @@ cudaError_t set_col_smem() {
 
 // ---- resident variant: configuration per size, occupancy query, launch
 template <int N> struct ResChoice;
-template <> struct ResChoice<64>  { static constexpr int C = 2, NT = 256; };
-template <> struct ResChoice<128> { static constexpr int C = 4, NT = 256; };
-template <> struct ResChoice<256> { static constexpr int C = 8, NT = 512; };
+#ifndef PD_RES256_C
+#define PD_RES256_C 8
+#define PD_RES256_NT 512
+#define PD_RES256_MINB 1
+#endif
+template <> struct ResChoice<64>  { static constexpr int C = 2, NT = 256, MINB = 1; };
+template <> struct ResChoice<128> { static constexpr int C = 4, NT = 256, MINB = 1; };
+template <> struct ResChoice<256> { static constexpr int C = PD_RES256_C, NT = PD_RES256_NT, MINB = PD_RES256_MINB; };
 
 template <int N, bool HAS_W, bool ANISO>
 cudaError_t resident_launch_config(cudaLaunchConfig_t *cfg, cudaLaunchAttribute *attr, int nclusters, cudaStream_t st) {
     using Ch = ResChoice<N>;
     using Cfg = pdk::ResCfg<N, Ch::C, Ch::NT>;
-    cudaError_t e = cudaFuncSetAttribute(pdk::resident_kernel<N, Ch::C, Ch::NT, HAS_W, ANISO>,
+    cudaError_t e = cudaFuncSetAttribute(pdk::resident_kernel<N, Ch::C, Ch::NT, Ch::MINB, HAS_W, ANISO>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
     if (e != cudaSuccess) return e;
+    if (Ch::C > 8) {
+        e = cudaFuncSetAttribute(pdk::resident_kernel<N, Ch::C, Ch::NT, Ch::MINB, HAS_W, ANISO>,
+                                 cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
     std::memset(cfg, 0, sizeof(*cfg));
     cfg->gridDim = dim3((unsigned)(nclusters * Ch::C), 1, 1);
     cfg->blockDim = dim3(Ch::NT, 1, 1);
@@ -189,7 +199,7 @@ int resident_max_clusters(int *out) {
     cudaError_t e = resident_launch_config<N, false, false>(&cfg, attr, 1, nullptr);
     if (e != cudaSuccess) return cuda_fail(e, "resident kernel attributes");
     int n = 0;
-    e = cudaOccupancyMaxActiveClusters(&n, pdk::resident_kernel<N, Ch::C, Ch::NT, false, false>, &cfg);
+    e = cudaOccupancyMaxActiveClusters(&n, pdk::resident_kernel<N, Ch::C, Ch::NT, Ch::MINB, false, false>, &cfg);
     if (e != cudaSuccess) return cuda_fail(e, "cudaOccupancyMaxActiveClusters");
     *out = n;
     return PD_OK;
@@ -202,7 +212,7 @@ cudaError_t resident_launch2(const ResidentArgs &a, int nclusters, cudaStream_t 
     cudaLaunchAttribute attr[1];
     cudaError_t e = resident_launch_config<N, HAS_W, ANISO>(&cfg, attr, nclusters, st);
     if (e != cudaSuccess) return e;
-    return cudaLaunchKernelEx(&cfg, pdk::resident_kernel<N, Ch::C, Ch::NT, HAS_W, ANISO>, a);
+    return cudaLaunchKernelEx(&cfg, pdk::resident_kernel<N, Ch::C, Ch::NT, Ch::MINB, HAS_W, ANISO>, a);
 }
 template <int N>
 cudaError_t resident_launch(const ResidentArgs &a, bool w, bool aniso, int nclusters, cudaStream_t st) {

@@ -296,8 +296,8 @@ __device__ __forceinline__ void dipole_col(float2 *zc, const float *__restrict__
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel
-template <int N, int C, int NT, bool HAS_W, bool ANISO>
-__global__ void __launch_bounds__(NT, 1)
+template <int N, int C, int NT, int MINB, bool HAS_W, bool ANISO>
+__global__ void __launch_bounds__(NT, MINB)
 resident_kernel(const ResidentArgs a) {
     using Cfg = ResCfg<N, C, NT>;
     constexpr int E = Cfg::E, T = Cfg::T, RPC = Cfg::RPC, P = N * N;

@@ -49,8 +49,11 @@ enum pd_option {
     PD_OPT_CHECK_EVERY = 3,  /* tolerance tested when (n+1) % value == 0 ; default 1 */
     PD_OPT_MASK_SHARED = 4,  /* 0 (default): mask is [batch][ny][nx] ; 1: one [ny][nx] mask for all slices */
     PD_OPT_UNSAFE_STEPS = 5, /* 1: skip the PD_ESTEP check at the next pd_set_steps call (not at pd_plan) */
-    PD_OPT_KERNEL_TIMING = 6 /* 1: bracket every kernel launch of pd_solve with CUDA events on the caller's stream
+    PD_OPT_KERNEL_TIMING = 6,/* 1: bracket every kernel launch of pd_solve with CUDA events on the caller's stream
                                 (read with pd_get_kernel_times); default 0 */
+    PD_OPT_FOURIER_DUAL = 7  /* 1 (default): when W is the identity keep the dual variable p in the Fourier domain
+                                (one FFT round trip per iteration; same iterates up to rounding);
+                                0: always apply K twice per iteration, literally as PAPER.md:49 */
 };
 /* kernel classes (streaming variant: 0-4; resident variant: one launch, class 5), for pd_get_kernel_times */
 enum pd_kernel_class { PD_KERNEL_INIT = 0, PD_KERNEL_DUAL = 1, PD_KERNEL_COLS = 2, PD_KERNEL_PRIMAL = 3,

@@ -4,6 +4,7 @@
 #include "../../include/pd.h"
 #include "pd_streaming.cuh"
 #include "pd_resident.cuh"
+#include "pd_resident_fd.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -12,6 +13,7 @@
 #include <vector>
 
 using pdk::ResidentArgs;
+using pdk::ResidentFdArgs;
 using pdk::SolveArgs;
 
 namespace {
@@ -38,7 +40,7 @@ struct pd_plan_s {
     int nx, ny, batch, npairs, b0_dir;
     // user-facing parameters (as given) and the effective ones of the rescaled problem (R2)
     float lambda_user, sigma_user, tau_user, theta;
-    int tv_mode, lambda_conv, variant, check_every, mask_shared, unsafe_steps;
+    int tv_mode, lambda_conv, variant, check_every, mask_shared, unsafe_steps, no_fd;
     const float *weight;
     // device tables and workspace
     float *Dtab;
@@ -54,6 +56,7 @@ struct pd_plan_s {
     int res_csize;         // CTAs per cluster
     float2 *res_scratch;   // [kResidentScratchArrays][res_clusters][nx*ny]
     float *rk_part;        // [res_clusters][res_csize][8]
+    float *Dpriv;          // D/(nx*ny) in the thread-private order of the Fourier-domain-dual kernel (pd_resident_fd.cuh)
     // host-buffer entry point staging
     float *h_field, *h_mask, *h_chi;
     int last_launches;
@@ -220,6 +223,53 @@ cudaError_t resident_launch(const ResidentArgs &a, bool w, bool aniso, int nclus
     return aniso ? resident_launch2<N, false, true>(a, nclusters, st) : resident_launch2<N, false, false>(a, nclusters, st);
 }
 
+// ---- Fourier-domain-dual resident kernel (W = identity): same cluster shape and shared-memory budget
+template <int N, bool ANISO>
+cudaError_t resident_fd_launch2(const ResidentFdArgs &a, int nclusters, cudaStream_t st) {
+    using Ch = ResChoice<N>;
+    using Cfg = pdk::ResCfg<N, Ch::C, Ch::NT>;
+    auto kern = pdk::resident_fd_kernel<N, Ch::C, Ch::NT, Ch::MINB, ANISO>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    if (Ch::C > 8) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    std::memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)(nclusters * Ch::C), 1, 1);
+    cfg.blockDim = dim3(Ch::NT, 1, 1);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = st;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = Ch::C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+template <int N>
+cudaError_t resident_fd_launch(const ResidentFdArgs &a, bool aniso, int nclusters, cudaStream_t st) {
+    return aniso ? resident_fd_launch2<N, true>(a, nclusters, st) : resident_fd_launch2<N, false>(a, nclusters, st);
+}
+
+// D/(N*N) in the order the column phase of resident_fd_kernel reads it: [rank][m][tid] (pd_resident_fd.cuh)
+template <int N>
+void build_dipole_private(std::vector<float> &out, const std::vector<float> &D) {
+    using Ch = ResChoice<N>;
+    constexpr int T = pdk::FftCfg<N>::T, E = pdk::FftCfg<N>::E, NT = Ch::NT, C = Ch::C;
+    out.assign((size_t)N * N, 0.f);
+    for (int rank = 0; rank < C; ++rank)
+        for (int m = 0; m < E; ++m)
+            for (int tid = 0; tid < NT; ++tid) {
+                const int cgi = tid / (16 * T), cc = tid % 16, cj = (tid / 16) % T;
+                const int kx = pdk::fd_column_of(N, rank, cgi, cc), ky = cj + T * m;
+                out[(size_t)rank * (N / C) * N + (size_t)m * NT + tid] = D[(size_t)ky * N + kx];
+            }
+}
+
 int resident_csize(int n) { return n == 64 ? ResChoice<64>::C : n == 128 ? ResChoice<128>::C : ResChoice<256>::C; }
 
 int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
@@ -254,6 +304,23 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
     }
     const bool w = p->weight != nullptr, aniso = p->tv_mode == PD_TV_ANISO;
     cudaError_t e;
+    if (!w && !p->no_fd) {
+        // W = identity: the dual variable p stays in the Fourier domain (pd_resident_fd.cuh)
+        ResidentFdArgs f;
+        std::memset(&f, 0, sizeof(f));
+        f.batch = a.batch; f.npairs = a.npairs; f.max_iters = a.max_iters; f.check_every = a.check_every;
+        f.alpha = a.alpha; f.sigma = a.sigma; f.tau = a.tau; f.theta = a.theta;
+        f.inv_one_plus_sigma = a.inv_one_plus_sigma; f.tol = a.tol;
+        f.field = field; f.mask = mask; f.mask_bstride = a.mask_bstride; f.chi_out = chi_out;
+        f.Z = a.Z; f.qy = a.qy; f.chi = a.chi; f.chibar = a.chibar; f.M2 = a.M2; f.phihat = a.phi2;
+        f.Dpriv = p->Dpriv; f.tw_tab = p->tw_row; f.part = p->rk_part;
+        f.iters_done = p->iters_done; f.relgap = p->relgap; f.relres = p->relres;
+        switch (p->nx) {
+            case 64: e = resident_fd_launch<64>(f, aniso, p->res_clusters, st); break;
+            case 128: e = resident_fd_launch<128>(f, aniso, p->res_clusters, st); break;
+            default: e = resident_fd_launch<256>(f, aniso, p->res_clusters, st); break;
+        }
+    } else
     switch (p->nx) {
         case 64: e = resident_launch<64>(a, w, aniso, p->res_clusters, st); break;
         case 128: e = resident_launch<128>(a, w, aniso, p->res_clusters, st); break;
@@ -343,6 +410,17 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
             rc = dev_alloc(&p->res_scratch, (size_t)pdk::kResidentScratchArrays * p->res_clusters * P);
             if (rc == PD_OK) rc = dev_alloc(&p->rk_part, (size_t)p->res_clusters * p->res_csize * 8);
             if (rc != PD_OK) { pd_destroy(p); return rc; }
+            if (rc == PD_OK) rc = dev_alloc(&p->Dpriv, P);
+            if (rc != PD_OK) { pd_destroy(p); return rc; }
+            {
+                std::vector<float> D(P), Dp;
+                build_dipole(D, nx, ny, B0_dir);
+                if (nx == 64) build_dipole_private<64>(Dp, D);
+                else if (nx == 128) build_dipole_private<128>(Dp, D);
+                else build_dipole_private<256>(Dp, D);
+                cudaError_t e2 = cudaMemcpy(p->Dpriv, Dp.data(), P * sizeof(float), cudaMemcpyHostToDevice);
+                if (e2 != cudaSuccess) { pd_destroy(p); return cuda_fail(e2, "private dipole table upload"); }
+            }
             cudaError_t e = cudaMemset(p->rk_part, 0, (size_t)p->res_clusters * p->res_csize * 8 * sizeof(float));
             if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "resident scratch init"); }
             p->res_ok = 1;
@@ -390,6 +468,9 @@ int pd_set_option(pd_plan_t p, int key, int value) {
         case PD_OPT_UNSAFE_STEPS:
             if (value != 0 && value != 1) return PD_EINVAL;
             p->unsafe_steps = value; return PD_OK;
+        case PD_OPT_FOURIER_DUAL:
+            if (value != 0 && value != 1) return PD_EINVAL;
+            p->no_fd = !value; return PD_OK;
         case PD_OPT_KERNEL_TIMING:
             if (value != 0 && value != 1) return PD_EINVAL;
             p->timing = value; return PD_OK;
@@ -537,7 +618,7 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
 int pd_destroy(pd_plan_t p) {
     if (!p) return PD_EINVAL;
     void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->chibar, p->p, p->qx, p->qy, p->Z, p->stop_iter, p->iters_done,
-                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part};
+                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part, p->Dpriv};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (p->ev) for (cudaEvent_t e : *p->ev) cudaEventDestroy(e);

@@ -78,6 +78,22 @@ def test_one_iteration_all_sizes(torch, pd, oracle, ny, nx, variant):
     assert np.all(g["iters_done"] == 1)
 
 
+@pytest.mark.parametrize("n", [64, 128, 256])
+@pytest.mark.parametrize("iters", [1, 2, 5])
+def test_identity_weight_fourier_domain_dual(torch, pd, oracle, n, iters):
+    """W = I: the resident kernel keeps p in the Fourier domain (one FFT round trip per iteration, gap by Parseval
+    over mirror-paired columns).  Same gates as the literal path, and agreement with it (PD_OPT_FOURIER_DUAL = 0)."""
+    case = synth.random_case(n, n, 5, seed=3 * n + iters, with_mask=True)        # odd batch: ragged last pair
+    g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2)
+    o = oracle.solve(case["field"], case["mask"], lambda_=0.2, sigma=0.25, tau=0.25, max_iters=iters)
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-4)
+    assert np.allclose(g["relres"], o["relres"][:, iters - 1], rtol=1e-3)
+    lit = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, options=[(pd.OPT_FOURIER_DUAL, 0)])
+    assert slice_rel(g["chi"], lit["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], lit["relgap"], rtol=1e-4)
+
+
 @pytest.mark.parametrize("iters", [2, 3, 7])
 def test_few_iterations_exercise_q_and_divergence(torch, pd, oracle, iters, variant):
     case = synth.random_case(128, 64, 4, seed=77, with_mask=True, with_weight=True)

@@ -36,6 +36,9 @@ KERNEL_BYTES_PER_PX = {
     "dual_rows": 44.0,    # Z r4 + p rw8 + phi r4 + chibar r4 + qx rw8 + qy rw8 + M r4 + Z w4
     "dipole_cols": 8.0,   # Z r4 + Z w4
     "primal_rows": 32.0,  # Z r4 + chi rw8 + chibar w4 + qx r4 + qy r4 + M r4 + Z w4
+    # W = identity, Fourier-domain dual (pd_streaming_fd.cuh): two launches per iteration, 64 B/px/slice-iteration
+    "fd_cols": 20.0,      # Z r4 w4 + phi^ r4 + p^ r4 w4
+    "fd_rows": 44.0,      # Z r4 w4 + chi r4 w4 + chibar r4 w4 + qx r4 w4 + qy r4 w4 + M r4
 }
 PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
 

@@ -55,9 +55,12 @@ enum pd_option {
                                 (one FFT round trip per iteration; same iterates up to rounding);
                                 0: always apply K twice per iteration, literally as PAPER.md:49 */
 };
-/* kernel classes (streaming variant: 0-4; resident variant: one launch, class 5), for pd_get_kernel_times */
+/* kernel classes for pd_get_kernel_times.  Streaming variant: init, finish and, per iteration, fd_cols + fd_rows
+ * (W = identity, Fourier-domain dual: two launches) or dual_rows + dipole_cols + primal_rows + dipole_cols (W set, or
+ * PD_OPT_FOURIER_DUAL = 0: four launches).  Resident variant: one launch, class 5. */
 enum pd_kernel_class { PD_KERNEL_INIT = 0, PD_KERNEL_DUAL = 1, PD_KERNEL_COLS = 2, PD_KERNEL_PRIMAL = 3,
-                       PD_KERNEL_FINISH = 4, PD_KERNEL_RESIDENT = 5, PD_NUM_KERNEL_CLASSES = 6 };
+                       PD_KERNEL_FINISH = 4, PD_KERNEL_RESIDENT = 5, PD_KERNEL_FD_COLS = 6, PD_KERNEL_FD_ROWS = 7,
+                       PD_NUM_KERNEL_CLASSES = 8 };
 enum { PD_TV_ISO = 0, PD_TV_ANISO = 1 };
 enum { PD_LAMBDA_REG = 0, PD_LAMBDA_DATA = 1 };
 enum { PD_VARIANT_AUTO = 0, PD_VARIANT_STREAMING = 1, PD_VARIANT_RESIDENT = 2 };

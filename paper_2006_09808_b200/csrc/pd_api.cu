@@ -5,6 +5,7 @@
 #include "pd_streaming.cuh"
 #include "pd_resident.cuh"
 #include "pd_resident_fd.cuh"
+#include "pd_streaming_fd.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -15,6 +16,7 @@
 using pdk::ResidentArgs;
 using pdk::ResidentFdArgs;
 using pdk::SolveArgs;
+using pdk::StreamFdArgs;
 
 namespace {
 
@@ -57,6 +59,11 @@ struct pd_plan_s {
     float2 *res_scratch;   // [kResidentScratchArrays][res_clusters][nx*ny]
     float *rk_part;        // [res_clusters][res_csize][8]
     float *Dpriv;          // D/(nx*ny) in the thread-private order of the Fourier-domain-dual kernel (pd_resident_fd.cuh)
+    // streaming variant with the Fourier-domain dual (pd_streaming_fd.cuh): allocated on first use
+    float2 *sfd_planes;    // 11 arrays of [npairs][ny][nx] float2
+    float *sfd_parts;      // per-CTA partial sums
+    int sfd_ncolparts, sfd_nrowparts;
+    int legacy_ok;         // the four-launch streaming workspace (W != I) is allocated
     // host-buffer entry point staging
     float *h_field, *h_mask, *h_chi;
     int last_launches;
@@ -270,6 +277,64 @@ void build_dipole_private(std::vector<float> &out, const std::vector<float> &D) 
             }
 }
 
+
+// ---- streaming workspaces: allocated when a streaming solve is first possible (plan time for sizes without a
+// resident kernel, pd_set_option(PD_OPT_VARIANT, PD_VARIANT_STREAMING) otherwise) so that resident plans stay small
+int ensure_legacy_workspace(pd_plan_s *p) {
+    if (p->legacy_ok) return PD_OK;
+    const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
+    int rc;
+    if ((rc = dev_alloc(&p->chibar, BP)) != PD_OK) return rc;
+    if ((rc = dev_alloc(&p->p, BP)) != PD_OK) return rc;
+    if ((rc = dev_alloc(&p->qx, BP)) != PD_OK) return rc;
+    if ((rc = dev_alloc(&p->qy, BP)) != PD_OK) return rc;
+    if (!p->Z && (rc = dev_alloc(&p->Z, P * (size_t)p->npairs)) != PD_OK) return rc;
+    p->legacy_ok = 1;
+    return PD_OK;
+}
+
+constexpr int kSfdPlanes = 11;   // Z, p^, phi^, chi, M, chibar x2, qx x2, qy x2
+
+int ensure_sfd_workspace(pd_plan_s *p) {
+    if (p->sfd_planes) return PD_OK;
+    const size_t PP = (size_t)p->nx * p->ny * (size_t)p->npairs;
+    p->sfd_ncolparts = p->nx / 16;
+    p->sfd_nrowparts = p->nparts;
+    int rc;
+    if ((rc = dev_alloc(&p->sfd_planes, PP * kSfdPlanes)) != PD_OK) return rc;
+    // p0_part [2], gap_col x2 [2], gap_row [2], res_part [4] per (pair, part)
+    const size_t nparts = (size_t)p->npairs * (size_t)(8 * p->sfd_nrowparts + 4 * p->sfd_ncolparts);
+    if ((rc = dev_alloc(&p->sfd_parts, nparts)) != PD_OK) return rc;
+    cudaError_t e = cudaMemset(p->sfd_parts, 0, nparts * sizeof(float));
+    if (e != cudaSuccess) return cuda_fail(e, "streaming partial sums init");
+    return PD_OK;
+}
+
+template <int NX> void sfd_launch_init_rows(const StreamFdArgs &a, cudaStream_t st) {
+    dim3 grid(a.ny / pdk::SfdRowCfg<NX>::G, a.npairs);
+    pdk::sfd_init_rows_kernel<NX><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a);
+}
+template <int NX> void sfd_launch_rows(const StreamFdArgs &a, int n, cudaStream_t st) {
+    dim3 grid(a.ny / pdk::SfdRowCfg<NX>::G, a.npairs);
+    pdk::sfd_rows_kernel<NX><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+}
+template <int NY> void sfd_launch_init_cols(const StreamFdArgs &a, cudaStream_t st) {
+    dim3 grid(a.nx / 16, a.npairs);
+    pdk::sfd_init_cols_kernel<NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a);
+}
+template <int NY> void sfd_launch_cols(const StreamFdArgs &a, int n, cudaStream_t st) {
+    dim3 grid(a.nx / 16, a.npairs);
+    pdk::sfd_cols_kernel<NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n);
+}
+template <int NY>
+cudaError_t sfd_set_col_smem() {
+    cudaError_t e = cudaFuncSetAttribute(pdk::sfd_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         pdk::SfdColCfg<NY>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(pdk::sfd_init_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                pdk::SfdColCfg<NY>::SMEM_BYTES);
+}
+
 int resident_csize(int n) { return n == 64 ? ResChoice<64>::C : n == 128 ? ResChoice<128>::C : ResChoice<256>::C; }
 
 int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
@@ -335,6 +400,74 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
     return PD_OK;
 }
 
+
+// One launch bracket for PD_OPT_KERNEL_TIMING (shared by the streaming paths)
+#define PD_LAUNCH(cls, stmt)                                                                       \
+    do {                                                                                           \
+        if (p->timing) {                                                                           \
+            while (p->ev->size() < 2 * (size_t)(launches + 1)) {                                   \
+                cudaEvent_t evn_;                                                                  \
+                PD_CUDA(cudaEventCreate(&evn_));                                                   \
+                p->ev->push_back(evn_);                                                            \
+            }                                                                                      \
+            PD_CUDA(cudaEventRecord((*p->ev)[2 * launches], st));                                  \
+        }                                                                                          \
+        stmt;                                                                                      \
+        if (p->timing) {                                                                           \
+            PD_CUDA(cudaEventRecord((*p->ev)[2 * launches + 1], st));                              \
+            p->ev_class->push_back(cls);                                                           \
+        }                                                                                          \
+        ++launches;                                                                                \
+    } while (0)
+
+// Streaming variant, W = identity: two launches per iteration (pd_streaming_fd.cuh)
+int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                       cudaStream_t st) {
+    int rc = ensure_sfd_workspace(p);
+    if (rc != PD_OK) return rc;
+    const size_t P = (size_t)p->nx * p->ny, PP = P * (size_t)p->npairs;
+    StreamFdArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.nx = p->nx; a.ny = p->ny; a.batch = p->batch; a.npairs = p->npairs;
+    a.max_iters = max_iters; a.check_every = p->check_every; a.aniso = p->tv_mode == PD_TV_ANISO;
+    effective_params(p, &a.alpha, &a.sigma, &a.tau);
+    a.theta = p->theta;
+    a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
+    a.tol = tol;
+    a.field = field; a.mask = mask; a.mask_bstride = p->mask_shared ? 0 : (long long)P;
+    a.chi_out = chi_out;
+    float2 *b = p->sfd_planes;
+    a.Z = b; a.phat = b + PP; a.phihat = b + 2 * PP; a.chi2 = b + 3 * PP; a.M2 = b + 4 * PP;
+    a.cb2[0] = b + 5 * PP; a.cb2[1] = b + 6 * PP; a.qx2[0] = b + 7 * PP; a.qx2[1] = b + 8 * PP;
+    a.qy2[0] = b + 9 * PP; a.qy2[1] = b + 10 * PP;
+    a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
+    a.stop_iter = p->stop_iter; a.P0 = p->P0; a.relgap = p->relgap; a.relres = p->relres; a.iters_done = p->iters_done;
+    a.ncolparts = p->sfd_ncolparts; a.nrowparts = p->sfd_nrowparts;
+    const size_t nr = (size_t)p->npairs * a.nrowparts, nc = (size_t)p->npairs * a.ncolparts;
+    float *q = p->sfd_parts;
+    a.p0_part = q; q += 2 * nr;
+    a.gap_row = q; q += 2 * nr;
+    a.res_part = q; q += 4 * nr;
+    a.gap_col[0] = q; q += 2 * nc;
+    a.gap_col[1] = q;
+
+    int launches = 0;
+    p->ev_class->clear();
+    PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->nx, sfd_launch_init_rows, a, st));
+    PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->ny, sfd_launch_init_cols, a, st));
+    for (int n = 0; n < max_iters; ++n) {
+        PD_LAUNCH(PD_KERNEL_FD_COLS, PD_DISPATCH(p->ny, sfd_launch_cols, a, n, st));
+        PD_LAUNCH(PD_KERNEL_FD_ROWS, PD_DISPATCH(p->nx, sfd_launch_rows, a, n, st));
+    }
+    {
+        const int gx = (int)((P + 256 * 8 - 1) / (256 * 8));
+        PD_LAUNCH(PD_KERNEL_FINISH, (pdk::sfd_finish_kernel<<<dim3(gx, p->npairs), 256, 0, st>>>(a)));
+    }
+    PD_CUDA(cudaGetLastError());
+    p->last_launches = launches;
+    return PD_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -363,16 +496,11 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     const int rows_per_cta = (nx == 64 || nx == 128) ? 16 : 8;  // = RowCfg<nx>::G
     p->nparts = ny / rows_per_cta;
 
-    const size_t P = (size_t)nx * ny, BP = P * (size_t)batch;
+    const size_t P = (size_t)nx * ny;
 #define PD_TRY(expr) do { rc = (expr); if (rc != PD_OK) { pd_destroy(p); return rc; } } while (0)
     PD_TRY(dev_alloc(&p->Dtab, P));
     PD_TRY(dev_alloc(&p->tw_row, (size_t)nx));
     PD_TRY(dev_alloc(&p->tw_col, (size_t)ny));
-    PD_TRY(dev_alloc(&p->chibar, BP));
-    PD_TRY(dev_alloc(&p->p, BP));
-    PD_TRY(dev_alloc(&p->qx, BP));
-    PD_TRY(dev_alloc(&p->qy, BP));
-    PD_TRY(dev_alloc(&p->Z, P * (size_t)p->npairs));
     PD_TRY(dev_alloc(&p->stop_iter, (size_t)batch + 1));
     PD_TRY(dev_alloc(&p->iters_done, (size_t)batch));
     PD_TRY(dev_alloc(&p->P0, (size_t)batch));
@@ -397,6 +525,10 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (e == cudaSuccess) e = set_col_smem<128>();
         if (e == cudaSuccess) e = set_col_smem<256>();
         if (e == cudaSuccess) e = set_col_smem<512>();
+        if (e == cudaSuccess) e = sfd_set_col_smem<64>();
+        if (e == cudaSuccess) e = sfd_set_col_smem<128>();
+        if (e == cudaSuccess) e = sfd_set_col_smem<256>();
+        if (e == cudaSuccess) e = sfd_set_col_smem<512>();
         if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "plan table upload"); }
     }
     // resident variant: square slices up to 256x256
@@ -428,6 +560,10 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
             cudaGetLastError();  // no cluster launch possible on this device: the streaming variant remains
         }
     }
+    if (!p->res_ok) {   // streaming is the only path of this plan: take its workspace now
+        rc = ensure_sfd_workspace(p);
+        if (rc != PD_OK) { pd_destroy(p); return rc; }
+    }
     *out = p;
     return PD_OK;
 }
@@ -458,7 +594,8 @@ int pd_set_option(pd_plan_t p, int key, int value) {
         case PD_OPT_VARIANT:
             if (value != PD_VARIANT_AUTO && value != PD_VARIANT_STREAMING && value != PD_VARIANT_RESIDENT) return PD_EINVAL;
             if (value == PD_VARIANT_RESIDENT && !p->res_ok) return PD_EVARIANT;
-            p->variant = value; return PD_OK;
+            p->variant = value;
+            return value == PD_VARIANT_STREAMING ? ensure_sfd_workspace(p) : PD_OK;
         case PD_OPT_CHECK_EVERY:
             if (value < 1) return PD_EINVAL;
             p->check_every = value; return PD_OK;
@@ -486,6 +623,11 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
     const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
 
     if (p->res_ok && p->variant != PD_VARIANT_STREAMING) return solve_resident(p, field, mask, chi_out, max_iters, tol, st);
+    if (!p->weight && !p->no_fd) return solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, st);
+    {
+        const int rc = ensure_legacy_workspace(p);
+        if (rc != PD_OK) return rc;
+    }
 
     SolveArgs a;
     std::memset(&a, 0, sizeof(a));
@@ -506,24 +648,6 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
 
     int launches = 0;
     p->ev_class->clear();
-    // LAUNCH(class, statement): enqueue one kernel; with PD_OPT_KERNEL_TIMING bracket it with two events on `st`
-#define PD_LAUNCH(cls, stmt)                                                                       \
-    do {                                                                                           \
-        if (p->timing) {                                                                           \
-            while (p->ev->size() < 2 * (size_t)(launches + 1)) {                                   \
-                cudaEvent_t evn_;                                                                  \
-                PD_CUDA(cudaEventCreate(&evn_));                                                   \
-                p->ev->push_back(evn_);                                                            \
-            }                                                                                      \
-            PD_CUDA(cudaEventRecord((*p->ev)[2 * launches], st));                                  \
-        }                                                                                          \
-        stmt;                                                                                      \
-        if (p->timing) {                                                                           \
-            PD_CUDA(cudaEventRecord((*p->ev)[2 * launches + 1], st));                              \
-            p->ev_class->push_back(cls);                                                           \
-        }                                                                                          \
-        ++launches;                                                                                \
-    } while (0)
     // chi_0 = p_0 = q_0 = 0, chibar_0 = chi_0; the spectrum of chibar_0 is 0 as well
     PD_CUDA(cudaMemsetAsync(chi_out, 0, BP * sizeof(float), st));
     PD_CUDA(cudaMemsetAsync(p->chibar, 0, BP * sizeof(float), st));
@@ -540,7 +664,6 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
         PD_LAUNCH(PD_KERNEL_PRIMAL, PD_DISPATCH(p->nx, launch_primal, a, n, st));
     }
     PD_LAUNCH(PD_KERNEL_FINISH, (pdk::finish_slices_kernel<<<(p->batch + 127) / 128, 128, 0, st>>>(a, p->iters_done)));
-#undef PD_LAUNCH
     PD_CUDA(cudaGetLastError());
     p->last_launches = launches;
     return PD_OK;
@@ -618,7 +741,8 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
 int pd_destroy(pd_plan_t p) {
     if (!p) return PD_EINVAL;
     void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->chibar, p->p, p->qx, p->qy, p->Z, p->stop_iter, p->iters_done,
-                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part, p->Dpriv};
+                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part, p->Dpriv,
+                    p->sfd_planes, p->sfd_parts};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (p->ev) for (cudaEvent_t e : *p->ev) cudaEventDestroy(e);

@@ -1,0 +1,479 @@
+// pd_streaming_fd.cuh -- streaming variant with the dual variable p kept in the FOURIER domain (W = identity).
+//
+// Same algebra as pd_resident_fd.cuh (PAPER.md:49 line 1 commutes with the FFT when W = I):
+//     p^_{n+1} = (p^_n + sigma (D X^_n - phi^)) / (1 + sigma),   X^_n = F chibar_n,   K p_{n+1} = F^-1 (D p^_{n+1}),
+// so one iteration is ONE forward 2-D FFT and ONE inverse: two launches over the whole batch instead of four,
+//   fd_cols : column FFT of Z (= X^_n), p^ update, column FFT of conj(D/(nx ny) p^_{n+1})      [PAPER.md:49 line 1]
+//   fd_rows : row FFT (finishes K p_{n+1}), q-update, G^T M q_{n+1}, chi-update, over-relaxation,
+//             row FFT of chibar_{n+1}                                                         [PAPER.md:49 lines 2-4]
+// All state is pair-interleaved float2 [npairs][ny][nx] (lane x = slice 2j, lane y = slice 2j+1): every access of a
+// group of T threads is one contiguous 8T-byte segment.  chibar and q are double-buffered by iteration parity, so
+// that a row group can redo the q-update of the row ABOVE its own (it needs (M qy_{n+1})[y-1] for the divergence)
+// from read-only data: no exchange between rows, no CTA-wide barrier; the duplicate loads hit L1/L2.
+//
+// HBM bytes per pixel PAIR and iteration: fd_cols Z r8 w8, phi^ r8, p^ r8 w8 = 40 ; fd_rows Z r8 w8, chi r8 w8,
+// chibar r8 w8, qx r8 w8, qy r8 w8, M r8 = 88  ->  64 B per pixel of one slice and iteration.
+//
+// Gap (R9): data term by Parseval over mirror-paired columns (as in pd_resident_fd.cuh), q term in fd_rows;
+// both as per-CTA partial sums.  Every CTA of fd_cols(n+1) reduces the partials of iteration n in the same fixed
+// order and reaches the same stop decision; column block 0 records it.  No host round trip.
+#pragma once
+#include "pd_resident.cuh"    // packed fp32x2 helpers, FFT building blocks
+#include "pd_streaming.cuh"   // group_sum
+
+namespace pdk {
+
+struct StreamFdArgs {
+    int nx, ny, batch, npairs, max_iters, check_every, aniso;
+    float alpha, sigma, tau, theta, inv_one_plus_sigma, tol;
+    const float *field, *mask;
+    long long mask_bstride;
+    float *chi_out;
+    float2 *Z, *phat, *phihat, *chi2, *M2;   // [npairs][ny][nx]
+    float2 *cb2[2], *qx2[2], *qy2[2];        // double-buffered by iteration parity
+    const float *Dtab;                       // D/(nx*ny), [ny][nx]
+    const float2 *tw_row, *tw_col;
+    int *stop_iter;                          // slice b is active in iteration n (0-based) iff n < stop_iter[b]
+    float *P0, *relgap, *relres;
+    int *iters_done;
+    float *p0_part;                          // [npairs][nrowparts][2]
+    float *gap_col[2];                       // [npairs][ncolparts][2], by iteration parity
+    float *gap_row;                          // [npairs][nrowparts][2]
+    float *res_part;                         // [npairs][nrowparts][4] (dn_a, cn_a, dn_b, cn_b)
+    int ncolparts, nrowparts;
+};
+
+template <int N> struct SfdRowCfg {
+    static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
+    static constexpr int THREADS = 128;
+    static constexpr int G = THREADS / T;
+    static constexpr int LD = T + 1;
+    static constexpr int SM_PER_GROUP = E * LD;
+};
+template <int N> struct SfdColCfg {
+    static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
+    static constexpr int HALF = 8, COLS = 16;          // 8 adjacent columns and their 8 mirror images
+    static constexpr int THREADS = COLS * T;
+    static constexpr int CS = N + 1;
+    static constexpr int SMEM_BYTES = (COLS * CS + E * T) * (int)sizeof(float2) + 128;
+};
+
+// column kx of (column block cb, half h, slot cc): [8cb, 8cb+8) and its mirror images nx - kx; the self-mirrored
+// columns 0 and nx/2 both sit in block 0, slot 0.
+__host__ __device__ constexpr int sfd_column_of(int nx, int cb, int h, int cc) {
+    const int lo = 8 * cb + cc;
+    return h == 0 ? lo : (lo == 0 ? nx / 2 : nx - lo);
+}
+
+// relgap of the pair's two lanes from the partial sums of iteration parity `par`, fixed order (same in every CTA)
+__device__ __forceinline__ float2 sfd_gap_sum(const StreamFdArgs &a, int pair, int par) {
+    float ga = 0.f, gb = 0.f;
+    const float *gc = a.gap_col[par] + (long long)pair * a.ncolparts * 2;
+    for (int k = 0; k < a.ncolparts; ++k) { ga += __ldcg(gc + 2 * k); gb += __ldcg(gc + 2 * k + 1); }
+    const float *gr = a.gap_row + (long long)pair * a.nrowparts * 2;
+    for (int k = 0; k < a.nrowparts; ++k) { ga += __ldcg(gr + 2 * k); gb += __ldcg(gr + 2 * k + 1); }
+    return make_float2(ga, gb);
+}
+
+// ------------------------------------------------------------------------------------------------ init
+// Load the pair's field rows, interleave the mask, zero the state that iteration 0 reads, partial sums of
+// 1/2 ||phi||^2, row FFT of phi -> Z.  (chi_0 = chibar_0 = p_0 = q_0 = 0.)
+template <int NX>
+__global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS)
+sfd_init_rows_kernel(const StreamFdArgs a) {
+    using Cfg = SfdRowCfg<NX>;
+    constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
+    __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
+    __shared__ float2 tws[E * T];
+    __shared__ float red[G][2];
+    TwiddlesSmem<NX>::fill(tws, a.tw_row, threadIdx.x, Cfg::THREADS);
+    __syncthreads();
+    const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
+    const bool has_b = s1 < a.batch;
+    const int g = threadIdx.x / T, j = threadIdx.x % T;
+    const int y = blockIdx.x * G + g;
+    const long long P = (long long)NX * a.ny, rowoff = (long long)y * NX, po = (long long)pair * P + rowoff;
+    TwiddlesSmem<NX> tw;
+    tw.w = tws + j;
+    const float *fa = a.field + (long long)s0 * P + rowoff;
+    const float *fb = a.field + (long long)s1 * P + rowoff;
+    const float *ma = a.mask ? a.mask + s0 * a.mask_bstride + rowoff : nullptr;
+    const float *mb = a.mask ? a.mask + s1 * a.mask_bstride + rowoff : nullptr;
+    const float2 zero = make_float2(0.f, 0.f);
+    float2 v[E];
+    float acc0 = 0.f, acc1 = 0.f;
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int x = j + T * m;
+        const float va = fa[x], vb = has_b ? fb[x] : 0.f;
+        v[m] = make_float2(va, vb);
+        acc0 = fmaf(va, va, acc0);
+        acc1 = fmaf(vb, vb, acc1);
+        a.M2[po + x] = make_float2(ma ? ma[x] : 1.f, has_b ? (mb ? mb[x] : 1.f) : 0.f);
+        a.chi2[po + x] = zero; a.cb2[0][po + x] = zero; a.qx2[0][po + x] = zero; a.qy2[0][po + x] = zero;
+    }
+    fft_line<NX, Cfg::LD>(v, sm + g * Cfg::SM_PER_GROUP, j, tw, WarpSync());
+#pragma unroll
+    for (int m = 0; m < E; ++m) a.Z[po + j + T * m] = v[m];
+    acc0 = group_sum<T>(acc0);
+    acc1 = group_sum<T>(acc1);
+    if (j == 0) { red[g][0] = acc0; red[g][1] = acc1; }
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        float t = 0.f;
+        for (int k = 0; k < G; ++k) t += red[k][threadIdx.x];
+        a.p0_part[((long long)pair * a.nrowparts + blockIdx.x) * 2 + threadIdx.x] = t;
+    }
+}
+
+// phi^ = column FFT of the row-transformed field; p^_0 = 0; column block 0 finishes P0 and resets the per-slice state.
+template <int NY>
+__global__ void __launch_bounds__(SfdColCfg<NY>::THREADS)
+sfd_init_cols_kernel(const StreamFdArgs a) {
+    using Cfg = SfdColCfg<NY>;
+    constexpr int E = Cfg::E, T = Cfg::T;
+    extern __shared__ __align__(16) unsigned char sfd_smem[];
+    float2 *smc = reinterpret_cast<float2 *>(sfd_smem);
+    float2 *tws = smc + Cfg::COLS * Cfg::CS;
+    TwiddlesSmem<NY>::fill(tws, a.tw_col, threadIdx.x, Cfg::THREADS);
+    __syncthreads();
+    const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
+    const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
+    const int kx = sfd_column_of(a.nx, blockIdx.x, c >> 3, c & 7);
+    const long long po = (long long)pair * a.nx * NY + kx;
+    TwiddlesSmem<NY> tw;
+    tw.w = tws + j;
+    float2 v[E];
+#pragma unroll
+    for (int m = 0; m < E; ++m) v[m] = a.Z[po + (long long)(j + T * m) * a.nx];
+    fft_line<NY, T>(v, smc + c * Cfg::CS, j, tw, BlockSync());
+    const float2 zero = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        a.phihat[po + (long long)(j + T * m) * a.nx] = v[m];
+        a.phat[po + (long long)(j + T * m) * a.nx] = zero;
+    }
+    if (blockIdx.x == 0 && threadIdx.x < 2) {
+        const int b = threadIdx.x ? s1 : s0;
+        if (b < a.batch) {
+            float t = 0.f;
+            const float *pp = a.p0_part + (long long)pair * a.nrowparts * 2 + threadIdx.x;
+            for (int k = 0; k < a.nrowparts; ++k) t += pp[2 * k];
+            const float P0 = 0.5f * t;
+            a.P0[b] = P0;
+            a.relgap[b] = 0.f;
+            a.relres[b] = 0.f;
+            a.stop_iter[b] = (P0 == 0.f) ? 0 : a.max_iters;   // R13b: an all-zero slice is never scheduled
+        }
+    }
+    if (blockIdx.x == 0)
+        for (int k = threadIdx.x; k < a.nrowparts * 4; k += Cfg::THREADS) a.res_part[(long long)pair * a.nrowparts * 4 + k] = 0.f;
+}
+
+// ------------------------------------------------------------------------------------------------ column kernel
+// Iteration n.  First the stop decision of iteration n-1 (if it was a checking iteration): every CTA of the pair
+// reduces the same partial sums in the same order; block 0 records relgap and stop_iter.  Then
+//   X^ = column FFT of Z (zero when n == 0) ; p^_{n+1} = (p^_n + sigma (D X^ - phi^))/(1 + sigma) ;
+//   Z <- column FFT of conj(D/(nx ny) p^_{n+1})      (the row kernel's FFT finishes the inverse transform)
+// want_gap: S1 = sum |dp|^2, S2 = Re sum dp(k) dp(-k), dp = p^_{n+1} - p^_n; the mirror column is in this CTA.
+template <int NY>
+__global__ void __launch_bounds__(SfdColCfg<NY>::THREADS, SfdColCfg<NY>::THREADS <= 128 ? 4 : 2)
+sfd_cols_kernel(const StreamFdArgs a, const int n) {
+    using Cfg = SfdColCfg<NY>;
+    constexpr int E = Cfg::E, T = Cfg::T, NT = Cfg::THREADS;
+    extern __shared__ __align__(16) unsigned char sfd_smem[];
+    float2 *smc = reinterpret_cast<float2 *>(sfd_smem);
+    float2 *tws = smc + Cfg::COLS * Cfg::CS;
+    float *dec = reinterpret_cast<float *>(tws + E * T);   // [0..1] stop flags of this launch ; [2..] reduction
+
+    const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
+    const bool has_b = s1 < a.batch;
+    int stop0 = a.stop_iter[s0], stop1 = has_b ? a.stop_iter[s1] : 0;
+    if (n >= stop0 && n >= stop1) return;
+
+    const bool decide = n > 0 && a.tol > 0.f && (n % a.check_every) == 0;   // iteration n-1 was a checking one
+    if (decide) {
+        if (threadIdx.x == 0) {
+            const float2 g = sfd_gap_sum(a, pair, (n - 1) & 1);
+            const float P0a = a.P0[s0], P0b = has_b ? a.P0[s1] : 0.f;
+            const float ra = P0a > 0.f ? g.x / P0a : 0.f, rb = P0b > 0.f ? g.y / P0b : 0.f;
+            int f0 = 0, f1 = 0;
+            if (n < stop0 && ra < a.tol) f0 = 1;
+            if (n < stop1 && rb < a.tol) f1 = 1;
+            dec[0] = (float)f0; dec[1] = (float)f1;
+            if (blockIdx.x == 0) {
+                if (n < stop0) { a.relgap[s0] = ra; if (f0) a.stop_iter[s0] = n; }
+                if (n < stop1) { a.relgap[s1] = rb; if (f1) a.stop_iter[s1] = n; }
+            }
+        }
+        __syncthreads();
+        if (dec[0] != 0.f) stop0 = n;
+        if (dec[1] != 0.f) stop1 = n;
+        if (n >= stop0 && n >= stop1) return;
+    }
+    const bool last = (n + 1 == a.max_iters);
+    const bool want_gap = last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0);
+
+    TwiddlesSmem<NY>::fill(tws, a.tw_col, threadIdx.x, NT);
+    const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
+    const int h = c >> 3, cc = c & 7;
+    const int nx = a.nx;
+    const int kx = sfd_column_of(nx, blockIdx.x, h, cc);
+    const bool self_mirror = (blockIdx.x == 0 && cc == 0);
+    float2 *smg = smc + c * Cfg::CS;
+    const float2 *smg_mir = self_mirror ? smg : smc + (c ^ 8) * Cfg::CS;
+    const long long po = (long long)pair * nx * NY + kx;
+    float2 *zc = a.Z + po, *ph = a.phat + po;
+    const float2 *phh = a.phihat + po;
+    const float *dcol = a.Dtab + kx;
+    TwiddlesSmem<NY> tw;
+    tw.w = tws + j;
+    __syncthreads();
+
+    float2 v[E];
+    if (n > 0) {
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = __ldcs(zc + (long long)(j + T * m) * nx);
+        fft_line<NY, T>(v, smg, j, tw, BlockSync());
+    } else {
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = make_float2(0.f, 0.f);
+    }
+    const float2 sig2 = splat(a.sigma), inv2 = splat(a.inv_one_plus_sigma);
+    const float NN = (float)nx * (float)NY;
+    float S1 = 0.f, S2 = 0.f;
+    if (want_gap) __syncthreads();   // the exchange region is free (readers of the FFT above are done)
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const long long o = (long long)(j + T * m) * nx;
+        const float d = __ldg(dcol + o);
+        const float2 phat = __ldcs(phh + o);
+        const float2 pold = __ldcs(ph + o);
+        const float2 res = sub2(mul2(splat(d * NN), v[m]), phat);
+        const float2 pn = mul2(fma2(sig2, res, pold), inv2);
+        if (want_gap) {
+            const float2 dp = sub2(pn, pold);
+            S1 = fmaf(dp.x, dp.x, fmaf(dp.y, dp.y, S1));
+            smg[j + T * m] = dp;
+        }
+        __stcs(ph + o, pn);
+        v[m] = make_float2(d * pn.x, -d * pn.y);
+    }
+    if (want_gap) {
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const int ky = j + T * m;
+            const float2 dp = smg[ky];
+            const float2 dm = smg_mir[(NY - ky) & (NY - 1)];
+            S2 = fmaf(dp.x, dm.x, fmaf(-dp.y, dm.y, S2));
+        }
+    }
+    fft_line<NY, T>(v, smg, j, tw, BlockSync());
+#pragma unroll
+    for (int m = 0; m < E; ++m) __stcs(zc + (long long)(j + T * m) * nx, v[m]);
+
+    if (want_gap) {   // CTA sums in fixed order: warp shuffles, then warp 0 over the per-warp values
+        __syncthreads();
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            S1 += __shfl_xor_sync(0xffffffffu, S1, o);
+            S2 += __shfl_xor_sync(0xffffffffu, S2, o);
+        }
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        if (lane == 0) { dec[2 + 2 * warp] = S1; dec[3 + 2 * warp] = S2; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float t1 = 0.f, t2 = 0.f;
+            for (int w = 0; w < NT / 32; ++w) { t1 += dec[2 + 2 * w]; t2 += dec[3 + 2 * w]; }
+            // 1/2 sum_x e^2 = (S1 +- S2) / (4 nx ny sigma^2)   (Parseval; pd_resident_fd.cuh header)
+            const float scale = 0.25f / (NN * a.sigma * a.sigma);
+            float *gc = a.gap_col[n & 1] + ((long long)pair * a.ncolparts + blockIdx.x) * 2;
+            gc[0] = scale * (t1 + t2);
+            gc[1] = scale * (t1 - t2);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ row kernel
+// isotropic / anisotropic projection of (tx, ty) onto the alpha-ball, both lanes (PAPER.md:49 line 2; R4, R13)
+__device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float alpha, const float alpha_sq, const bool aniso) {
+    if (aniso) {
+        tx.x = fminf(fmaxf(tx.x, -alpha), alpha); tx.y = fminf(fmaxf(tx.y, -alpha), alpha);
+        ty.x = fminf(fmaxf(ty.x, -alpha), alpha); ty.y = fminf(fmaxf(ty.y, -alpha), alpha);
+    } else {
+        const float2 n2 = fma2(ty, ty, mul2(tx, tx));
+        float2 sc;
+        sc.x = (n2.x > alpha_sq) ? alpha * rsqrtf(n2.x) : 1.f;
+        sc.y = (n2.y > alpha_sq) ? alpha * rsqrtf(n2.y) : 1.f;
+        tx = mul2(tx, sc);
+        ty = mul2(ty, sc);
+    }
+}
+
+// Iteration n, one row y per group of T threads (same warp):
+//   v = K p_{n+1}: row FFT of Z gives (v_a, -v_b)
+//   q_{n+1} = proj_alpha(q_n + sigma M G chibar_n) for row y (stored) and, redundantly, its qy for row y-1
+//   d = G^T (M q_{n+1}) ; chi_{n+1} = chi_n - tau (v + d) ; chibar_{n+1} = chi_{n+1} + theta (chi_{n+1} - chi_n)
+//   Z <- row FFT of chibar_{n+1}
+template <int NX>
+__global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, NX == 512 ? 3 : 4)
+sfd_rows_kernel(const StreamFdArgs a, const int n) {
+    using Cfg = SfdRowCfg<NX>;
+    constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
+    __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
+    __shared__ float2 tws[E * T];
+    __shared__ float red[G][6];
+
+    const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
+    const bool act0 = n < a.stop_iter[s0];
+    const bool act1 = (s1 < a.batch) && (n < a.stop_iter[s1]);
+    if (!act0 && !act1) return;
+    const bool last = (n + 1 == a.max_iters);
+    const bool want_gap = last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0);
+
+    TwiddlesSmem<NX>::fill(tws, a.tw_row, threadIdx.x, Cfg::THREADS);
+    const int g = threadIdx.x / T, j = threadIdx.x % T;
+    const int y = blockIdx.x * G + g;
+    const int ny = a.ny;
+    float2 *smg = sm + g * Cfg::SM_PER_GROUP;
+    TwiddlesSmem<NX> tw;
+    tw.w = tws + j;
+    const long long po = ((long long)pair * ny + y) * NX;
+    const int rd = n & 1, wr = rd ^ 1;
+    float2 *zr = a.Z + po;
+    const float2 *cbr = a.cb2[rd] + po, *qxr = a.qx2[rd] + po, *qyr = a.qy2[rd] + po, *M = a.M2 + po;
+    float2 *cbw = a.cb2[wr] + po, *qxw = a.qx2[wr] + po, *qyw = a.qy2[wr] + po, *chi = a.chi2 + po;
+    const bool has_up = y > 0, has_down = y < ny - 1;
+
+    float2 v[E];
+#pragma unroll
+    for (int m = 0; m < E; ++m) v[m] = __ldcs(zr + j + T * m);
+    __syncthreads();   // twiddle table
+    fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
+
+    const float2 sig2 = splat(a.sigma), zero = make_float2(0.f, 0.f);
+    const float alpha = a.alpha, alpha_sq = a.alpha * a.alpha;
+    const bool aniso = a.aniso != 0;
+    const float2 ntau2 = splat(-a.tau), ntau_v = make_float2(-a.tau, a.tau), theta2 = splat(a.theta);
+    const float2 actm = make_float2(act0 ? 1.f : 0.f, act1 ? 1.f : 0.f);
+    float2 gap = zero, dn = zero, cn = zero, mqx_prev = zero;
+    float2 c0n = __ldg(cbr + j), cun = has_up ? __ldg(cbr - NX + j) : zero;
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int x = j + T * m;
+        const float2 c0 = c0n, cu = cun;                       // chibar_n[y][x], chibar_n[y-1][x]
+        if (m + 1 < E) { c0n = __ldg(cbr + x + T); cun = has_up ? __ldg(cbr - NX + x + T) : zero; }
+        const float2 cd = has_down ? __ldg(cbr + NX + x) : c0; // Neumann: no row below -> gy = 0
+        // right neighbours [.][x+1]: lane j+1 (same m), or lane 0's element m+1 when j == T-1
+        const float2 give0 = (j == 0 && m + 1 < E) ? c0n : c0;
+        const float2 giveu = (j == 0 && m + 1 < E) ? cun : cu;
+        float2 cr = shfl2(give0, (j + 1) & (T - 1), T);
+        float2 cur = shfl2(giveu, (j + 1) & (T - 1), T);
+        if (m == E - 1 && j == T - 1) { cr = c0; cur = cu; }   // Neumann: no column to the right -> gx = 0
+        const float2 mm = __ldg(M + x);
+        // own row: q_{n+1}[y][x]
+        const float2 gx = mul2(mm, sub2(cr, c0));
+        const float2 gy = mul2(mm, sub2(cd, c0));
+        float2 tx = fma2(sig2, gx, __ldcs(qxr + x));
+        float2 ty = fma2(sig2, gy, __ldcs(qyr + x));
+        sfd_project(tx, ty, alpha, alpha_sq, aniso);
+        __stcs(qxw + x, tx);
+        __stcs(qyw + x, ty);
+        if (want_gap) {   // alpha |g| - <g, q_{n+1}>
+            float2 gn;
+            if (aniso) {
+                gn = make_float2(fabsf(gx.x) + fabsf(gy.x), fabsf(gx.y) + fabsf(gy.y));
+            } else {
+                const float2 g2 = fma2(gy, gy, mul2(gx, gx));
+                gn = make_float2(sqrtf(g2.x), sqrtf(g2.y));
+            }
+            gap = add2(gap, sub2(mul2(splat(alpha), gn), fma2(gy, ty, mul2(gx, tx))));
+        }
+        // row above, redundantly: (M qy_{n+1})[y-1][x]
+        float2 mqy_up = zero;
+        if (has_up) {
+            const float2 mu = __ldg(M - NX + x);
+            float2 ux = fma2(sig2, mul2(mu, sub2(cur, cu)), __ldg(qxr - NX + x));
+            float2 uy = fma2(sig2, mul2(mu, sub2(c0, cu)), __ldg(qyr - NX + x));
+            sfd_project(ux, uy, alpha, alpha_sq, aniso);
+            mqy_up = mul2(mu, uy);
+        }
+        // d = G^T (M q) = -div(M q): qx is 0 in the last column and qy in the last row, so no predicate
+        const float2 mqx = mul2(mm, tx);
+        const float2 give = (j == T - 1 && m > 0) ? mqx_prev : mqx;
+        float2 left = shfl2(give, (j + T - 1) & (T - 1), T);   // (M qx)[y][x-1]
+        if (m == 0 && j == 0) left = zero;
+        const float2 d = add2(sub2(left, mqx), sub2(mqy_up, mul2(mm, ty)));
+        mqx_prev = mqx;
+        // chi_{n+1}, chibar_{n+1}; a lane whose slice has stopped keeps its chi
+        const float2 c_old = __ldcs(chi + x);
+        const float2 step = fma2(ntau2, d, mul2(ntau_v, v[m]));
+        const float2 c_new = fma2(actm, step, c_old);
+        const float2 dc = sub2(c_new, c_old);
+        dn = fma2(dc, dc, dn);
+        cn = fma2(c_new, c_new, cn);
+        const float2 cbar = fma2(theta2, dc, c_new);
+        __stcs(chi + x, c_new);
+        cbw[x] = cbar;
+        v[m] = cbar;
+    }
+    if (!last) {   // the stop decision of this iteration is taken by the next column kernel
+        fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
+#pragma unroll
+        for (int m = 0; m < E; ++m) __stcs(zr + j + T * m, v[m]);
+    }
+
+    // per-CTA partial sums, fixed order
+    float s6[6] = {gap.x, gap.y, dn.x, cn.x, dn.y, cn.y};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) s6[k] = group_sum<T>(s6[k]);
+    if (j == 0) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) red[g][k] = s6[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        const int k = threadIdx.x;
+        float t = 0.f;
+        for (int q = 0; q < G; ++q) t += red[q][k];
+        const long long part = (long long)pair * a.nrowparts + blockIdx.x;
+        if (k < 2) { if (want_gap) a.gap_row[part * 2 + k] = t; }
+        else if ((k < 4) ? act0 : act1) a.res_part[part * 4 + (k - 2)] = t;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ finish
+// chi_N of every slice -> the caller's planes (S7); column... block 0 of the pair: relgap of slices that ran to
+// max_iters (the others recorded theirs when they stopped), relres, iters_done.
+__global__ void __launch_bounds__(256)
+sfd_finish_kernel(const StreamFdArgs a) {
+    const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
+    const bool has_b = s1 < a.batch;
+    const long long P = (long long)a.nx * a.ny;
+    const float2 *c2 = a.chi2 + (long long)pair * P;
+    float *oa = a.chi_out + (long long)s0 * P, *ob = a.chi_out + (long long)s1 * P;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P; i += (long long)gridDim.x * blockDim.x) {
+        const float2 c = __ldcs(c2 + i);
+        oa[i] = c.x;
+        if (has_b) ob[i] = c.y;
+    }
+    if (blockIdx.x == 0 && threadIdx.x < 2 && (threadIdx.x == 0 || has_b)) {
+        const int s = threadIdx.x, b = s ? s1 : s0;
+        const int stop = a.stop_iter[b];
+        const float P0 = a.P0[b];
+        if (stop >= a.max_iters && a.max_iters > 0 && P0 > 0.f) {
+            const float2 g = sfd_gap_sum(a, pair, (a.max_iters - 1) & 1);
+            a.relgap[b] = (s ? g.y : g.x) / P0;
+        }
+        float dn = 0.f, cn = 0.f;
+        if (stop > 0) {
+            const float *rp = a.res_part + (long long)pair * a.nrowparts * 4 + 2 * s;
+            for (int k = 0; k < a.nrowparts; ++k) { dn += rp[4 * k]; cn += rp[4 * k + 1]; }
+        }
+        a.relres[b] = (cn > 0.f) ? sqrtf(dn) / sqrtf(cn) : 0.f;
+        a.iters_done[b] = (P0 == 0.f && !(a.tol > 0.f)) ? a.max_iters : min(stop, a.max_iters);
+    }
+}
+
+}  // namespace pdk

@@ -94,6 +94,26 @@ def test_identity_weight_fourier_domain_dual(torch, pd, oracle, n, iters):
     assert np.allclose(g["relgap"], lit["relgap"], rtol=1e-4)
 
 
+@pytest.mark.parametrize("ny,nx", [(64, 64), (128, 128), (256, 256), (512, 512), (64, 256), (512, 128), (128, 64)])
+@pytest.mark.parametrize("iters", [1, 2, 5])
+def test_streaming_fourier_domain_dual(torch, pd, oracle, ny, nx, iters):
+    """W = I, streaming variant: two launches per iteration (pd_streaming_fd.cuh), every size including non-square.
+    Same gates as the literal four-launch path (PD_OPT_FOURIER_DUAL = 0), and agreement with it."""
+    case = synth.random_case(nx, ny, 5, seed=nx + 3 * ny + iters, with_mask=True)   # odd batch: ragged last pair
+    g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, variant="streaming")
+    assert g["launches"] == 2 * iters + 3
+    o = oracle.solve(case["field"], case["mask"], lambda_=0.2, sigma=0.25, tau=0.25, max_iters=iters)
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-4)
+    assert np.allclose(g["relres"], o["relres"][:, iters - 1], rtol=1e-3)
+    assert np.all(g["iters_done"] == iters)
+    lit = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, variant="streaming",
+                    options=[(pd.OPT_FOURIER_DUAL, 0)])
+    assert lit["launches"] == 4 * iters + 1
+    assert slice_rel(g["chi"], lit["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], lit["relgap"], rtol=1e-4)
+
+
 @pytest.mark.parametrize("iters", [2, 3, 7])
 def test_few_iterations_exercise_q_and_divergence(torch, pd, oracle, iters, variant):
     case = synth.random_case(128, 64, 4, seed=77, with_mask=True, with_weight=True)

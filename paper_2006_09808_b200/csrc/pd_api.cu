@@ -293,7 +293,7 @@ int ensure_legacy_workspace(pd_plan_s *p) {
     return PD_OK;
 }
 
-constexpr int kSfdPlanes = 11;   // Z, p^, phi^, chi, M, chibar x2, qx x2, qy x2
+constexpr int kSfdPlanes = 13;   // Z, phi^, M, and p^, chi, chibar, qx, qy twice each
 
 int ensure_sfd_workspace(pd_plan_s *p) {
     if (p->sfd_planes) return PD_OK;
@@ -437,9 +437,11 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     a.field = field; a.mask = mask; a.mask_bstride = p->mask_shared ? 0 : (long long)P;
     a.chi_out = chi_out;
     float2 *b = p->sfd_planes;
-    a.Z = b; a.phat = b + PP; a.phihat = b + 2 * PP; a.chi2 = b + 3 * PP; a.M2 = b + 4 * PP;
-    a.cb2[0] = b + 5 * PP; a.cb2[1] = b + 6 * PP; a.qx2[0] = b + 7 * PP; a.qx2[1] = b + 8 * PP;
-    a.qy2[0] = b + 9 * PP; a.qy2[1] = b + 10 * PP;
+    a.Z = b; a.phihat = b + PP; a.M2 = b + 2 * PP;
+    for (int k = 0; k < 2; ++k) {
+        a.phat[k] = b + (3 + k) * PP; a.chi2[k] = b + (5 + k) * PP; a.cb2[k] = b + (7 + k) * PP;
+        a.qx2[k] = b + (9 + k) * PP; a.qy2[k] = b + (11 + k) * PP;
+    }
     a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
     a.stop_iter = p->stop_iter; a.P0 = p->P0; a.relgap = p->relgap; a.relres = p->relres; a.iters_done = p->iters_done;
     a.ncolparts = p->sfd_ncolparts; a.nrowparts = p->sfd_nrowparts;

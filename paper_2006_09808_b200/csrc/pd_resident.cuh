@@ -149,18 +149,31 @@ __device__ __forceinline__ void q_update_row(const RowPtrs &r, const ResidentArg
     float2 c0[E];
 #pragma unroll
     for (int m = 0; m < E; ++m) c0[m] = ldcg2(r.chibar + j + T * m);
+    // operands are loaded a chunk ahead of the stores: a load cannot be scheduled above an earlier store to a
+    // possibly aliasing address, so a load-use-store loop body would expose one L2 latency per element
+    constexpr int CH = 8;
+    float2 cdv[CH], mmv[CH], qyv[CH];
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int x = j + T * m;
-        const float2 cd = has_down ? ldcg2(r.chibar + N + x) : c0[m];    // Neumann: no row below -> gy = 0
+        if (m % CH == 0) {
+#pragma unroll
+            for (int k = 0; k < CH; ++k) {
+                const int xk = x + T * k;
+                cdv[k] = has_down ? ldcg2(r.chibar + N + xk) : c0[m + k];   // Neumann: no row below -> gy = 0
+                mmv[k] = ldcg2(r.M2 + xk);
+                qyv[k] = ldcg2(r.qy + xk);
+            }
+        }
+        const float2 cd = cdv[m % CH];
         const float2 give = (j == 0 && m + 1 < E) ? c0[m + 1 < E ? m + 1 : m] : c0[m];
         float2 cr = shfl2(give, (j + 1) & (T - 1), T);                   // chibar[y][x+1]
         if (m == E - 1 && j == T - 1) cr = c0[m];                        // Neumann: no column to the right -> gx = 0
-        const float2 mm = r.M2[x];
+        const float2 mm = mmv[m % CH];
         const float2 gx = mul2(mm, sub2(cr, c0[m]));
         const float2 gy = mul2(mm, sub2(cd, c0[m]));
         float2 tx = fma2(sig2, gx, r.qx_s[m * NT]);
-        float2 ty = fma2(sig2, gy, r.qy[x]);
+        float2 ty = fma2(sig2, gy, qyv[m % CH]);
         if (ANISO) {
             tx.x = fminf(fmaxf(tx.x, -alpha), alpha);
             tx.y = fminf(fmaxf(tx.y, -alpha), alpha);
@@ -256,10 +269,16 @@ __device__ __forceinline__ void primal_z_row(const RowPtrs &r, const ResidentArg
     for (int m = 0; m < E; ++m) v[m] = ldcg2(r.Z + j + T * m);
     fft_line<N, LDR>(v, smg, j, tw, WarpSync());  // v = (v_a, v_b)
     const float2 ntau2 = splat(-a.tau), theta2 = splat(a.theta);
+    constexpr int CH = 8;   // chi is loaded a chunk ahead of the stores (see q_update_row)
+    float2 cov[CH];
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int x = j + T * m;
-        const float2 c_old = r.chi[x];
+        if (m % CH == 0) {
+#pragma unroll
+            for (int k = 0; k < CH; ++k) cov[k] = ldcg2(r.chi + x + T * k);
+        }
+        const float2 c_old = cov[m % CH];
         const float2 c_new = fma2(ntau2, d[m], fma2(ntau2, v[m], c_old));
         const float2 dc = sub2(c_new, c_old);
         dn = fma2(dc, dc, dn);

@@ -118,10 +118,16 @@ __device__ __forceinline__ void primal_fd_row(const RowPtrs &r, const ResidentFd
     for (int m = 0; m < E; ++m) v[m] = ldcg2(r.Z + j + T * m);
     fft_line<N, LDR>(v, smg, j, tw, WarpSync());
     const float2 ntau2 = splat(-a.tau), ntau_v = make_float2(-a.tau, a.tau), theta2 = splat(a.theta);
+    constexpr int CH = 8;   // chi is loaded a chunk ahead of the stores (see q_update_row)
+    float2 cov[CH];
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int x = j + T * m;
-        const float2 c_old = ldcg2(r.chi + x);
+        if (m % CH == 0) {
+#pragma unroll
+            for (int k = 0; k < CH; ++k) cov[k] = ldcg2(r.chi + x + T * k);
+        }
+        const float2 c_old = cov[m % CH];
         const float2 c_new = fma2(ntau2, d[m], fma2(ntau_v, v[m], c_old));
         const float2 dc = sub2(c_new, c_old);
         dn = fma2(dc, dc, dn);

@@ -10,6 +10,9 @@
 // group of T threads is one contiguous 8T-byte segment.  chibar and q are double-buffered by iteration parity, so
 // that a row group can redo the q-update of the row ABOVE its own (it needs (M qy_{n+1})[y-1] for the divergence)
 // from read-only data: no exchange between rows, no CTA-wide barrier; the duplicate loads hit L1/L2.
+// chi and p^ are double-buffered too: then every load inside the update loops is from data that is read-only for
+// the launch (ld.global.nc), which the scheduler may hoist above the stores of earlier elements -- with in-place
+// updates every element would expose one full memory latency (load -> use -> store -> next load).
 //
 // HBM bytes per pixel PAIR and iteration: fd_cols Z r8 w8, phi^ r8, p^ r8 w8 = 40 ; fd_rows Z r8 w8, chi r8 w8,
 // chibar r8 w8, qx r8 w8, qy r8 w8, M r8 = 88  ->  64 B per pixel of one slice and iteration.
@@ -29,8 +32,8 @@ struct StreamFdArgs {
     const float *field, *mask;
     long long mask_bstride;
     float *chi_out;
-    float2 *Z, *phat, *phihat, *chi2, *M2;   // [npairs][ny][nx]
-    float2 *cb2[2], *qx2[2], *qy2[2];        // double-buffered by iteration parity
+    float2 *Z, *phihat, *M2;                 // [npairs][ny][nx]
+    float2 *phat[2], *chi2[2], *cb2[2], *qx2[2], *qy2[2];   // double-buffered by iteration parity: iteration n reads [n&1]
     const float *Dtab;                       // D/(nx*ny), [ny][nx]
     const float2 *tw_row, *tw_col;
     int *stop_iter;                          // slice b is active in iteration n (0-based) iff n < stop_iter[b]
@@ -110,7 +113,7 @@ sfd_init_rows_kernel(const StreamFdArgs a) {
         acc0 = fmaf(va, va, acc0);
         acc1 = fmaf(vb, vb, acc1);
         a.M2[po + x] = make_float2(ma ? ma[x] : 1.f, has_b ? (mb ? mb[x] : 1.f) : 0.f);
-        a.chi2[po + x] = zero; a.cb2[0][po + x] = zero; a.qx2[0][po + x] = zero; a.qy2[0][po + x] = zero;
+        a.chi2[0][po + x] = zero; a.cb2[0][po + x] = zero; a.qx2[0][po + x] = zero; a.qy2[0][po + x] = zero;
     }
     fft_line<NX, Cfg::LD>(v, sm + g * Cfg::SM_PER_GROUP, j, tw, WarpSync());
 #pragma unroll
@@ -151,7 +154,7 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         a.phihat[po + (long long)(j + T * m) * a.nx] = v[m];
-        a.phat[po + (long long)(j + T * m) * a.nx] = zero;
+        a.phat[0][po + (long long)(j + T * m) * a.nx] = zero;
     }
     if (blockIdx.x == 0 && threadIdx.x < 2) {
         const int b = threadIdx.x ? s1 : s0;
@@ -223,8 +226,8 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
     float2 *smg = smc + c * Cfg::CS;
     const float2 *smg_mir = self_mirror ? smg : smc + (c ^ 8) * Cfg::CS;
     const long long po = (long long)pair * nx * NY + kx;
-    float2 *zc = a.Z + po, *ph = a.phat + po;
-    const float2 *phh = a.phihat + po;
+    float2 *zc = a.Z + po, *phw = a.phat[(n & 1) ^ 1] + po;
+    const float2 *phh = a.phihat + po, *phr = a.phat[n & 1] + po;
     const float *dcol = a.Dtab + kx;
     TwiddlesSmem<NY> tw;
     tw.w = tws + j;
@@ -247,8 +250,8 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
     for (int m = 0; m < E; ++m) {
         const long long o = (long long)(j + T * m) * nx;
         const float d = __ldg(dcol + o);
-        const float2 phat = __ldcs(phh + o);
-        const float2 pold = __ldcs(ph + o);
+        const float2 phat = __ldg(phh + o);
+        const float2 pold = __ldg(phr + o);
         const float2 res = sub2(mul2(splat(d * NN), v[m]), phat);
         const float2 pn = mul2(fma2(sig2, res, pold), inv2);
         if (want_gap) {
@@ -256,7 +259,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
             S1 = fmaf(dp.x, dp.x, fmaf(dp.y, dp.y, S1));
             smg[j + T * m] = dp;
         }
-        __stcs(ph + o, pn);
+        __stcs(phw + o, pn);
         v[m] = make_float2(d * pn.x, -d * pn.y);
     }
     if (want_gap) {
@@ -343,7 +346,8 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
     const int rd = n & 1, wr = rd ^ 1;
     float2 *zr = a.Z + po;
     const float2 *cbr = a.cb2[rd] + po, *qxr = a.qx2[rd] + po, *qyr = a.qy2[rd] + po, *M = a.M2 + po;
-    float2 *cbw = a.cb2[wr] + po, *qxw = a.qx2[wr] + po, *qyw = a.qy2[wr] + po, *chi = a.chi2 + po;
+    float2 *cbw = a.cb2[wr] + po, *qxw = a.qx2[wr] + po, *qyw = a.qy2[wr] + po, *chiw = a.chi2[wr] + po;
+    const float2 *chir = a.chi2[rd] + po;
     const bool has_up = y > 0, has_down = y < ny - 1;
 
     float2 v[E];
@@ -375,8 +379,8 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
         // own row: q_{n+1}[y][x]
         const float2 gx = mul2(mm, sub2(cr, c0));
         const float2 gy = mul2(mm, sub2(cd, c0));
-        float2 tx = fma2(sig2, gx, __ldcs(qxr + x));
-        float2 ty = fma2(sig2, gy, __ldcs(qyr + x));
+        float2 tx = fma2(sig2, gx, __ldg(qxr + x));
+        float2 ty = fma2(sig2, gy, __ldg(qyr + x));
         sfd_project(tx, ty, alpha, alpha_sq, aniso);
         __stcs(qxw + x, tx);
         __stcs(qyw + x, ty);
@@ -407,14 +411,14 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
         const float2 d = add2(sub2(left, mqx), sub2(mqy_up, mul2(mm, ty)));
         mqx_prev = mqx;
         // chi_{n+1}, chibar_{n+1}; a lane whose slice has stopped keeps its chi
-        const float2 c_old = __ldcs(chi + x);
+        const float2 c_old = __ldg(chir + x);
         const float2 step = fma2(ntau2, d, mul2(ntau_v, v[m]));
         const float2 c_new = fma2(actm, step, c_old);
         const float2 dc = sub2(c_new, c_old);
         dn = fma2(dc, dc, dn);
         cn = fma2(c_new, c_new, cn);
         const float2 cbar = fma2(theta2, dc, c_new);
-        __stcs(chi + x, c_new);
+        __stcs(chiw + x, c_new);
         cbw[x] = cbar;
         v[m] = cbar;
     }
@@ -451,7 +455,9 @@ sfd_finish_kernel(const StreamFdArgs a) {
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
     const bool has_b = s1 < a.batch;
     const long long P = (long long)a.nx * a.ny;
-    const float2 *c2 = a.chi2 + (long long)pair * P;
+    // the last row kernel that ran for this pair was iteration max(stop) - 1, which wrote buffer max(stop) & 1
+    const int st0 = a.stop_iter[s0], st1 = has_b ? a.stop_iter[s1] : 0;
+    const float2 *c2 = a.chi2[(st0 > st1 ? st0 : st1) & 1] + (long long)pair * P;
     float *oa = a.chi_out + (long long)s0 * P, *ob = a.chi_out + (long long)s1 * P;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P; i += (long long)gridDim.x * blockDim.x) {
         const float2 c = __ldcs(c2 + i);

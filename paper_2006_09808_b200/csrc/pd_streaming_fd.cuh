@@ -52,6 +52,11 @@ template <int N> struct SfdRowCfg {
     static constexpr int G = THREADS / T;
     static constexpr int LD = T + 1;
     static constexpr int SM_PER_GROUP = E * LD;
+#ifndef PD_SFD_STAGE_MIN
+#define PD_SFD_STAGE_MIN 256
+#endif
+    static constexpr bool STAGE = N >= PD_SFD_STAGE_MIN;   // park the spectrum in shared memory during the update loop
+    static constexpr int MINB = STAGE ? 4 : (N == 512 ? 3 : 4);
 };
 template <int N> struct SfdColCfg {
     static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
@@ -320,7 +325,7 @@ __device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float 
 //   d = G^T (M q_{n+1}) ; chi_{n+1} = chi_n - tau (v + d) ; chibar_{n+1} = chi_{n+1} + theta (chi_{n+1} - chi_n)
 //   Z <- row FFT of chibar_{n+1}
 template <int NX>
-__global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, NX == 512 ? 3 : 4)
+__global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, SfdRowCfg<NX>::MINB)
 sfd_rows_kernel(const StreamFdArgs a, const int n) {
     using Cfg = SfdRowCfg<NX>;
     constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
@@ -355,6 +360,14 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
     for (int m = 0; m < E; ++m) v[m] = __ldcs(zr + j + T * m);
     __syncthreads();   // twiddle table
     fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
+    // STAGE: park K p in the group's exchange region during the update loop, so that the registers hold loads in
+    // flight instead of the spectrum (each thread reads back only what it wrote)
+    constexpr bool STAGE = Cfg::STAGE;
+    if (STAGE) {
+        __syncwarp();   // the second FFT stage of the other threads has read the region
+#pragma unroll
+        for (int m = 0; m < E; ++m) smg[j + T * m] = v[m];
+    }
 
     const float2 sig2 = splat(a.sigma), zero = make_float2(0.f, 0.f);
     const float alpha = a.alpha, alpha_sq = a.alpha * a.alpha;
@@ -412,7 +425,7 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
         mqx_prev = mqx;
         // chi_{n+1}, chibar_{n+1}; a lane whose slice has stopped keeps its chi
         const float2 c_old = __ldg(chir + x);
-        const float2 step = fma2(ntau2, d, mul2(ntau_v, v[m]));
+        const float2 step = fma2(ntau2, d, mul2(ntau_v, STAGE ? smg[x] : v[m]));
         const float2 c_new = fma2(actm, step, c_old);
         const float2 dc = sub2(c_new, c_old);
         dn = fma2(dc, dc, dn);
@@ -420,9 +433,13 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
         const float2 cbar = fma2(theta2, dc, c_new);
         __stcs(chiw + x, c_new);
         cbw[x] = cbar;
-        v[m] = cbar;
+        if (STAGE) smg[x] = cbar; else v[m] = cbar;
     }
     if (!last) {   // the stop decision of this iteration is taken by the next column kernel
+        if (STAGE) {
+#pragma unroll
+            for (int m = 0; m < E; ++m) v[m] = smg[j + T * m];
+        }
         fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
 #pragma unroll
         for (int m = 0; m < E; ++m) __stcs(zr + j + T * m, v[m]);

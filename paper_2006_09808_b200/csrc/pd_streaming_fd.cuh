@@ -56,7 +56,7 @@ template <int N> struct SfdRowCfg {
 #define PD_SFD_STAGE_MIN 256
 #endif
     static constexpr bool STAGE = N >= PD_SFD_STAGE_MIN;   // park the spectrum in shared memory during the update loop
-    static constexpr int MINB = STAGE ? 4 : (N == 512 ? 3 : 4);
+    static constexpr int MINB = STAGE ? 5 : (N == 512 ? 3 : 4);
 };
 template <int N> struct SfdColCfg {
     static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
@@ -64,6 +64,10 @@ template <int N> struct SfdColCfg {
     static constexpr int THREADS = COLS * T;
     static constexpr int CS = N + 1;
     static constexpr int SMEM_BYTES = (COLS * CS + E * T) * (int)sizeof(float2) + 128;
+#ifndef PD_SFD_COL_STAGE_MIN
+#define PD_SFD_COL_STAGE_MIN 256
+#endif
+    static constexpr bool STAGE = N >= PD_SFD_COL_STAGE_MIN;   // park the spectrum in shared memory during the p^ update
 };
 
 // column kx of (column block cb, half h, slot cc): [8cb, 8cb+8) and its mirror images nx - kx; the self-mirrored
@@ -250,31 +254,72 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
     const float2 sig2 = splat(a.sigma), inv2 = splat(a.inv_one_plus_sigma);
     const float NN = (float)nx * (float)NY;
     float S1 = 0.f, S2 = 0.f;
-    if (want_gap) __syncthreads();   // the exchange region is free (readers of the FFT above are done)
+    if (Cfg::STAGE) {
+        // Park X^ in the column's exchange region (slot ky), so that the registers hold the loads of the update in
+        // flight instead of the spectrum; each slot then receives p^_{n+1}, from which both the Parseval sums and
+        // the next transform's input are taken.
+        __syncthreads();   // every thread's second FFT stage has read the region
 #pragma unroll
-    for (int m = 0; m < E; ++m) {
-        const long long o = (long long)(j + T * m) * nx;
-        const float d = __ldg(dcol + o);
-        const float2 phat = __ldg(phh + o);
-        const float2 pold = __ldg(phr + o);
-        const float2 res = sub2(mul2(splat(d * NN), v[m]), phat);
-        const float2 pn = mul2(fma2(sig2, res, pold), inv2);
-        if (want_gap) {
-            const float2 dp = sub2(pn, pold);
-            S1 = fmaf(dp.x, dp.x, fmaf(dp.y, dp.y, S1));
-            smg[j + T * m] = dp;
-        }
-        __stcs(phw + o, pn);
-        v[m] = make_float2(d * pn.x, -d * pn.y);
-    }
-    if (want_gap) {
-        __syncthreads();
+        for (int m = 0; m < E; ++m) smg[j + T * m] = v[m];
 #pragma unroll
         for (int m = 0; m < E; ++m) {
-            const int ky = j + T * m;
-            const float2 dp = smg[ky];
-            const float2 dm = smg_mir[(NY - ky) & (NY - 1)];
-            S2 = fmaf(dp.x, dm.x, fmaf(-dp.y, dm.y, S2));
+            const long long o = (long long)(j + T * m) * nx;
+            const float d = __ldg(dcol + o);
+            const float2 phat = __ldg(phh + o);
+            const float2 pold = __ldg(phr + o);
+            const float2 res = sub2(mul2(splat(d * NN), smg[j + T * m]), phat);
+            const float2 pn = mul2(fma2(sig2, res, pold), inv2);
+            if (want_gap) {
+                const float2 dp = sub2(pn, pold);
+                S1 = fmaf(dp.x, dp.x, fmaf(dp.y, dp.y, S1));
+            }
+            __stcs(phw + o, pn);
+            smg[j + T * m] = pn;
+        }
+        if (want_gap) {   // dp(k) dp(-k): p^_{n+1} of the mirror element from its slot, p^_n of both reloaded (L1/L2)
+            __syncthreads();
+            const float2 *phr_mir = a.phat[n & 1] + (long long)pair * nx * NY + (self_mirror ? kx : sfd_column_of(nx, blockIdx.x, h ^ 1, cc));
+#pragma unroll
+            for (int m = 0; m < E; ++m) {
+                const int ky = j + T * m, kym = (NY - ky) & (NY - 1);
+                const float2 dp = sub2(smg[ky], __ldg(phr + (long long)ky * nx));
+                const float2 dm = sub2(smg_mir[kym], __ldg(phr_mir + (long long)kym * nx));
+                S2 = fmaf(dp.x, dm.x, fmaf(-dp.y, dm.y, S2));
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const float d = __ldg(dcol + (long long)(j + T * m) * nx);
+            const float2 pn = smg[j + T * m];
+            v[m] = make_float2(d * pn.x, -d * pn.y);
+        }
+    } else {
+        if (want_gap) __syncthreads();   // the exchange region is free (readers of the FFT above are done)
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const long long o = (long long)(j + T * m) * nx;
+            const float d = __ldg(dcol + o);
+            const float2 phat = __ldg(phh + o);
+            const float2 pold = __ldg(phr + o);
+            const float2 res = sub2(mul2(splat(d * NN), v[m]), phat);
+            const float2 pn = mul2(fma2(sig2, res, pold), inv2);
+            if (want_gap) {
+                const float2 dp = sub2(pn, pold);
+                S1 = fmaf(dp.x, dp.x, fmaf(dp.y, dp.y, S1));
+                smg[j + T * m] = dp;
+            }
+            __stcs(phw + o, pn);
+            v[m] = make_float2(d * pn.x, -d * pn.y);
+        }
+        if (want_gap) {
+            __syncthreads();
+#pragma unroll
+            for (int m = 0; m < E; ++m) {
+                const int ky = j + T * m;
+                const float2 dp = smg[ky];
+                const float2 dm = smg_mir[(NY - ky) & (NY - 1)];
+                S2 = fmaf(dp.x, dm.x, fmaf(-dp.y, dm.y, S2));
+            }
         }
     }
     fft_line<NY, T>(v, smg, j, tw, BlockSync());

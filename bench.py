@@ -12,6 +12,7 @@ Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the meaning of e
 """
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -50,6 +51,14 @@ def load_peaks():
             pk = json.load(f)
         return float(pk["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_sm_mhz():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f).get("sm_max_mhz", 1965.0))
+    return 1965.0
 
 
 class ClockSampler:
@@ -177,6 +186,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the north-star single-coil stack timing")
+    ap.add_argument("--hybrid-tail", type=int, default=-1,
+                    help="PD_OPT_HYBRID_TAIL: slice pairs run by the streaming kernels beside the resident clusters "
+                         "(-1 automatic, 0 off)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -210,7 +222,9 @@ def main():
     plan = binding.Plan(cfg.nx, cfg.ny, batch, b0, cfg.lam, cfg.sigma, cfg.tau, cfg.theta)
     if args.variant != "auto":
         plan.set_option(binding.OPT_VARIANT, {"streaming": binding.VARIANT_STREAMING, "resident": binding.VARIANT_RESIDENT}[args.variant])
+    plan.set_option(binding.OPT_HYBRID_TAIL, args.hybrid_tail)
     plan_info = plan.info()
+    plan_info["hybrid_tail_pairs"] = plan.hybrid_tail()
     small = batch * P * 32 <= 2 * 126e6
     flush = torch.empty(64 * 1024 * 1024, device="cuda") if small else None
 
@@ -294,6 +308,15 @@ def main():
                      "achieved": path_bytes * args.steps / (ms * 1e-3) / 1e9 if world == 1 else path_bytes / (ms / args.steps * 1e-3) / 1e9,
                      "peak": peak}
     roofline_path["frac"] = roofline_path["achieved"] / peak
+    # FP32 view of the same step: algorithmic flops P (10 log2 P + 32) per slice-iteration against
+    # 148 SMs x 128 lanes x 2 flop x SM clock
+    sm_mhz = load_sm_mhz()
+    alu_peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12
+    flops = P * (10.0 * math.log2(P) + 32.0) * float(its_local.sum())
+    alu_ach = flops * (args.steps if world == 1 else 1) / ((ms if world == 1 else ms / args.steps) * 1e-3) / 1e12
+    roofline_alu = {"bound": "alu", "what": "whole path, algorithmic flops P(10 log2 P + 32) per slice-iteration",
+                    "unit": "TFLOP/s", "achieved": alu_ach, "peak": alu_peak, "frac": alu_ach / alu_peak,
+                    "peak_source": "148 SMs x 128 FP32 lanes x 2 x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz, else 1965)" % sm_mhz}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), H2D and D2H inside the timed region
     e2e = None
@@ -316,6 +339,7 @@ def main():
         plan2 = binding.Plan(ns.nx, ns.ny, ns.batch, b0, ns.lam, ns.sigma, ns.tau, ns.theta)
         if args.variant != "auto":
             plan2.set_option(binding.OPT_VARIANT, {"streaming": binding.VARIANT_STREAMING, "resident": binding.VARIANT_RESIDENT}[args.variant])
+        plan2.set_option(binding.OPT_HYBRID_TAIL, args.hybrid_tail)
         for _ in range(3):
             plan2.solve(f2, m2, c2, ns.iters, 0.0)
         torch.cuda.synchronize()
@@ -332,7 +356,8 @@ def main():
         t_ns = float(np.median(times))
         extra = {"workload": "NS: 128 slices x 256x256, 1 field map per slice, 200 iterations (BASELINE.json north_star target)",
                  "stack_recon_ms": t_ns, "slice_iterations_per_s": ns.batch * ns.iters / (t_ns * 1e-3),
-                 "hbm_floor_frac": PATH_FLOOR_BYTES_PER_PX * ns.nx * ns.ny * ns.batch * ns.iters / (t_ns * 1e-3) / 1e9 / peak}
+                 "hbm_floor_frac": PATH_FLOOR_BYTES_PER_PX * ns.nx * ns.ny * ns.batch * ns.iters / (t_ns * 1e-3) / 1e9 / peak,
+                 "hybrid_tail_pairs": plan2.hybrid_tail()}
         plan2.destroy()
 
     if rank == 0:
@@ -349,7 +374,7 @@ def main():
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic", "config": dict(workload_config(cfg, args.workload, batch, world), **plan_info),
             "stack_recon_ms": ms / args.steps, "slice_iterations_per_step": slice_its,
-            "roofline": roofline, "roofline_path": roofline_path, "cpu_baseline": cpu, "e2e": e2e,
+            "roofline": roofline, "roofline_path": roofline_path, "roofline_alu": roofline_alu, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches, "clocks": clocks, "north_star_stack": extra,
             "paper_context": "paper reports 4-15x GPU over CPU on unnamed hardware (PAPER.md:118); not comparable",
         }

@@ -51,9 +51,14 @@ enum pd_option {
     PD_OPT_UNSAFE_STEPS = 5, /* 1: skip the PD_ESTEP check at the next pd_set_steps call (not at pd_plan) */
     PD_OPT_KERNEL_TIMING = 6,/* 1: bracket every kernel launch of pd_solve with CUDA events on the caller's stream
                                 (read with pd_get_kernel_times); default 0 */
-    PD_OPT_FOURIER_DUAL = 7  /* 1 (default): when W is the identity keep the dual variable p in the Fourier domain
+    PD_OPT_FOURIER_DUAL = 7, /* 1 (default): when W is the identity keep the dual variable p in the Fourier domain
                                 (one FFT round trip per iteration; same iterates up to rounding);
                                 0: always apply K twice per iteration, literally as PAPER.md:49 */
+    PD_OPT_HYBRID_TAIL = 8   /* 256x256, W = identity, PD_VARIANT_AUTO only: slice pairs (from the END of the batch) that
+                                run through the streaming kernels on a plan-owned second stream, concurrently with the
+                                resident clusters, on the SMs those leave free (slices are independent).
+                                -1 (default): chosen from the batch size ; 0: off ; n > 0: exactly n pairs.
+                                pd_solve still returns with all work ordered on the caller's stream. */
 };
 /* kernel classes for pd_get_kernel_times.  Streaming variant: init, finish and, per iteration, fd_cols + fd_rows
  * (W = identity, Fourier-domain dual: two launches) or dual_rows + dipole_cols + primal_rows + dipole_cols (W set, or
@@ -127,6 +132,10 @@ int pd_last_launch_count(pd_plan_t p);
  * launched with (the paper's "N slices at a time", here slice PAIRS in flight; 0 for streaming);
  * *cluster_size = CTAs per cluster (0 for streaming). */
 int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size);
+
+/* Slice pairs the next pd_solve hands to the streaming kernels under the hybrid schedule (PD_OPT_HYBRID_TAIL);
+ * 0 when the schedule does not apply.  HOST pointer. */
+int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs);
 
 int pd_destroy(pd_plan_t p);
 

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libpd_b200.so")
 
 B0_X, B0_Y = 0, 1
 OK, EINVAL, ESIZE, ESTEP, ENOMEM, ECUDA, EVARIANT = 0, -1, -2, -3, -4, -5, -6
-OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING, OPT_FOURIER_DUAL = range(8)
+OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING, OPT_FOURIER_DUAL, OPT_HYBRID_TAIL = range(9)
 KERNEL_CLASSES = ["init", "dual_rows", "dipole_cols", "primal_rows", "finish", "resident", "fd_cols", "fd_rows"]
 TV_ISO, TV_ANISO = 0, 1
 LAMBDA_REG, LAMBDA_DATA = 0, 1
@@ -23,7 +23,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -54,6 +54,7 @@ def lib():
         L.pd_get_kernel_times.argtypes = [vp, vp, vp]
         L.pd_last_launch_count.argtypes = [vp]
         L.pd_get_info.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
+        L.pd_get_hybrid_tail.argtypes = [vp, C.POINTER(ip)]
         L.pd_destroy.argtypes = [vp]
         L.pd_strerror.argtypes = [ip]
         L.pd_strerror.restype = C.c_char_p
@@ -170,6 +171,12 @@ class Plan:
         _check(lib().pd_get_info(self._h, C.byref(v), C.byref(n), C.byref(c)))
         return {"variant": "resident" if v.value == VARIANT_RESIDENT else "streaming", "clusters": n.value,
                 "cluster_size": c.value}
+
+    def hybrid_tail(self):
+        """pd_get_hybrid_tail: slice pairs the next solve runs through the streaming kernels beside the resident clusters."""
+        n = C.c_int()
+        _check(lib().pd_get_hybrid_tail(self._h, C.byref(n)))
+        return n.value
 
     @property
     def last_launch_count(self):

@@ -55,6 +55,8 @@ struct pd_plan_s {
     // resident variant (pd_resident.cuh): per-cluster scratch, 9 arrays of nx*ny float2 per cluster
     int res_ok;            // this size has a resident kernel
     int res_clusters;      // clusters launched (= scratch slots)
+    int res_max_clusters;  // what the occupancy query allows
+    int num_sms;
     int res_csize;         // CTAs per cluster
     float2 *res_scratch;   // [kResidentScratchArrays][res_clusters][nx*ny]
     float *rk_part;        // [res_clusters][res_csize][8]
@@ -64,6 +66,12 @@ struct pd_plan_s {
     float *sfd_parts;      // per-CTA partial sums
     int sfd_ncolparts, sfd_nrowparts;
     int legacy_ok;         // the four-launch streaming workspace (W != I) is allocated
+    size_t sfd_pairs_alloc; // slice pairs the Fourier-domain streaming workspace holds
+    // hybrid schedule (256x256, W = I, PD_VARIANT_AUTO): the resident clusters cover 120 of the 148 SMs; the last
+    // `tail` slice pairs run through the streaming kernels on a second stream, on the SMs the clusters leave free
+    int hybrid_tail;       // -1: automatic ; >= 0: slice pairs given to the streaming kernels
+    cudaStream_t aux;
+    cudaEvent_t ev_fork, ev_join;
     // host-buffer entry point staging
     float *h_field, *h_mask, *h_chi;
     int last_launches;
@@ -295,18 +303,21 @@ int ensure_legacy_workspace(pd_plan_s *p) {
 
 constexpr int kSfdPlanes = 13;   // Z, phi^, M, and p^, chi, chibar, qx, qy twice each
 
-int ensure_sfd_workspace(pd_plan_s *p) {
-    if (p->sfd_planes) return PD_OK;
-    const size_t PP = (size_t)p->nx * p->ny * (size_t)p->npairs;
+int ensure_sfd_workspace(pd_plan_s *p, size_t npairs) {
+    if (p->sfd_planes && p->sfd_pairs_alloc >= npairs) return PD_OK;
+    if (p->sfd_planes) { cudaFree(p->sfd_planes); p->sfd_planes = nullptr; }
+    if (p->sfd_parts) { cudaFree(p->sfd_parts); p->sfd_parts = nullptr; }
+    const size_t PP = (size_t)p->nx * p->ny * npairs;
     p->sfd_ncolparts = p->nx / 16;
     p->sfd_nrowparts = p->nparts;
     int rc;
     if ((rc = dev_alloc(&p->sfd_planes, PP * kSfdPlanes)) != PD_OK) return rc;
     // p0_part [2], gap_col x2 [2], gap_row [2], res_part [4] per (pair, part)
-    const size_t nparts = (size_t)p->npairs * (size_t)(8 * p->sfd_nrowparts + 4 * p->sfd_ncolparts);
+    const size_t nparts = npairs * (size_t)(8 * p->sfd_nrowparts + 4 * p->sfd_ncolparts);
     if ((rc = dev_alloc(&p->sfd_parts, nparts)) != PD_OK) return rc;
     cudaError_t e = cudaMemset(p->sfd_parts, 0, nparts * sizeof(float));
     if (e != cudaSuccess) return cuda_fail(e, "streaming partial sums init");
+    p->sfd_pairs_alloc = npairs;
     return PD_OK;
 }
 
@@ -337,12 +348,36 @@ cudaError_t sfd_set_col_smem() {
 
 int resident_csize(int n) { return n == 64 ? ResChoice<64>::C : n == 128 ? ResChoice<128>::C : ResChoice<256>::C; }
 
+int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                       cudaStream_t st, int first = 0, int *launches_out = nullptr);
+
+// Hybrid schedule: slice pairs handed to the streaming kernels.  The resident clusters finish
+// `ncl` pairs per wave; the streaming kernels on the SMs they leave free finish about kHybridRho * ncl in the same
+// time (measured at 256x256).  Choose the number of resident waves w that minimises max(w, tail / (rho ncl)).
+constexpr double kHybridRho = 0.14;
+int hybrid_tail_pairs(const pd_plan_s *p) {
+    if (p->nx != 256 || p->weight || p->no_fd || p->variant != PD_VARIANT_AUTO || !p->aux) return 0;
+    if (p->hybrid_tail >= 0) return p->hybrid_tail < p->npairs ? p->hybrid_tail : p->npairs - 1;
+    const int ncl = p->res_max_clusters;
+    if (ncl * 8 + 16 > p->num_sms) return 0;   // no SMs left over
+    int best_tail = 0;
+    double best_t = 1e30;
+    for (int w = (p->npairs + ncl - 1) / ncl; w >= 1; --w) {
+        const int tail = p->npairs > w * ncl ? p->npairs - w * ncl : 0;
+        const double ts = (double)tail / (kHybridRho * ncl), t = ts > w ? ts : (double)w;
+        if (t < best_t - 1e-9) { best_t = t; best_tail = tail; }
+    }
+    return best_tail;
+}
+
 int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
                    cudaStream_t st) {
     const size_t P = (size_t)p->nx * p->ny;
+    const int tail = hybrid_tail_pairs(p);
+    const int res_pairs = p->npairs - tail, res_batch = tail ? 2 * res_pairs : p->batch;
     ResidentArgs a;
     std::memset(&a, 0, sizeof(a));
-    a.batch = p->batch; a.npairs = p->npairs; a.max_iters = max_iters; a.check_every = p->check_every;
+    a.batch = res_batch; a.npairs = res_pairs; a.max_iters = max_iters; a.check_every = p->check_every;
     effective_params(p, &a.alpha, &a.sigma, &a.tau);
     a.theta = p->theta;
     a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
@@ -367,7 +402,12 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
         }
         PD_CUDA(cudaEventRecord((*p->ev)[0], st));
     }
+    if (tail) {   // fork: the streaming kernels of the tail run on the plan's second stream
+        PD_CUDA(cudaEventRecord(p->ev_fork, st));
+        PD_CUDA(cudaStreamWaitEvent(p->aux, p->ev_fork, 0));
+    }
     const bool w = p->weight != nullptr, aniso = p->tv_mode == PD_TV_ANISO;
+    const int nclusters = res_pairs < p->res_clusters ? res_pairs : p->res_clusters;
     cudaError_t e;
     if (!w && !p->no_fd) {
         // W = identity: the dual variable p stays in the Fourier domain (pd_resident_fd.cuh)
@@ -381,22 +421,32 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
         f.Dpriv = p->Dpriv; f.tw_tab = p->tw_row; f.part = p->rk_part;
         f.iters_done = p->iters_done; f.relgap = p->relgap; f.relres = p->relres;
         switch (p->nx) {
-            case 64: e = resident_fd_launch<64>(f, aniso, p->res_clusters, st); break;
-            case 128: e = resident_fd_launch<128>(f, aniso, p->res_clusters, st); break;
-            default: e = resident_fd_launch<256>(f, aniso, p->res_clusters, st); break;
+            case 64: e = resident_fd_launch<64>(f, aniso, nclusters, st); break;
+            case 128: e = resident_fd_launch<128>(f, aniso, nclusters, st); break;
+            default: e = resident_fd_launch<256>(f, aniso, nclusters, st); break;
         }
     } else
     switch (p->nx) {
-        case 64: e = resident_launch<64>(a, w, aniso, p->res_clusters, st); break;
-        case 128: e = resident_launch<128>(a, w, aniso, p->res_clusters, st); break;
-        default: e = resident_launch<256>(a, w, aniso, p->res_clusters, st); break;
+        case 64: e = resident_launch<64>(a, w, aniso, nclusters, st); break;
+        case 128: e = resident_launch<128>(a, w, aniso, nclusters, st); break;
+        default: e = resident_launch<256>(a, w, aniso, nclusters, st); break;
     }
     if (e != cudaSuccess) return cuda_fail(e, "resident kernel launch");
+    int tail_launches = 0;
+    if (tail) {   // the tail, then join
+        const int timing = p->timing;
+        p->timing = 0;   // the class-5 bracket below covers the whole hybrid step
+        const int rc = solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, p->aux, 2 * res_pairs, &tail_launches);
+        p->timing = timing;
+        if (rc != PD_OK) return rc;
+        PD_CUDA(cudaEventRecord(p->ev_join, p->aux));
+        PD_CUDA(cudaStreamWaitEvent(st, p->ev_join, 0));
+    }
     if (p->timing) {
         PD_CUDA(cudaEventRecord((*p->ev)[1], st));
         p->ev_class->push_back(PD_KERNEL_RESIDENT);
     }
-    p->last_launches = 1;
+    p->last_launches = 1 + tail_launches;
     return PD_OK;
 }
 
@@ -421,21 +471,25 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
     } while (0)
 
 // Streaming variant, W = identity: two launches per iteration (pd_streaming_fd.cuh)
+// Slices [first, batch) of the plan (first even); field, mask and chi_out are the caller's whole-batch pointers.
 int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
-                       cudaStream_t st) {
-    int rc = ensure_sfd_workspace(p);
+                       cudaStream_t st, int first, int *launches_out) {
+    const int nb = p->batch - first, np = (nb + 1) / 2;
+    int rc = ensure_sfd_workspace(p, (size_t)np);
     if (rc != PD_OK) return rc;
-    const size_t P = (size_t)p->nx * p->ny, PP = P * (size_t)p->npairs;
+    const size_t P = (size_t)p->nx * p->ny, PP = P * (size_t)np;
     StreamFdArgs a;
     std::memset(&a, 0, sizeof(a));
-    a.nx = p->nx; a.ny = p->ny; a.batch = p->batch; a.npairs = p->npairs;
+    a.nx = p->nx; a.ny = p->ny; a.batch = nb; a.npairs = np;
     a.max_iters = max_iters; a.check_every = p->check_every; a.aniso = p->tv_mode == PD_TV_ANISO;
     effective_params(p, &a.alpha, &a.sigma, &a.tau);
     a.theta = p->theta;
     a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
     a.tol = tol;
-    a.field = field; a.mask = mask; a.mask_bstride = p->mask_shared ? 0 : (long long)P;
-    a.chi_out = chi_out;
+    a.mask_bstride = p->mask_shared ? 0 : (long long)P;
+    a.field = field + (size_t)first * P;
+    a.mask = mask ? mask + (size_t)first * (size_t)a.mask_bstride : nullptr;
+    a.chi_out = chi_out + (size_t)first * P;
     float2 *b = p->sfd_planes;
     a.Z = b; a.phihat = b + PP; a.M2 = b + 2 * PP;
     for (int k = 0; k < 2; ++k) {
@@ -443,9 +497,10 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
         a.qx2[k] = b + (9 + k) * PP; a.qy2[k] = b + (11 + k) * PP;
     }
     a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
-    a.stop_iter = p->stop_iter; a.P0 = p->P0; a.relgap = p->relgap; a.relres = p->relres; a.iters_done = p->iters_done;
+    a.stop_iter = p->stop_iter + first; a.P0 = p->P0 + first; a.relgap = p->relgap + first;
+    a.relres = p->relres + first; a.iters_done = p->iters_done + first;
     a.ncolparts = p->sfd_ncolparts; a.nrowparts = p->sfd_nrowparts;
-    const size_t nr = (size_t)p->npairs * a.nrowparts, nc = (size_t)p->npairs * a.ncolparts;
+    const size_t nr = (size_t)np * a.nrowparts, nc = (size_t)np * a.ncolparts;
     float *q = p->sfd_parts;
     a.p0_part = q; q += 2 * nr;
     a.gap_row = q; q += 2 * nr;
@@ -454,7 +509,7 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     a.gap_col[1] = q;
 
     int launches = 0;
-    p->ev_class->clear();
+    if (!launches_out) p->ev_class->clear();
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->nx, sfd_launch_init_rows, a, st));
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->ny, sfd_launch_init_cols, a, st));
     for (int n = 0; n < max_iters; ++n) {
@@ -463,10 +518,10 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     }
     {
         const int gx = (int)((P + 256 * 8 - 1) / (256 * 8));
-        PD_LAUNCH(PD_KERNEL_FINISH, (pdk::sfd_finish_kernel<<<dim3(gx, p->npairs), 256, 0, st>>>(a)));
+        PD_LAUNCH(PD_KERNEL_FINISH, (pdk::sfd_finish_kernel<<<dim3(gx, np), 256, 0, st>>>(a)));
     }
     PD_CUDA(cudaGetLastError());
-    p->last_launches = launches;
+    if (launches_out) *launches_out = launches; else p->last_launches = launches;
     return PD_OK;
 }
 
@@ -491,8 +546,10 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     p->nx = nx; p->ny = ny; p->batch = batch; p->npairs = (batch + 1) / 2; p->b0_dir = B0_dir;
     p->lambda_user = lambda; p->sigma_user = sigma; p->tau_user = tau; p->theta = theta;
     p->check_every = 1;
+    p->hybrid_tail = -1;
     {
         cudaError_t e = cudaGetDevice(&p->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "cudaGetDevice"); }
     }
     const int rows_per_cta = (nx == 64 || nx == 128) ? 16 : 8;  // = RowCfg<nx>::G
@@ -541,6 +598,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (rc == PD_OK && maxc >= 1) {
             p->res_csize = resident_csize(nx);
             p->res_clusters = maxc < p->npairs ? maxc : p->npairs;
+            p->res_max_clusters = maxc;
             rc = dev_alloc(&p->res_scratch, (size_t)pdk::kResidentScratchArrays * p->res_clusters * P);
             if (rc == PD_OK) rc = dev_alloc(&p->rk_part, (size_t)p->res_clusters * p->res_csize * 8);
             if (rc != PD_OK) { pd_destroy(p); return rc; }
@@ -558,12 +616,20 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
             cudaError_t e = cudaMemset(p->rk_part, 0, (size_t)p->res_clusters * p->res_csize * 8 * sizeof(float));
             if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "resident scratch init"); }
             p->res_ok = 1;
+            if (nx == 256) {   // second stream of the hybrid schedule, and the workspace of its automatic tail
+                cudaError_t e3 = cudaStreamCreateWithFlags(&p->aux, cudaStreamNonBlocking);
+                if (e3 == cudaSuccess) e3 = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+                if (e3 == cudaSuccess) e3 = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+                if (e3 != cudaSuccess) { pd_destroy(p); return cuda_fail(e3, "hybrid stream"); }
+                const int tail = hybrid_tail_pairs(p);
+                if (tail > 0 && (rc = ensure_sfd_workspace(p, (size_t)tail)) != PD_OK) { pd_destroy(p); return rc; }
+            }
         } else {
             cudaGetLastError();  // no cluster launch possible on this device: the streaming variant remains
         }
     }
     if (!p->res_ok) {   // streaming is the only path of this plan: take its workspace now
-        rc = ensure_sfd_workspace(p);
+        rc = ensure_sfd_workspace(p, (size_t)p->npairs);
         if (rc != PD_OK) { pd_destroy(p); return rc; }
     }
     *out = p;
@@ -597,7 +663,7 @@ int pd_set_option(pd_plan_t p, int key, int value) {
             if (value != PD_VARIANT_AUTO && value != PD_VARIANT_STREAMING && value != PD_VARIANT_RESIDENT) return PD_EINVAL;
             if (value == PD_VARIANT_RESIDENT && !p->res_ok) return PD_EVARIANT;
             p->variant = value;
-            return value == PD_VARIANT_STREAMING ? ensure_sfd_workspace(p) : PD_OK;
+            return value == PD_VARIANT_STREAMING ? ensure_sfd_workspace(p, (size_t)p->npairs) : PD_OK;
         case PD_OPT_CHECK_EVERY:
             if (value < 1) return PD_EINVAL;
             p->check_every = value; return PD_OK;
@@ -613,6 +679,9 @@ int pd_set_option(pd_plan_t p, int key, int value) {
         case PD_OPT_KERNEL_TIMING:
             if (value != 0 && value != 1) return PD_EINVAL;
             p->timing = value; return PD_OK;
+        case PD_OPT_HYBRID_TAIL:
+            if (value < -1) return PD_EINVAL;
+            p->hybrid_tail = value; return PD_OK;
         default: return PD_EINVAL;
     }
 }
@@ -740,6 +809,12 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
     return PD_OK;
 }
 
+int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs) {
+    if (!p || !tail_pairs) return PD_EINVAL;
+    *tail_pairs = (p->res_ok && p->variant != PD_VARIANT_STREAMING) ? hybrid_tail_pairs(p) : 0;
+    return PD_OK;
+}
+
 int pd_destroy(pd_plan_t p) {
     if (!p) return PD_EINVAL;
     void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->chibar, p->p, p->qx, p->qy, p->Z, p->stop_iter, p->iters_done,
@@ -747,6 +822,9 @@ int pd_destroy(pd_plan_t p) {
                     p->sfd_planes, p->sfd_parts};
     for (void *q : ptrs)
         if (q) cudaFree(q);
+    if (p->aux) cudaStreamDestroy(p->aux);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->ev) for (cudaEvent_t e : *p->ev) cudaEventDestroy(e);
     delete p->ev;
     delete p->ev_class;

@@ -114,6 +114,25 @@ def test_streaming_fourier_domain_dual(torch, pd, oracle, ny, nx, iters):
     assert np.allclose(g["relgap"], lit["relgap"], rtol=1e-4)
 
 
+@pytest.mark.parametrize("tail", [1, 2, 4])
+def test_hybrid_schedule_tail_through_streaming(torch, pd, oracle, tail):
+    """256x256, W = I: the last `tail` slice pairs run through the streaming kernels on the plan's second stream while
+    the resident clusters take the rest (PD_OPT_HYBRID_TAIL).  Same gates; stats of both parts land in one array."""
+    case = synth.random_case(256, 256, 9, seed=900 + tail, with_mask=True)        # odd batch: ragged last pair
+    iters = 4
+    plan_opts = [(pd.OPT_HYBRID_TAIL, tail)]
+    g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, options=plan_opts)
+    assert g["launches"] == 1 + 2 * iters + 3
+    o = oracle.solve(case["field"], case["mask"], lambda_=0.2, sigma=0.25, tau=0.25, max_iters=iters)
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-4)
+    assert np.allclose(g["relres"], o["relres"][:, iters - 1], rtol=1e-3)
+    assert np.all(g["iters_done"] == iters)
+    off = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, options=[(pd.OPT_HYBRID_TAIL, 0)])
+    assert off["launches"] == 1
+    assert slice_rel(g["chi"], off["chi"]).max() < TOL_1IT
+
+
 @pytest.mark.parametrize("iters", [2, 3, 7])
 def test_few_iterations_exercise_q_and_divergence(torch, pd, oracle, iters, variant):
     case = synth.random_case(128, 64, 4, seed=77, with_mask=True, with_weight=True)

@@ -71,9 +71,13 @@ enum { PD_LAMBDA_REG = 0, PD_LAMBDA_DATA = 1 };
 enum { PD_VARIANT_AUTO = 0, PD_VARIANT_STREAMING = 1, PD_VARIANT_RESIDENT = 2 };
 
 /* pd_plan (host call; PAPER.md:44 step 1, "dipole kernel convolution operator D").
- * Builds the dipole table D for (nx, ny, B0_dir), the FFT twiddle tables (computed in double), and the
- * device workspace for `batch` slices: p, q (2 comps), chibar, one complex spectrum per slice pair, the
- * per-slice state variables.  sigma <= 0 or tau <= 0 selects the automatic steps
+ * Builds the dipole table D for (nx, ny, B0_dir), the FFT twiddle tables (computed in double), the per-slice
+ * state variables and the device workspace of the variant the plan will run: the per-cluster
+ * scratch of the resident kernel (square sizes <= 256), and/or the streaming planes (sizes without a resident
+ * kernel, or the tail of the hybrid schedule).  A streaming workspace that only a later option or weight makes
+ * necessary is allocated by pd_set_option(PD_OPT_VARIANT, ...) or by the first pd_solve that needs it (that one
+ * call then contains a cudaMalloc and a NULL-stream synchronisation).  A plan serves one pd_solve at a time.
+ * sigma <= 0 or tau <= 0 selects the automatic steps
  * sigma = tau = 1/sqrt(4/9 + 8) (upper bound on ||K_full||_2).  *out receives the plan.
  * Errors: PD_EINVAL, PD_ESIZE, PD_ESTEP, PD_ENOMEM, PD_ECUDA.  Uses the current CUDA device. */
 int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir,
@@ -89,10 +93,11 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir,
  *          checked iteration n+1 with relgap_{n+1} < tol (relative Fenchel-Young gap, R9), else at
  *          max_iters; stopped slices cost (almost) nothing afterwards.  A slice whose W*phi is identically zero
  *          returns chi = 0 (iters_done 0 when tol > 0).
- * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Everything is enqueued on it; the call does not
- *          synchronise and never copies to the host.  Buffers must stay alive until the stream
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Everything is enqueued on it, or -- hybrid schedule,
+ *          PD_OPT_HYBRID_TAIL -- on a plan-owned second stream that is forked from and joined back into it with
+ *          events; the call does not synchronise and never copies to the host.  Buffers must stay alive until the stream
  *          reaches the end of the enqueued work.  Inputs are never written.
- * Errors: PD_EINVAL, PD_ECUDA. */
+ * Errors: PD_EINVAL, PD_ENOMEM, PD_ECUDA. */
 int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
              int max_iters, float tol, void *cuda_stream);
 

@@ -301,7 +301,7 @@ int ensure_legacy_workspace(pd_plan_s *p) {
     return PD_OK;
 }
 
-constexpr int kSfdPlanes = 13;   // Z, phi^, M, and p^, chi, chibar, qx, qy twice each
+constexpr int kSfdPlanes = 12;   // Z, phi^, M; p^, qx, qy twice each; chi three times
 
 int ensure_sfd_workspace(pd_plan_s *p, size_t npairs) {
     if (p->sfd_planes && p->sfd_pairs_alloc >= npairs) return PD_OK;
@@ -315,7 +315,10 @@ int ensure_sfd_workspace(pd_plan_s *p, size_t npairs) {
     // p0_part [2], gap_col x2 [2], gap_row [2], res_part [4] per (pair, part)
     const size_t nparts = npairs * (size_t)(8 * p->sfd_nrowparts + 4 * p->sfd_ncolparts);
     if ((rc = dev_alloc(&p->sfd_parts, nparts)) != PD_OK) return rc;
+    // cudaMemset runs on the NULL stream and may return early; the solve may be on a non-blocking stream (the hybrid
+    // schedule's second stream always is), so the zeroing must have finished before anything is enqueued
     cudaError_t e = cudaMemset(p->sfd_parts, 0, nparts * sizeof(float));
+    if (e == cudaSuccess) e = cudaStreamSynchronize(nullptr);
     if (e != cudaSuccess) return cuda_fail(e, "streaming partial sums init");
     p->sfd_pairs_alloc = npairs;
     return PD_OK;
@@ -327,7 +330,8 @@ template <int NX> void sfd_launch_init_rows(const StreamFdArgs &a, cudaStream_t 
 }
 template <int NX> void sfd_launch_rows(const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid(a.ny / pdk::SfdRowCfg<NX>::G, a.npairs);
-    pdk::sfd_rows_kernel<NX><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+    if (a.mask) pdk::sfd_rows_kernel<NX, true><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+    else pdk::sfd_rows_kernel<NX, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
 }
 template <int NY> void sfd_launch_init_cols(const StreamFdArgs &a, cudaStream_t st) {
     dim3 grid(a.nx / 16, a.npairs);
@@ -492,10 +496,8 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     a.chi_out = chi_out + (size_t)first * P;
     float2 *b = p->sfd_planes;
     a.Z = b; a.phihat = b + PP; a.M2 = b + 2 * PP;
-    for (int k = 0; k < 2; ++k) {
-        a.phat[k] = b + (3 + k) * PP; a.chi2[k] = b + (5 + k) * PP; a.cb2[k] = b + (7 + k) * PP;
-        a.qx2[k] = b + (9 + k) * PP; a.qy2[k] = b + (11 + k) * PP;
-    }
+    for (int k = 0; k < 2; ++k) { a.phat[k] = b + (3 + k) * PP; a.qx2[k] = b + (5 + k) * PP; a.qy2[k] = b + (7 + k) * PP; }
+    for (int k = 0; k < 3; ++k) a.chi3[k] = b + (9 + k) * PP;
     a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
     a.stop_iter = p->stop_iter + first; a.P0 = p->P0 + first; a.relgap = p->relgap + first;
     a.relres = p->relres + first; a.iters_done = p->iters_done + first;
@@ -627,6 +629,10 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         } else {
             cudaGetLastError();  // no cluster launch possible on this device: the streaming variant remains
         }
+    }
+    {   // table uploads and memsets above ran on the NULL stream: finish them before a solve on any other stream
+        cudaError_t e = cudaStreamSynchronize(nullptr);
+        if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "plan synchronize"); }
     }
     if (!p->res_ok) {   // streaming is the only path of this plan: take its workspace now
         rc = ensure_sfd_workspace(p, (size_t)p->npairs);

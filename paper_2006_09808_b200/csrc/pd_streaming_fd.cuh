@@ -14,8 +14,13 @@
 // the launch (ld.global.nc), which the scheduler may hoist above the stores of earlier elements -- with in-place
 // updates every element would expose one full memory latency (load -> use -> store -> next load).
 //
-// HBM bytes per pixel PAIR and iteration: fd_cols Z r8 w8, phi^ r8, p^ r8 w8 = 40 ; fd_rows Z r8 w8, chi r8 w8,
-// chibar r8 w8, qx r8 w8, qy r8 w8, M r8 = 88  ->  64 B per pixel of one slice and iteration.
+// chibar is never stored: chibar_n = chi_n + theta (chi_n - chi_{n-1}) is recomputed (bit-identically) from the two
+// last iterates, which a third chi buffer keeps readable while chi_{n+1} is written.  Without a mask (M = 1) the
+// mask plane is neither built nor read.
+//
+// HBM bytes per pixel PAIR and iteration: fd_cols Z r8 w8, phi^ r8, p^ r8 w8 = 40 ; fd_rows Z r8 w8, chi_n r8,
+// chi_{n-1} r8, chi_{n+1} w8, qx r8 w8, qy r8 w8, M r8 = 80  ->  60 B per pixel of one slice and iteration, 56 without
+// a mask.
 //
 // Gap (R9): data term by Parseval over mirror-paired columns (as in pd_resident_fd.cuh), q term in fd_rows;
 // both as per-CTA partial sums.  Every CTA of fd_cols(n+1) reduces the partials of iteration n in the same fixed
@@ -33,7 +38,8 @@ struct StreamFdArgs {
     long long mask_bstride;
     float *chi_out;
     float2 *Z, *phihat, *M2;                 // [npairs][ny][nx]
-    float2 *phat[2], *chi2[2], *cb2[2], *qx2[2], *qy2[2];   // double-buffered by iteration parity: iteration n reads [n&1]
+    float2 *phat[2], *qx2[2], *qy2[2];       // double-buffered by iteration parity: iteration n reads [n&1]
+    float2 *chi3[3];                         // chi_n in [n%3], chi_{n-1} in [(n+2)%3], chi_{n+1} written to [(n+1)%3]
     const float *Dtab;                       // D/(nx*ny), [ny][nx]
     const float2 *tw_row, *tw_col;
     int *stop_iter;                          // slice b is active in iteration n (0-based) iff n < stop_iter[b]
@@ -121,8 +127,8 @@ sfd_init_rows_kernel(const StreamFdArgs a) {
         v[m] = make_float2(va, vb);
         acc0 = fmaf(va, va, acc0);
         acc1 = fmaf(vb, vb, acc1);
-        a.M2[po + x] = make_float2(ma ? ma[x] : 1.f, has_b ? (mb ? mb[x] : 1.f) : 0.f);
-        a.chi2[0][po + x] = zero; a.cb2[0][po + x] = zero; a.qx2[0][po + x] = zero; a.qy2[0][po + x] = zero;
+        if (ma) a.M2[po + x] = make_float2(ma[x], has_b ? mb[x] : 0.f);
+        a.chi3[0][po + x] = zero; a.chi3[2][po + x] = zero; a.qx2[0][po + x] = zero; a.qy2[0][po + x] = zero;
     }
     fft_line<NX, Cfg::LD>(v, sm + g * Cfg::SM_PER_GROUP, j, tw, WarpSync());
 #pragma unroll
@@ -369,7 +375,7 @@ __device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float 
 //   q_{n+1} = proj_alpha(q_n + sigma M G chibar_n) for row y (stored) and, redundantly, its qy for row y-1
 //   d = G^T (M q_{n+1}) ; chi_{n+1} = chi_n - tau (v + d) ; chibar_{n+1} = chi_{n+1} + theta (chi_{n+1} - chi_n)
 //   Z <- row FFT of chibar_{n+1}
-template <int NX>
+template <int NX, bool MASKED>
 __global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, SfdRowCfg<NX>::MINB)
 sfd_rows_kernel(const StreamFdArgs a, const int n) {
     using Cfg = SfdRowCfg<NX>;
@@ -395,9 +401,9 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
     const long long po = ((long long)pair * ny + y) * NX;
     const int rd = n & 1, wr = rd ^ 1;
     float2 *zr = a.Z + po;
-    const float2 *cbr = a.cb2[rd] + po, *qxr = a.qx2[rd] + po, *qyr = a.qy2[rd] + po, *M = a.M2 + po;
-    float2 *cbw = a.cb2[wr] + po, *qxw = a.qx2[wr] + po, *qyw = a.qy2[wr] + po, *chiw = a.chi2[wr] + po;
-    const float2 *chir = a.chi2[rd] + po;
+    const float2 *qxr = a.qx2[rd] + po, *qyr = a.qy2[rd] + po, *M = a.M2 + po;
+    float2 *qxw = a.qx2[wr] + po, *qyw = a.qy2[wr] + po, *chiw = a.chi3[(n + 1) % 3] + po;
+    const float2 *chn = a.chi3[n % 3] + po, *chp = a.chi3[(n + 2) % 3] + po;   // chi_n, chi_{n-1}
     const bool has_up = y > 0, has_down = y < ny - 1;
 
     float2 v[E];
@@ -420,23 +426,29 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
     const float2 ntau2 = splat(-a.tau), ntau_v = make_float2(-a.tau, a.tau), theta2 = splat(a.theta);
     const float2 actm = make_float2(act0 ? 1.f : 0.f, act1 ? 1.f : 0.f);
     float2 gap = zero, dn = zero, cn = zero, mqx_prev = zero;
-    float2 c0n = __ldg(cbr + j), cun = has_up ? __ldg(cbr - NX + j) : zero;
+    // chibar_n = chi_n + theta (chi_n - chi_{n-1}), the same operations that produced it in iteration n-1 (PAPER.md:49 line 4)
+    auto cbar_at = [&](const int off, float2 &chi_n) {
+        chi_n = __ldg(chn + off);
+        return fma2(theta2, sub2(chi_n, __ldg(chp + off)), chi_n);
+    };
+    float2 tmp, con;                                           // con: chi_n[y][x] of the next element
+    float2 c0n = cbar_at(j, con), cun = has_up ? cbar_at(j - NX, tmp) : zero;
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int x = j + T * m;
-        const float2 c0 = c0n, cu = cun;                       // chibar_n[y][x], chibar_n[y-1][x]
-        if (m + 1 < E) { c0n = __ldg(cbr + x + T); cun = has_up ? __ldg(cbr - NX + x + T) : zero; }
-        const float2 cd = has_down ? __ldg(cbr + NX + x) : c0; // Neumann: no row below -> gy = 0
+        const float2 c0 = c0n, cu = cun, c_old = con;          // chibar_n[y][x], chibar_n[y-1][x], chi_n[y][x]
+        if (m + 1 < E) { c0n = cbar_at(x + T, con); cun = has_up ? cbar_at(x + T - NX, tmp) : zero; }
+        const float2 cd = has_down ? cbar_at(x + NX, tmp) : c0; // Neumann: no row below -> gy = 0
         // right neighbours [.][x+1]: lane j+1 (same m), or lane 0's element m+1 when j == T-1
         const float2 give0 = (j == 0 && m + 1 < E) ? c0n : c0;
         const float2 giveu = (j == 0 && m + 1 < E) ? cun : cu;
         float2 cr = shfl2(give0, (j + 1) & (T - 1), T);
         float2 cur = shfl2(giveu, (j + 1) & (T - 1), T);
         if (m == E - 1 && j == T - 1) { cr = c0; cur = cu; }   // Neumann: no column to the right -> gx = 0
-        const float2 mm = __ldg(M + x);
+        const float2 mm = MASKED ? __ldg(M + x) : make_float2(1.f, 1.f);
         // own row: q_{n+1}[y][x]
-        const float2 gx = mul2(mm, sub2(cr, c0));
-        const float2 gy = mul2(mm, sub2(cd, c0));
+        const float2 gx = MASKED ? mul2(mm, sub2(cr, c0)) : sub2(cr, c0);
+        const float2 gy = MASKED ? mul2(mm, sub2(cd, c0)) : sub2(cd, c0);
         float2 tx = fma2(sig2, gx, __ldg(qxr + x));
         float2 ty = fma2(sig2, gy, __ldg(qyr + x));
         sfd_project(tx, ty, alpha, alpha_sq, aniso);
@@ -455,21 +467,20 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
         // row above, redundantly: (M qy_{n+1})[y-1][x]
         float2 mqy_up = zero;
         if (has_up) {
-            const float2 mu = __ldg(M - NX + x);
-            float2 ux = fma2(sig2, mul2(mu, sub2(cur, cu)), __ldg(qxr - NX + x));
-            float2 uy = fma2(sig2, mul2(mu, sub2(c0, cu)), __ldg(qyr - NX + x));
+            const float2 mu = MASKED ? __ldg(M - NX + x) : make_float2(1.f, 1.f);
+            float2 ux = fma2(sig2, MASKED ? mul2(mu, sub2(cur, cu)) : sub2(cur, cu), __ldg(qxr - NX + x));
+            float2 uy = fma2(sig2, MASKED ? mul2(mu, sub2(c0, cu)) : sub2(c0, cu), __ldg(qyr - NX + x));
             sfd_project(ux, uy, alpha, alpha_sq, aniso);
-            mqy_up = mul2(mu, uy);
+            mqy_up = MASKED ? mul2(mu, uy) : uy;
         }
         // d = G^T (M q) = -div(M q): qx is 0 in the last column and qy in the last row, so no predicate
-        const float2 mqx = mul2(mm, tx);
+        const float2 mqx = MASKED ? mul2(mm, tx) : tx;
         const float2 give = (j == T - 1 && m > 0) ? mqx_prev : mqx;
         float2 left = shfl2(give, (j + T - 1) & (T - 1), T);   // (M qx)[y][x-1]
         if (m == 0 && j == 0) left = zero;
-        const float2 d = add2(sub2(left, mqx), sub2(mqy_up, mul2(mm, ty)));
+        const float2 d = add2(sub2(left, mqx), sub2(mqy_up, MASKED ? mul2(mm, ty) : ty));
         mqx_prev = mqx;
         // chi_{n+1}, chibar_{n+1}; a lane whose slice has stopped keeps its chi
-        const float2 c_old = __ldg(chir + x);
         const float2 step = fma2(ntau2, d, mul2(ntau_v, STAGE ? smg[x] : v[m]));
         const float2 c_new = fma2(actm, step, c_old);
         const float2 dc = sub2(c_new, c_old);
@@ -477,7 +488,6 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
         cn = fma2(c_new, c_new, cn);
         const float2 cbar = fma2(theta2, dc, c_new);
         __stcs(chiw + x, c_new);
-        cbw[x] = cbar;
         if (STAGE) smg[x] = cbar; else v[m] = cbar;
     }
     if (!last) {   // the stop decision of this iteration is taken by the next column kernel
@@ -517,9 +527,9 @@ sfd_finish_kernel(const StreamFdArgs a) {
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
     const bool has_b = s1 < a.batch;
     const long long P = (long long)a.nx * a.ny;
-    // the last row kernel that ran for this pair was iteration max(stop) - 1, which wrote buffer max(stop) & 1
+    // the last row kernel that ran for this pair was iteration max(stop) - 1, which wrote buffer max(stop) % 3
     const int st0 = a.stop_iter[s0], st1 = has_b ? a.stop_iter[s1] : 0;
-    const float2 *c2 = a.chi2[(st0 > st1 ? st0 : st1) & 1] + (long long)pair * P;
+    const float2 *c2 = a.chi3[(st0 > st1 ? st0 : st1) % 3] + (long long)pair * P;
     float *oa = a.chi_out + (long long)s0 * P, *ob = a.chi_out + (long long)s1 * P;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P; i += (long long)gridDim.x * blockDim.x) {
         const float2 c = __ldcs(c2 + i);

@@ -133,6 +133,36 @@ def test_hybrid_schedule_tail_through_streaming(torch, pd, oracle, tail):
     assert slice_rel(g["chi"], off["chi"]).max() < TOL_1IT
 
 
+def test_hybrid_schedule_tolerance_stop(torch, pd, oracle):
+    """Per-slice stopping under the hybrid schedule: the resident clusters and the streaming tail each stop their own
+    slices on the device; both parts agree with the hybrid-off run and with the oracle's stop iteration (R16)."""
+    d = synth.generate(2, nslices=7)          # C2 phantoms, 256x256
+    tol = 2e-3
+    g = gpu_solve(torch, pd, d["field"], d["mask"], 120, lam=0.005, tol=tol, options=[(pd.OPT_HYBRID_TAIL, 2)])
+    off = gpu_solve(torch, pd, d["field"], d["mask"], 120, lam=0.005, tol=tol, options=[(pd.OPT_HYBRID_TAIL, 0)])
+    assert np.abs(g["iters_done"].astype(int) - off["iters_done"].astype(int)).max() <= 1
+    assert np.all(g["iters_done"] < 120) and np.all(g["iters_done"] > 0)
+    for b in (0, 3, 4, 6):                    # two from the resident part, two from the tail (slices 3..6)
+        ob = oracle.solve(d["field"][b], d["mask"][b], lambda_=0.005, sigma=0.25, tau=0.25,
+                          max_iters=int(g["iters_done"][b]), want_hist=True)
+        assert slice_rel(g["chi"][b:b + 1], ob["chi"]).max() < TOL_FULL
+        assert abs(g["relgap"][b] / ob["relgap"][0, -1] - 1) < 1e-3
+        assert g["relgap"][b] < tol
+
+
+@pytest.mark.parametrize("ny,nx", [(64, 128), (256, 256), (512, 512)])
+def test_streaming_without_mask(torch, pd, oracle, ny, nx):
+    """mask = NULL (M = 1): the streaming row kernel neither builds nor reads the mask plane; 3 iterations also pass
+    through all three chi buffers (chibar is recomputed from chi_n and chi_{n-1})."""
+    case = synth.random_case(nx, ny, 3, seed=5 * nx + ny, with_mask=False)
+    for iters in (1, 4):
+        g = gpu_solve(torch, pd, case["field"], None, iters, lam=0.2, variant="streaming")
+        o = oracle.solve(case["field"], None, lambda_=0.2, sigma=0.25, tau=0.25, max_iters=iters)
+        assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+        assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-4)
+        assert np.allclose(g["relres"], o["relres"][:, iters - 1], rtol=1e-3)
+
+
 @pytest.mark.parametrize("iters", [2, 3, 7])
 def test_few_iterations_exercise_q_and_divergence(torch, pd, oracle, iters, variant):
     case = synth.random_case(128, 64, 4, seed=77, with_mask=True, with_weight=True)
@@ -170,7 +200,9 @@ def _sampled_full_config(torch, pd, oracle, cid, sample, host=False, variant="au
     """Run the GPU on the FULL config (the launch configuration bench.py times); oracle on sampled batch entries."""
     d = synth.generate(cid)
     cfg = d["cfg"]
-    g = gpu_solve(torch, pd, d["field"], d["mask"], cfg.iters, lam=cfg.lam, tol=cfg.tol, host=host, variant=variant)
+    # as bench.py: a config whose mask is all ones passes mask = NULL (M = 1)
+    gmask = None if bool((d["mask"] == 1.0).all()) else d["mask"]
+    g = gpu_solve(torch, pd, d["field"], gmask, cfg.iters, lam=cfg.lam, tol=cfg.tol, host=host, variant=variant)
     assert np.all(np.isfinite(g["chi"]))
     # property that holds at any size: every iterate has zero mean (DESIGN.md pin P7)
     means = np.abs(g["chi"].reshape(cfg.batch, -1).astype(np.float64).mean(axis=1))

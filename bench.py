@@ -30,16 +30,24 @@ METRIC = "pd_slice_iterations_per_s"
 UNIT = "slice-iterations/s"
 WORKLOADS = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4, "NS": 5}
 
-# Algorithmic HBM bytes per pixel and launch of each kernel class of the streaming variant:
+# Algorithmic HBM bytes per pixel of a slice and launch of each kernel class of the streaming variant:
 # what the pass must read and write once, spectra counted at 4 B/px/slice (one float2 per pixel of a slice PAIR).
 KERNEL_BYTES_PER_PX = {
     "resident": 48.0,     # one launch = the whole path: the streaming floor per slice-ITERATION (x iterations below)
-    "dual_rows": 44.0,    # Z r4 + p rw8 + phi r4 + chibar r4 + qx rw8 + qy rw8 + M r4 + Z w4
+    # literal path (W set, or PD_OPT_FOURIER_DUAL = 0): cols + dual_rows + cols + fd_rows, 80 B/px/slice-iteration
+    "dual_rows": 24.0,    # Z r4 w4 + phi r4 + W r4 + p r4 w4
     "dipole_cols": 8.0,   # Z r4 + Z w4
-    "primal_rows": 32.0,  # Z r4 + chi rw8 + chibar w4 + qx r4 + qy r4 + M r4 + Z w4
     # W = identity, Fourier-domain dual (pd_streaming_fd.cuh): two launches per iteration, 64 B/px/slice-iteration
     "fd_cols": 20.0,      # Z r4 w4 + phi^ r4 + p^ r4 w4
     "fd_rows": 40.0,      # Z r4 w4 + chi_n r4 + chi_{n-1} r4 + chi_{n+1} w4 + qx r4 w4 + qy r4 w4 + M r4 (36 without a mask)
+}
+# DRAM bytes per pixel of a slice per launch measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one
+# `--set full` capture over the whole batch, profiles/r01/ncu_sfd_*): (kernel, line length, masked) -> B/px
+NCU_DRAM_BYTES_PER_PX = {
+    ("fd_rows", 512, False): 35.2,   # ncu_sfd_rows_c4_v2.txt: 1.342 + 1.020 GB over 256 slices of 512x512
+    ("fd_cols", 512, False): 21.2,   # ncu_sfd_cols_c4_v2.txt: 0.865 + 0.559 GB
+    ("fd_rows", 256, True): 39.3,    # ncu_sfd_rows_c3.txt: 1.611 + 1.028 GB over 1024 slices of 256x256
+    ("fd_cols", 256, True): 19.7,    # ncu_sfd_cols_c3.txt: 0.827 + 0.492 GB
 }
 PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
 
@@ -310,9 +318,14 @@ def main():
     if dom == "resident":   # a single launch runs every iteration of every slice
         bytes_per_launch = KERNEL_BYTES_PER_PX[dom] * P * float(its_local.sum())
     achieved = bytes_per_launch / (dom_ms / dom_n * 1e-3) / 1e9
+    ncu_px = NCU_DRAM_BYTES_PER_PX.get((dom, cfg.nx if dom == "fd_rows" else cfg.ny, not mask_is_one))
+    traffic = ncu_px * P * avg_active_slices if ncu_px is not None else None
+    if dom == "resident" and cfg.nx == 256 and plan_info.get("hybrid_tail_pairs", 0) == 0 and not args.weighted:
+        # ncu_resident_fd_c2_v3.txt: 34.2 + 25.6 MB for 64 slices of 256x256, whole solve (load + store only)
+        traffic = 14.26 * P * batch
     ksum = sum(v[0] for v in ktot.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
+                "traffic": traffic, "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
                 "avg_launch_us": 1e3 * dom_ms / dom_n, "share_of_step": dom_ms / ksum,
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in ktot.items()},
                 "step_ms_with_events": ms_evt / args.steps}

@@ -61,8 +61,9 @@ enum pd_option {
                                 pd_solve still returns with all work ordered on the caller's stream. */
 };
 /* kernel classes for pd_get_kernel_times.  Streaming variant: init, finish and, per iteration, fd_cols + fd_rows
- * (W = identity, Fourier-domain dual: two launches) or dual_rows + dipole_cols + primal_rows + dipole_cols (W set, or
- * PD_OPT_FOURIER_DUAL = 0: four launches).  Resident variant: one launch, class 5. */
+ * (W = identity, Fourier-domain dual: two launches) or dipole_cols + dual_rows + dipole_cols + fd_rows (W set, or
+ * PD_OPT_FOURIER_DUAL = 0: four launches; class 3 is no longer used).  Resident variant: class 5, one bracket around
+ * the whole step (with the hybrid schedule that includes the streaming tail on the second stream). */
 enum pd_kernel_class { PD_KERNEL_INIT = 0, PD_KERNEL_DUAL = 1, PD_KERNEL_COLS = 2, PD_KERNEL_PRIMAL = 3,
                        PD_KERNEL_FINISH = 4, PD_KERNEL_RESIDENT = 5, PD_KERNEL_FD_COLS = 6, PD_KERNEL_FD_ROWS = 7,
                        PD_NUM_KERNEL_CLASSES = 8 };

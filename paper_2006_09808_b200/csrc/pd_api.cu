@@ -1,8 +1,7 @@
 // pd_api.cu -- host side of the C ABI declared in include/pd.h: plan construction (dipole table, twiddle
 // tables, workspace), launch sequencing of the PD iteration on a caller-provided stream.
-// No CPU fallback exists: every arithmetic step of the path runs in the kernels of pd_streaming.cuh.
+// No CPU fallback exists: every arithmetic step of the path runs in the kernels of pd_resident*.cuh / pd_streaming_fd.cuh.
 #include "../../include/pd.h"
-#include "pd_streaming.cuh"
 #include "pd_resident.cuh"
 #include "pd_resident_fd.cuh"
 #include "pd_streaming_fd.cuh"
@@ -15,7 +14,6 @@
 
 using pdk::ResidentArgs;
 using pdk::ResidentFdArgs;
-using pdk::SolveArgs;
 using pdk::StreamFdArgs;
 
 namespace {
@@ -47,10 +45,8 @@ struct pd_plan_s {
     // device tables and workspace
     float *Dtab;
     float2 *tw_row, *tw_col;
-    float *chibar, *p, *qx, *qy;
-    float2 *Z;
     int *stop_iter, *iters_done;
-    float *P0, *relgap, *relres, *gap_part, *res_part;
+    float *P0, *relgap, *relres;
     int nparts;
     // resident variant (pd_resident.cuh): per-cluster scratch, 9 arrays of nx*ny float2 per cluster
     int res_ok;            // this size has a resident kernel
@@ -65,7 +61,6 @@ struct pd_plan_s {
     float2 *sfd_planes;    // 11 arrays of [npairs][ny][nx] float2
     float *sfd_parts;      // per-CTA partial sums
     int sfd_ncolparts, sfd_nrowparts;
-    int legacy_ok;         // the four-launch streaming workspace (W != I) is allocated
     size_t sfd_pairs_alloc; // slice pairs the Fourier-domain streaming workspace holds
     // hybrid schedule (256x256, W = I, PD_VARIANT_AUTO): the resident clusters cover 120 of the 148 SMs; the last
     // `tail` slice pairs run through the streaming kernels on a second stream, on the SMs the clusters leave free
@@ -142,22 +137,6 @@ void build_twiddles(std::vector<float2> &tw, int n) {
     }
 }
 
-template <int NX>
-void launch_dual(const SolveArgs &a, int n, cudaStream_t st) {
-    dim3 grid(a.ny / pdk::RowCfg<NX>::G, a.npairs);
-    pdk::dual_rows_kernel<NX><<<grid, pdk::RowCfg<NX>::THREADS, 0, st>>>(a, n);
-}
-template <int NX>
-void launch_primal(const SolveArgs &a, int n, cudaStream_t st) {
-    dim3 grid(a.ny / pdk::RowCfg<NX>::G, a.npairs);
-    pdk::primal_rows_kernel<NX><<<grid, pdk::RowCfg<NX>::THREADS, 0, st>>>(a, n);
-}
-template <int NY>
-void launch_cols(const SolveArgs &a, int n, int fin, cudaStream_t st) {
-    dim3 grid(a.nx / pdk::ColCfg<NY>::COLS, a.npairs);
-    pdk::dipole_cols_kernel<NY><<<grid, pdk::ColCfg<NY>::THREADS, pdk::ColCfg<NY>::SMEM_BYTES, st>>>(a, n, fin);
-}
-
 #define PD_DISPATCH(n, F, ...)                    \
     switch (n) {                                  \
         case 64: F<64>(__VA_ARGS__); break;       \
@@ -165,12 +144,6 @@ void launch_cols(const SolveArgs &a, int n, int fin, cudaStream_t st) {
         case 256: F<256>(__VA_ARGS__); break;     \
         default: F<512>(__VA_ARGS__); break;      \
     }
-
-template <int NY>
-cudaError_t set_col_smem() {
-    return cudaFuncSetAttribute(pdk::dipole_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                pdk::ColCfg<NY>::SMEM_BYTES);
-}
 
 // ---- resident variant: configuration per size, occupancy query, launch
 template <int N> struct ResChoice;
@@ -286,22 +259,10 @@ void build_dipole_private(std::vector<float> &out, const std::vector<float> &D) 
 }
 
 
-// ---- streaming workspaces: allocated when a streaming solve is first possible (plan time for sizes without a
-// resident kernel, pd_set_option(PD_OPT_VARIANT, PD_VARIANT_STREAMING) otherwise) so that resident plans stay small
-int ensure_legacy_workspace(pd_plan_s *p) {
-    if (p->legacy_ok) return PD_OK;
-    const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
-    int rc;
-    if ((rc = dev_alloc(&p->chibar, BP)) != PD_OK) return rc;
-    if ((rc = dev_alloc(&p->p, BP)) != PD_OK) return rc;
-    if ((rc = dev_alloc(&p->qx, BP)) != PD_OK) return rc;
-    if ((rc = dev_alloc(&p->qy, BP)) != PD_OK) return rc;
-    if (!p->Z && (rc = dev_alloc(&p->Z, P * (size_t)p->npairs)) != PD_OK) return rc;
-    p->legacy_ok = 1;
-    return PD_OK;
-}
-
-constexpr int kSfdPlanes = 12;   // Z, phi^, M; p^, qx, qy twice each; chi three times
+// ---- streaming workspace: allocated when a streaming solve is first possible (plan time for sizes without a
+// resident kernel or with a hybrid tail, pd_set_option(PD_OPT_VARIANT, PD_VARIANT_STREAMING) otherwise) so that
+// resident plans stay small
+constexpr int kSfdPlanes = 13;   // Z, phi^ (or phi), M, W; p^ (or p), qx, qy twice each; chi three times
 
 int ensure_sfd_workspace(pd_plan_s *p, size_t npairs) {
     if (p->sfd_planes && p->sfd_pairs_alloc >= npairs) return PD_OK;
@@ -312,8 +273,10 @@ int ensure_sfd_workspace(pd_plan_s *p, size_t npairs) {
     p->sfd_nrowparts = p->nparts;
     int rc;
     if ((rc = dev_alloc(&p->sfd_planes, PP * kSfdPlanes)) != PD_OK) return rc;
-    // p0_part [2], gap_col x2 [2], gap_row [2], res_part [4] per (pair, part)
-    const size_t nparts = npairs * (size_t)(8 * p->sfd_nrowparts + 4 * p->sfd_ncolparts);
+    // p0_part [2], gap_row [2], res_part [4] per (pair, row part); gap_col x2 [2] per (pair, column part) -- sized for
+    // the literal path too, whose data-term partials come from the dual row kernel (row parts)
+    const int ncp = p->sfd_ncolparts > p->sfd_nrowparts ? p->sfd_ncolparts : p->sfd_nrowparts;
+    const size_t nparts = npairs * (size_t)(8 * p->sfd_nrowparts + 4 * ncp);
     if ((rc = dev_alloc(&p->sfd_parts, nparts)) != PD_OK) return rc;
     // cudaMemset runs on the NULL stream and may return early; the solve may be on a non-blocking stream (the hybrid
     // schedule's second stream always is), so the zeroing must have finished before anything is enqueued
@@ -339,12 +302,23 @@ template <int NY> void sfd_launch_init_cols(const StreamFdArgs &a, cudaStream_t 
 }
 template <int NY> void sfd_launch_cols(const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid(a.nx / 16, a.npairs);
-    pdk::sfd_cols_kernel<NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n);
+    pdk::sfd_cols_kernel<NY, false><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, 1);
+}
+template <int NY> void sfd_launch_cols_plain(const StreamFdArgs &a, int n, int decide, cudaStream_t st) {
+    dim3 grid(a.nx / 16, a.npairs);
+    pdk::sfd_cols_kernel<NY, true><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
+}
+template <int NX> void sfd_launch_dual_rows(const StreamFdArgs &a, int n, cudaStream_t st) {
+    dim3 grid(a.ny / pdk::SfdRowCfg<NX>::G, a.npairs);
+    pdk::sfd_dual_rows_kernel<NX><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
 }
 template <int NY>
 cudaError_t sfd_set_col_smem() {
-    cudaError_t e = cudaFuncSetAttribute(pdk::sfd_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(pdk::sfd_cols_kernel<NY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          pdk::SfdColCfg<NY>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(pdk::sfd_cols_kernel<NY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             pdk::SfdColCfg<NY>::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(pdk::sfd_init_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 pdk::SfdColCfg<NY>::SMEM_BYTES);
@@ -358,7 +332,7 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
 // Hybrid schedule: slice pairs handed to the streaming kernels.  The resident clusters finish
 // `ncl` pairs per wave; the streaming kernels on the SMs they leave free finish about kHybridRho * ncl in the same
 // time (measured at 256x256).  Choose the number of resident waves w that minimises max(w, tail / (rho ncl)).
-constexpr double kHybridRho = 0.14;
+constexpr double kHybridRho = 0.19;
 int hybrid_tail_pairs(const pd_plan_s *p) {
     if (p->nx != 256 || p->weight || p->no_fd || p->variant != PD_VARIANT_AUTO || !p->aux) return 0;
     if (p->hybrid_tail >= 0) return p->hybrid_tail < p->npairs ? p->hybrid_tail : p->npairs - 1;
@@ -491,6 +465,9 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
     a.tol = tol;
     a.mask_bstride = p->mask_shared ? 0 : (long long)P;
+    const bool literal = p->weight != nullptr || p->no_fd;   // p in the image domain, K applied twice (PAPER.md:49 literally)
+    a.literal = literal ? 1 : 0;
+    a.weight = p->weight ? p->weight + (size_t)first * P : nullptr;
     a.field = field + (size_t)first * P;
     a.mask = mask ? mask + (size_t)first * (size_t)a.mask_bstride : nullptr;
     a.chi_out = chi_out + (size_t)first * P;
@@ -498,11 +475,13 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     a.Z = b; a.phihat = b + PP; a.M2 = b + 2 * PP;
     for (int k = 0; k < 2; ++k) { a.phat[k] = b + (3 + k) * PP; a.qx2[k] = b + (5 + k) * PP; a.qy2[k] = b + (7 + k) * PP; }
     for (int k = 0; k < 3; ++k) a.chi3[k] = b + (9 + k) * PP;
+    a.W2 = b + 12 * PP;
     a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
     a.stop_iter = p->stop_iter + first; a.P0 = p->P0 + first; a.relgap = p->relgap + first;
     a.relres = p->relres + first; a.iters_done = p->iters_done + first;
-    a.ncolparts = p->sfd_ncolparts; a.nrowparts = p->sfd_nrowparts;
-    const size_t nr = (size_t)np * a.nrowparts, nc = (size_t)np * a.ncolparts;
+    a.nrowparts = p->sfd_nrowparts;
+    a.ncolparts = literal ? p->sfd_nrowparts : p->sfd_ncolparts;   // who writes the data term of the gap
+    const size_t nr = (size_t)np * a.nrowparts, nc = (size_t)np * (size_t)(p->sfd_ncolparts > p->sfd_nrowparts ? p->sfd_ncolparts : p->sfd_nrowparts);
     float *q = p->sfd_parts;
     a.p0_part = q; q += 2 * nr;
     a.gap_row = q; q += 2 * nr;
@@ -515,7 +494,13 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->nx, sfd_launch_init_rows, a, st));
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->ny, sfd_launch_init_cols, a, st));
     for (int n = 0; n < max_iters; ++n) {
-        PD_LAUNCH(PD_KERNEL_FD_COLS, PD_DISPATCH(p->ny, sfd_launch_cols, a, n, st));
+        if (literal) {
+            if (n > 0) PD_LAUNCH(PD_KERNEL_COLS, PD_DISPATCH(p->ny, sfd_launch_cols_plain, a, n, 1, st));   // K1 (chibar_0 = 0)
+            PD_LAUNCH(PD_KERNEL_DUAL, PD_DISPATCH(p->nx, sfd_launch_dual_rows, a, n, st));
+            PD_LAUNCH(PD_KERNEL_COLS, PD_DISPATCH(p->ny, sfd_launch_cols_plain, a, n, 0, st));              // K2
+        } else {
+            PD_LAUNCH(PD_KERNEL_FD_COLS, PD_DISPATCH(p->ny, sfd_launch_cols, a, n, st));
+        }
         PD_LAUNCH(PD_KERNEL_FD_ROWS, PD_DISPATCH(p->nx, sfd_launch_rows, a, n, st));
     }
     {
@@ -554,7 +539,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
         if (e != cudaSuccess) { delete p; return cuda_fail(e, "cudaGetDevice"); }
     }
-    const int rows_per_cta = (nx == 64 || nx == 128) ? 16 : 8;  // = RowCfg<nx>::G
+    const int rows_per_cta = (nx == 64 || nx == 128) ? 16 : 8;  // = SfdRowCfg<nx>::G
     p->nparts = ny / rows_per_cta;
 
     const size_t P = (size_t)nx * ny;
@@ -567,8 +552,6 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     PD_TRY(dev_alloc(&p->P0, (size_t)batch));
     PD_TRY(dev_alloc(&p->relgap, (size_t)batch));
     PD_TRY(dev_alloc(&p->relres, (size_t)batch));
-    PD_TRY(dev_alloc(&p->gap_part, (size_t)batch * p->nparts));
-    PD_TRY(dev_alloc(&p->res_part, (size_t)batch * p->nparts * 2));
 #undef PD_TRY
     {
         std::vector<float> D(P);
@@ -582,10 +565,6 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (e == cudaSuccess) e = cudaMemset(p->iters_done, 0, batch * sizeof(int));
         if (e == cudaSuccess) e = cudaMemset(p->relgap, 0, batch * sizeof(float));
         if (e == cudaSuccess) e = cudaMemset(p->relres, 0, batch * sizeof(float));
-        if (e == cudaSuccess) e = set_col_smem<64>();
-        if (e == cudaSuccess) e = set_col_smem<128>();
-        if (e == cudaSuccess) e = set_col_smem<256>();
-        if (e == cudaSuccess) e = set_col_smem<512>();
         if (e == cudaSuccess) e = sfd_set_col_smem<64>();
         if (e == cudaSuccess) e = sfd_set_col_smem<128>();
         if (e == cudaSuccess) e = sfd_set_col_smem<256>();
@@ -697,53 +676,8 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
     if (!p || !field || !chi_out || max_iters < 0) return PD_EINVAL;
     if (p->lambda_conv == PD_LAMBDA_DATA && !(p->lambda_user > 0.f)) return PD_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
-
     if (p->res_ok && p->variant != PD_VARIANT_STREAMING) return solve_resident(p, field, mask, chi_out, max_iters, tol, st);
-    if (!p->weight && !p->no_fd) return solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, st);
-    {
-        const int rc = ensure_legacy_workspace(p);
-        if (rc != PD_OK) return rc;
-    }
-
-    SolveArgs a;
-    std::memset(&a, 0, sizeof(a));
-    a.nx = p->nx; a.ny = p->ny; a.batch = p->batch; a.npairs = p->npairs;
-    a.field = field; a.mask = mask; a.weight = p->weight;
-    a.mask_bstride = p->mask_shared ? 0 : (long long)P;
-    a.chi = chi_out; a.chibar = p->chibar; a.p = p->p; a.qx = p->qx; a.qy = p->qy; a.Z = p->Z;
-    a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
-    a.stop_iter = p->stop_iter; a.P0 = p->P0; a.relgap = p->relgap; a.relres = p->relres;
-    a.gap_part = p->gap_part; a.res_part = p->res_part; a.nparts = p->nparts;
-    effective_params(p, &a.alpha, &a.sigma, &a.tau);
-    a.theta = p->theta;
-    a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
-    a.tol = tol;
-    a.aniso = p->tv_mode == PD_TV_ANISO;
-    a.check_every = p->check_every;
-    a.max_iters = max_iters;
-
-    int launches = 0;
-    p->ev_class->clear();
-    // chi_0 = p_0 = q_0 = 0, chibar_0 = chi_0; the spectrum of chibar_0 is 0 as well
-    PD_CUDA(cudaMemsetAsync(chi_out, 0, BP * sizeof(float), st));
-    PD_CUDA(cudaMemsetAsync(p->chibar, 0, BP * sizeof(float), st));
-    PD_CUDA(cudaMemsetAsync(p->p, 0, BP * sizeof(float), st));
-    PD_CUDA(cudaMemsetAsync(p->qx, 0, BP * sizeof(float), st));
-    PD_CUDA(cudaMemsetAsync(p->qy, 0, BP * sizeof(float), st));
-    PD_CUDA(cudaMemsetAsync(p->Z, 0, P * (size_t)p->npairs * sizeof(float2), st));
-    PD_CUDA(cudaMemsetAsync(p->stop_iter, 0, ((size_t)p->batch + 1) * sizeof(int), st));
-    PD_LAUNCH(PD_KERNEL_INIT, (pdk::init_slices_kernel<<<p->batch, 256, 0, st>>>(a)));
-    for (int n = 0; n < max_iters; ++n) {
-        if (n > 0) PD_LAUNCH(PD_KERNEL_COLS, PD_DISPATCH(p->ny, launch_cols, a, n, 0, st));  // K1 column pass (chibar_0 = 0)
-        PD_LAUNCH(PD_KERNEL_DUAL, PD_DISPATCH(p->nx, launch_dual, a, n, st));
-        PD_LAUNCH(PD_KERNEL_COLS, PD_DISPATCH(p->ny, launch_cols, a, n, 1, st));             // K2 column pass + gap / stop flag
-        PD_LAUNCH(PD_KERNEL_PRIMAL, PD_DISPATCH(p->nx, launch_primal, a, n, st));
-    }
-    PD_LAUNCH(PD_KERNEL_FINISH, (pdk::finish_slices_kernel<<<(p->batch + 127) / 128, 128, 0, st>>>(a, p->iters_done)));
-    PD_CUDA(cudaGetLastError());
-    p->last_launches = launches;
-    return PD_OK;
+    return solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, st);
 }
 
 int pd_solve_host(pd_plan_t p, const float *field_host, const float *mask_host, float *chi_out_host, int max_iters,
@@ -823,8 +757,8 @@ int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs) {
 
 int pd_destroy(pd_plan_t p) {
     if (!p) return PD_EINVAL;
-    void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->chibar, p->p, p->qx, p->qy, p->Z, p->stop_iter, p->iters_done,
-                    p->P0, p->relgap, p->relres, p->gap_part, p->res_part, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part, p->Dpriv,
+    void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->stop_iter, p->iters_done,
+                    p->P0, p->relgap, p->relres, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part, p->Dpriv,
                     p->sfd_planes, p->sfd_parts};
     for (void *q : ptrs)
         if (q) cudaFree(q);

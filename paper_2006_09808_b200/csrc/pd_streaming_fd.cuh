@@ -1,4 +1,6 @@
-// pd_streaming_fd.cuh -- streaming variant with the dual variable p kept in the FOURIER domain (W = identity).
+// pd_streaming_fd.cuh -- the streaming variant: dual variable p kept in the FOURIER domain when W = identity (two
+// launches per iteration, described first); the literal iteration for W != I on the same planes (four launches,
+// sfd_dual_rows_kernel and sfd_cols_kernel<PLAIN> further down).
 //
 // Same algebra as pd_resident_fd.cuh (PAPER.md:49 line 1 commutes with the FFT when W = I):
 //     p^_{n+1} = (p^_n + sigma (D X^_n - phi^)) / (1 + sigma),   X^_n = F chibar_n,   K p_{n+1} = F^-1 (D p^_{n+1}),
@@ -34,10 +36,12 @@ namespace pdk {
 struct StreamFdArgs {
     int nx, ny, batch, npairs, max_iters, check_every, aniso;
     float alpha, sigma, tau, theta, inv_one_plus_sigma, tol;
-    const float *field, *mask;
+    const float *field, *mask, *weight;
     long long mask_bstride;
     float *chi_out;
     float2 *Z, *phihat, *M2;                 // [npairs][ny][nx]
+    float2 *W2;                              // literal path only: interleaved W; phihat then holds phi itself
+    int literal;                             // 1: W != I or PD_OPT_FOURIER_DUAL = 0 (p kept in the image domain)
     float2 *phat[2], *qx2[2], *qy2[2];       // double-buffered by iteration parity: iteration n reads [n&1]
     float2 *chi3[3];                         // chi_n in [n%3], chi_{n-1} in [(n+2)%3], chi_{n+1} written to [(n+1)%3]
     const float *Dtab;                       // D/(nx*ny), [ny][nx]
@@ -125,14 +129,23 @@ sfd_init_rows_kernel(const StreamFdArgs a) {
         const int x = j + T * m;
         const float va = fa[x], vb = has_b ? fb[x] : 0.f;
         v[m] = make_float2(va, vb);
-        acc0 = fmaf(va, va, acc0);
-        acc1 = fmaf(vb, vb, acc1);
+        float wa = 1.f, wb = 1.f;
+        if (a.literal) {   // phi and W interleaved, p_0 = 0; P0 = 1/2 ||W phi||^2
+            if (a.weight) { wa = a.weight[(long long)s0 * P + rowoff + x]; wb = has_b ? a.weight[(long long)s1 * P + rowoff + x] : 0.f; }
+            a.phihat[po + x] = v[m];
+            a.W2[po + x] = make_float2(wa, wb);
+            a.phat[0][po + x] = zero;
+        }
+        acc0 = fmaf(wa * va, wa * va, acc0);
+        acc1 = fmaf(wb * vb, wb * vb, acc1);
         if (ma) a.M2[po + x] = make_float2(ma[x], has_b ? mb[x] : 0.f);
         a.chi3[0][po + x] = zero; a.chi3[2][po + x] = zero; a.qx2[0][po + x] = zero; a.qy2[0][po + x] = zero;
     }
-    fft_line<NX, Cfg::LD>(v, sm + g * Cfg::SM_PER_GROUP, j, tw, WarpSync());
+    if (!a.literal) {   // phi^ needs the transform of the field; the literal path starts from chibar_0 = 0
+        fft_line<NX, Cfg::LD>(v, sm + g * Cfg::SM_PER_GROUP, j, tw, WarpSync());
 #pragma unroll
-    for (int m = 0; m < E; ++m) a.Z[po + j + T * m] = v[m];
+        for (int m = 0; m < E; ++m) a.Z[po + j + T * m] = v[m];
+    }
     acc0 = group_sum<T>(acc0);
     acc1 = group_sum<T>(acc1);
     if (j == 0) { red[g][0] = acc0; red[g][1] = acc1; }
@@ -161,15 +174,17 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
     const long long po = (long long)pair * a.nx * NY + kx;
     TwiddlesSmem<NY> tw;
     tw.w = tws + j;
-    float2 v[E];
+    if (!a.literal) {
+        float2 v[E];
 #pragma unroll
-    for (int m = 0; m < E; ++m) v[m] = a.Z[po + (long long)(j + T * m) * a.nx];
-    fft_line<NY, T>(v, smc + c * Cfg::CS, j, tw, BlockSync());
-    const float2 zero = make_float2(0.f, 0.f);
+        for (int m = 0; m < E; ++m) v[m] = a.Z[po + (long long)(j + T * m) * a.nx];
+        fft_line<NY, T>(v, smc + c * Cfg::CS, j, tw, BlockSync());
+        const float2 zero = make_float2(0.f, 0.f);
 #pragma unroll
-    for (int m = 0; m < E; ++m) {
-        a.phihat[po + (long long)(j + T * m) * a.nx] = v[m];
-        a.phat[0][po + (long long)(j + T * m) * a.nx] = zero;
+        for (int m = 0; m < E; ++m) {
+            a.phihat[po + (long long)(j + T * m) * a.nx] = v[m];
+            a.phat[0][po + (long long)(j + T * m) * a.nx] = zero;
+        }
     }
     if (blockIdx.x == 0 && threadIdx.x < 2) {
         const int b = threadIdx.x ? s1 : s0;
@@ -194,9 +209,11 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
 //   X^ = column FFT of Z (zero when n == 0) ; p^_{n+1} = (p^_n + sigma (D X^ - phi^))/(1 + sigma) ;
 //   Z <- column FFT of conj(D/(nx ny) p^_{n+1})      (the row kernel's FFT finishes the inverse transform)
 // want_gap: S1 = sum |dp|^2, S2 = Re sum dp(k) dp(-k), dp = p^_{n+1} - p^_n; the mirror column is in this CTA.
-template <int NY>
+// PLAIN (literal path): only Z <- column FFT of conj(D/(nx ny) X^), i.e. one application of K between two row passes;
+// `decide` is set for the first of the two column launches of an iteration.
+template <int NY, bool PLAIN>
 __global__ void __launch_bounds__(SfdColCfg<NY>::THREADS, SfdColCfg<NY>::THREADS <= 128 ? 4 : 2)
-sfd_cols_kernel(const StreamFdArgs a, const int n) {
+sfd_cols_kernel(const StreamFdArgs a, const int n, const int do_decide) {
     using Cfg = SfdColCfg<NY>;
     constexpr int E = Cfg::E, T = Cfg::T, NT = Cfg::THREADS;
     extern __shared__ __align__(16) unsigned char sfd_smem[];
@@ -209,7 +226,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
     int stop0 = a.stop_iter[s0], stop1 = has_b ? a.stop_iter[s1] : 0;
     if (n >= stop0 && n >= stop1) return;
 
-    const bool decide = n > 0 && a.tol > 0.f && (n % a.check_every) == 0;   // iteration n-1 was a checking one
+    const bool decide = do_decide && n > 0 && a.tol > 0.f && (n % a.check_every) == 0;   // iteration n-1 was a checking one
     if (decide) {
         if (threadIdx.x == 0) {
             const float2 g = sfd_gap_sum(a, pair, (n - 1) & 1);
@@ -230,7 +247,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
         if (n >= stop0 && n >= stop1) return;
     }
     const bool last = (n + 1 == a.max_iters);
-    const bool want_gap = last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0);
+    const bool want_gap = !PLAIN && (last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0));
 
     TwiddlesSmem<NY>::fill(tws, a.tw_col, threadIdx.x, NT);
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
@@ -249,7 +266,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
     __syncthreads();
 
     float2 v[E];
-    if (n > 0) {
+    if (n > 0 || PLAIN) {
 #pragma unroll
         for (int m = 0; m < E; ++m) v[m] = __ldcs(zc + (long long)(j + T * m) * nx);
         fft_line<NY, T>(v, smg, j, tw, BlockSync());
@@ -260,7 +277,13 @@ sfd_cols_kernel(const StreamFdArgs a, const int n) {
     const float2 sig2 = splat(a.sigma), inv2 = splat(a.inv_one_plus_sigma);
     const float NN = (float)nx * (float)NY;
     float S1 = 0.f, S2 = 0.f;
-    if (Cfg::STAGE) {
+    if (PLAIN) {
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const float d = __ldg(dcol + (long long)(j + T * m) * nx);
+            v[m] = make_float2(d * v[m].x, -d * v[m].y);
+        }
+    } else if (Cfg::STAGE) {
         // Park X^ in the column's exchange region (slot ky), so that the registers hold the loads of the update in
         // flight instead of the spectrum; each slot then receives p^_{n+1}, from which both the Parseval sums and
         // the next transform's input are taken.
@@ -516,6 +539,88 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
         const long long part = (long long)pair * a.nrowparts + blockIdx.x;
         if (k < 2) { if (want_gap) a.gap_row[part * 2 + k] = t; }
         else if ((k < 4) ? act0 : act1) a.res_part[part * 4 + (k - 2)] = t;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ dual rows (literal path)
+// W != I (or PD_OPT_FOURIER_DUAL = 0): p lives in the image domain, K is applied twice per iteration (PAPER.md:49
+// literally).  Iteration n:  [sfd_cols<PLAIN>]  this kernel  [sfd_cols<PLAIN>]  sfd_rows.
+//   u = K chibar_n: row FFT of Z gives (u_a, -u_b) (zero in iteration 0)
+//   p_{n+1} = (p_n + sigma W (u - phi)) / (1 + sigma)                      [PAPER.md:49 line 1; R2, R3]
+//   Z <- row FFT of W p_{n+1}        ;        data term of the gap 1/2 ||W(u - phi) - p_{n+1}||^2 per CTA
+// Same structure as sfd_rows: read-only double-buffered p, spectrum parked in the exchange region.
+template <int NX>
+__global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, 4)
+sfd_dual_rows_kernel(const StreamFdArgs a, const int n) {
+    using Cfg = SfdRowCfg<NX>;
+    constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
+    __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
+    __shared__ float2 tws[E * T];
+    __shared__ float red[G][2];
+
+    const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
+    const bool act0 = n < a.stop_iter[s0];
+    const bool act1 = (s1 < a.batch) && (n < a.stop_iter[s1]);
+    if (!act0 && !act1) return;
+    const bool last = (n + 1 == a.max_iters);
+    const bool want_gap = last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0);
+
+    TwiddlesSmem<NX>::fill(tws, a.tw_row, threadIdx.x, Cfg::THREADS);
+    const int g = threadIdx.x / T, j = threadIdx.x % T;
+    const int y = blockIdx.x * G + g;
+    float2 *smg = sm + g * Cfg::SM_PER_GROUP;
+    TwiddlesSmem<NX> tw;
+    tw.w = tws + j;
+    const long long po = ((long long)pair * a.ny + y) * NX;
+    float2 *zr = a.Z + po, *pw = a.phat[(n & 1) ^ 1] + po;
+    const float2 *pr = a.phat[n & 1] + po, *phi = a.phihat + po, *W = a.W2 + po;
+
+    float2 v[E];
+    if (n > 0) {
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = __ldcs(zr + j + T * m);
+    } else {
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = make_float2(0.f, 0.f);
+    }
+    __syncthreads();   // twiddle table
+    if (n > 0) fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
+    __syncwarp();      // the second FFT stage of the other threads has read the region
+#pragma unroll
+    for (int m = 0; m < E; ++m) smg[j + T * m] = v[m];
+
+    const float2 sig2 = splat(a.sigma), inv2 = splat(a.inv_one_plus_sigma), half2 = splat(0.5f);
+    const float2 sgn = make_float2(1.f, -1.f);   // lane y of the transform carries -u_b
+    float2 gap = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int x = j + T * m;
+        const float2 w = __ldg(W + x);
+        const float2 res = mul2(w, sub2(mul2(sgn, smg[x]), __ldg(phi + x)));
+        const float2 pn = mul2(fma2(sig2, res, __ldg(pr + x)), inv2);
+        if (want_gap) {
+            const float2 e = sub2(res, pn);
+            gap = fma2(mul2(e, half2), e, gap);
+        }
+        __stcs(pw + x, pn);
+        smg[x] = mul2(w, pn);
+    }
+#pragma unroll
+    for (int m = 0; m < E; ++m) v[m] = smg[j + T * m];
+    fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
+#pragma unroll
+    for (int m = 0; m < E; ++m) __stcs(zr + j + T * m, v[m]);
+
+    if (want_gap) {   // per-CTA partial sums, fixed order; read by sfd_gap_sum through gap_col (ncolparts = nrowparts)
+        gap.x = group_sum<T>(gap.x);
+        gap.y = group_sum<T>(gap.y);
+        if (j == 0) { red[g][0] = gap.x; red[g][1] = gap.y; }
+        __syncthreads();
+        if (threadIdx.x < 2) {
+            float t = 0.f;
+            for (int q = 0; q < G; ++q) t += red[q][threadIdx.x];
+            a.gap_col[n & 1][((long long)pair * a.ncolparts + blockIdx.x) * 2 + threadIdx.x] = t;
+        }
     }
 }
 

@@ -67,6 +67,10 @@ template <int N> struct SfdRowCfg {
 #endif
     static constexpr bool STAGE = N >= PD_SFD_STAGE_MIN;   // park the spectrum in shared memory during the update loop
     static constexpr int MINB = STAGE ? 5 : (N == 512 ? 3 : 4);
+#ifndef PD_SFD_UNROLL
+#define PD_SFD_UNROLL 4
+#endif
+    static constexpr int UNROLL = PD_SFD_UNROLL;           // elements of the update loop per unrolled body (STAGE only)
 };
 template <int N> struct SfdColCfg {
     static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
@@ -86,6 +90,10 @@ __host__ __device__ constexpr int sfd_column_of(int nx, int cb, int h, int cc) {
     const int lo = 8 * cb + cc;
     return h == 0 ? lo : (lo == 0 ? nx / 2 : nx - lo);
 }
+
+// L2 prefetch of one 128-byte line: no register is held while the line travels (used to start the operand rows of the
+// update loops before the first FFT of a line)
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // relgap of the pair's two lanes from the partial sums of iteration parity `par`, fixed order (same in every CTA)
 __device__ __forceinline__ float2 sfd_gap_sum(const StreamFdArgs &a, int pair, int par) {
@@ -269,6 +277,10 @@ sfd_cols_kernel(const StreamFdArgs a, const int n, const int do_decide) {
     if (n > 0 || PLAIN) {
 #pragma unroll
         for (int m = 0; m < E; ++m) v[m] = __ldcs(zc + (long long)(j + T * m) * nx);
+        if (!PLAIN && (c & 7) == 1) {   // the 64-byte segments of phi^ and p^_n this half-block of 8 columns will read
+#pragma unroll
+            for (int m = 0; m < E; ++m) { prefetch_l2(phh + (long long)(j + T * m) * nx); prefetch_l2(phr + (long long)(j + T * m) * nx); }
+        }
         fft_line<NY, T>(v, smg, j, tw, BlockSync());
     } else {
 #pragma unroll
@@ -432,6 +444,14 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
     float2 v[E];
 #pragma unroll
     for (int m = 0; m < E; ++m) v[m] = __ldcs(zr + j + T * m);
+    {   // own row of chi_n, chi_{n-1}, qx, qy (and M): one 128-byte line per 16 elements; the rows above and below are
+        // the neighbouring groups' own rows
+        constexpr int LINES = NX / 16;
+        for (int l = j; l < LINES; l += T) {
+            prefetch_l2(chn + 16 * l); prefetch_l2(chp + 16 * l); prefetch_l2(qxr + 16 * l); prefetch_l2(qyr + 16 * l);
+            if (MASKED) prefetch_l2(M + 16 * l);
+        }
+    }
     __syncthreads();   // twiddle table
     fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
     // STAGE: park K p in the group's exchange region during the update loop, so that the registers hold loads in
@@ -456,7 +476,10 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
     };
     float2 tmp, con;                                           // con: chi_n[y][x] of the next element
     float2 c0n = cbar_at(j, con), cun = has_up ? cbar_at(j - NX, tmp) : zero;
-#pragma unroll
+    // with the spectrum parked nothing in the loop is indexed by m at compile time: unroll by UNR only (the fully
+    // unrolled 512-point kernel was 120 KB of straight-line code, far beyond the instruction cache)
+    constexpr int UNR = STAGE ? Cfg::UNROLL : E;
+#pragma unroll UNR
     for (int m = 0; m < E; ++m) {
         const int x = j + T * m;
         const float2 c0 = c0n, cu = cun, c_old = con;          // chibar_n[y][x], chibar_n[y-1][x], chi_n[y][x]

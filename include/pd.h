@@ -143,6 +143,12 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size);
  * 0 when the schedule does not apply.  HOST pointer. */
 int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs);
 
+/* The rule behind the automatic tail (pure host arithmetic, no device needed): with `clusters` resident clusters in
+ * flight, each finishing one slice pair per wave, and the streaming side finishing about 0.19 * clusters pairs in the
+ * same time, the number of whole resident waves w that minimises max(w, tail / (0.19 * clusters)) is taken and
+ * tail = npairs - w * clusters (0 if that is negative) is returned. */
+int pd_hybrid_tail_rule(int npairs, int clusters);
+
 int pd_destroy(pd_plan_t p);
 
 const char *pd_strerror(int code);

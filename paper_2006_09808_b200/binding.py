@@ -23,7 +23,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -55,6 +55,7 @@ def lib():
         L.pd_last_launch_count.argtypes = [vp]
         L.pd_get_info.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
         L.pd_get_hybrid_tail.argtypes = [vp, C.POINTER(ip)]
+        L.pd_hybrid_tail_rule.argtypes = [ip, ip]
         L.pd_destroy.argtypes = [vp]
         L.pd_strerror.argtypes = [ip]
         L.pd_strerror.restype = C.c_char_p
@@ -92,6 +93,11 @@ def _stream_handle(stream):
     if isinstance(stream, int):
         return C.c_void_p(stream)
     return C.c_void_p(stream.cuda_stream)
+
+
+def hybrid_tail_rule(npairs, clusters):
+    """pd_hybrid_tail_rule: the automatic tail of the hybrid schedule for `npairs` slice pairs and `clusters` clusters."""
+    return lib().pd_hybrid_tail_rule(int(npairs), int(clusters))
 
 
 class Plan:

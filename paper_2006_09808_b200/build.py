@@ -15,7 +15,7 @@ LIB = os.path.join(HERE, "libpd_b200.so")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-shared", "-Xcompiler", "-fPIC",
-]
+] + os.environ.get("PD_EXTRA_NVCC_FLAGS", "").split()
 
 
 def sources():

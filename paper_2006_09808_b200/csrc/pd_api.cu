@@ -333,19 +333,22 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
 // `ncl` pairs per wave; the streaming kernels on the SMs they leave free finish about kHybridRho * ncl in the same
 // time (measured at 256x256).  Choose the number of resident waves w that minimises max(w, tail / (rho ncl)).
 constexpr double kHybridRho = 0.19;
-int hybrid_tail_pairs(const pd_plan_s *p) {
-    if (p->nx != 256 || p->weight || p->no_fd || p->variant != PD_VARIANT_AUTO || !p->aux) return 0;
-    if (p->hybrid_tail >= 0) return p->hybrid_tail < p->npairs ? p->hybrid_tail : p->npairs - 1;
-    const int ncl = p->res_max_clusters;
-    if (ncl * 8 + 16 > p->num_sms) return 0;   // no SMs left over
+int hybrid_tail_rule(int npairs, int ncl) {
+    if (npairs < 1 || ncl < 1) return 0;
     int best_tail = 0;
     double best_t = 1e30;
-    for (int w = (p->npairs + ncl - 1) / ncl; w >= 1; --w) {
-        const int tail = p->npairs > w * ncl ? p->npairs - w * ncl : 0;
+    for (int w = (npairs + ncl - 1) / ncl; w >= 1; --w) {
+        const int tail = npairs > w * ncl ? npairs - w * ncl : 0;
         const double ts = (double)tail / (kHybridRho * ncl), t = ts > w ? ts : (double)w;
         if (t < best_t - 1e-9) { best_t = t; best_tail = tail; }
     }
     return best_tail;
+}
+int hybrid_tail_pairs(const pd_plan_s *p) {
+    if (p->nx != 256 || p->weight || p->no_fd || p->variant != PD_VARIANT_AUTO || !p->aux) return 0;
+    if (p->hybrid_tail >= 0) return p->hybrid_tail < p->npairs ? p->hybrid_tail : p->npairs - 1;
+    if (p->res_max_clusters * 8 + 16 > p->num_sms) return 0;   // no SMs left over
+    return hybrid_tail_rule(p->npairs, p->res_max_clusters);
 }
 
 int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
@@ -748,6 +751,8 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
     if (cluster_size) *cluster_size = res ? p->res_csize : 0;
     return PD_OK;
 }
+
+int pd_hybrid_tail_rule(int npairs, int clusters) { return hybrid_tail_rule(npairs, clusters); }
 
 int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs) {
     if (!p || !tail_pairs) return PD_EINVAL;

@@ -64,3 +64,24 @@ def test_product_does_not_import_the_oracle():
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "#include \"../paper" not in text and "import paper_2006_09808_b200" not in text
             assert "csrc/" not in text.replace("paper_2006_09808_b200/csrc/", "")  # only mentioned in a comment
+
+
+def test_hybrid_tail_rule_host_logic(libpath):
+    """pd_hybrid_tail_rule (pure host arithmetic behind PD_OPT_HYBRID_TAIL = -1): the resident clusters
+    run whole waves, the tail is what is left, and it never asks the streaming side for more than it can do in that time."""
+    from paper_2006_09808_b200 import binding
+    rule = binding.hybrid_tail_rule
+    assert rule(64, 15) == 4        # NS: 128 slices = 64 pairs = 4 full waves of 15 + 4
+    assert rule(512, 15) == 77      # C3: 29 waves + 77 (30 waves + 62 would take one wave longer)
+    assert rule(32, 15) == 2        # C2
+    assert rule(15, 15) == 0 and rule(30, 15) == 0 and rule(7, 15) == 0   # whole waves / less than one wave: no tail
+    assert rule(0, 15) == 0 and rule(10, 0) == 0
+    rho = 0.19
+    for ncl in (1, 7, 15, 18):
+        for npairs in range(1, 400):
+            t = rule(npairs, ncl)
+            assert 0 <= t < npairs
+            assert (npairs - t) % ncl == 0 or t == 0          # the resident part is whole waves whenever a tail is split off
+            w = -(-(npairs - t) // ncl)
+            assert t / (rho * ncl) <= max(w, -(-npairs // ncl)) + 1e-9   # the tail never becomes the bottleneck vs no tail
+            assert max(w, t / (rho * ncl)) <= -(-npairs // ncl) + 1e-9   # never slower than the pure resident schedule

@@ -58,7 +58,8 @@ template <int N, int NT, class Tw>
 __device__ __forceinline__ void dual_fd_col(float2 *zc, const float *__restrict__ dpriv, const float2 *phh,
                                             float2 *ph_s, const int j, float2 *smg, const float2 *smg_mirror,
                                             const Tw &tw, const ResidentFdArgs &a, const bool first,
-                                            const bool want_gap, float &S1, float &S2) {
+                                            const bool want_gap, float &S1, float &S2,
+                                            const float2 (&pht)[FftCfg<N>::E]) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
     float2 v[E];
     float dv[E];
@@ -78,7 +79,7 @@ __device__ __forceinline__ void dual_fd_col(float2 *zc, const float *__restrict_
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const float d = dv[m];
-        const float2 phat = ldcg2(phh + m * NT);
+        const float2 phat = pht[m];   // phi^, loaded by the caller while it waited at the cluster barrier
         const float2 pold = ph_s[m * NT];
         const float2 res = sub2(mul2(splat(d * NN), v[m]), phat);
         const float2 pn = mul2(fma2(sig2, res, pold), inv2);
@@ -254,6 +255,7 @@ resident_fd_kernel(const ResidentFdArgs a) {
         if (stop_a == 0) for (int i = tid; i < RPC * N; i += NT) a.chi_out[(long long)s0 * P + row0 * N + i] = 0.f;
         if (has_b && stop_b == 0) for (int i = tid; i < RPC * N; i += NT) a.chi_out[(long long)s1 * P + row0 * N + i] = 0.f;
 
+        float2 pht[E];
         for (int n = 0; n < a.max_iters; ++n) {
             const bool act_a = n < stop_a, act_b = n < stop_b;
             if (!act_a && !act_b) break;
@@ -263,7 +265,11 @@ resident_fd_kernel(const ResidentFdArgs a) {
 
             // (1) column phase: p^_{n+1} and the spectrum of K p_{n+1}
             float S1 = 0.f, S2 = 0.f;
-            dual_fd_col<N, NT>(zcol, dpriv, phh, ph_s, cj, smg_col, smg_mir, tw_col, a, n == 0, want_gap, S1, S2);
+            if (n == 0) {
+#pragma unroll
+                for (int m = 0; m < E; ++m) pht[m] = ldcg2(phh + m * NT);
+            }
+            dual_fd_col<N, NT>(zcol, dpriv, phh, ph_s, cj, smg_col, smg_mir, tw_col, a, n == 0, want_gap, S1, S2, pht);
             // (2) q-update from chibar_n (chibar_0 = 0 and q_0 = 0: nothing to do in the first iteration)
             float2 gap = zero;
             if (n > 0) q_update_row<N, NT, ANISO>(r, qa, y, j, want_gap, gap);
@@ -301,7 +307,11 @@ resident_fd_kernel(const ResidentFdArgs a) {
                     if (tid < 4 && ((tid < 2) ? out_a != nullptr : out_b != nullptr)) part[rank * 8 + 4 + tid] = t;
                 }
             }
-            cluster_sync_all<C>();
+            // the next column phase's thread-private operand phi^ travels while the cluster barrier is waited for
+            cluster_arrive<C>();
+#pragma unroll
+            for (int m = 0; m < E; ++m) pht[m] = ldcg2(phh + m * NT);
+            cluster_wait<C>();
         }
         // ---- per-slice state variables
         if (rank == 0 && tid < 2 && (tid == 0 || has_b)) {

@@ -3,7 +3,7 @@
 // No CPU fallback exists: every arithmetic step of the path runs in the kernels of pd_resident*.cuh / pd_streaming_fd.cuh.
 #include "../../include/pd.h"
 #include "pd_resident.cuh"
-#include "pd_resident_fd.cuh"
+#include "pd_resident_tm.cuh"
 #include "pd_streaming_fd.cuh"
 
 #include <cmath>
@@ -13,7 +13,7 @@
 #include <vector>
 
 using pdk::ResidentArgs;
-using pdk::ResidentFdArgs;
+using pdk::ResidentTmArgs;
 using pdk::StreamFdArgs;
 
 namespace {
@@ -56,7 +56,7 @@ struct pd_plan_s {
     int res_csize;         // CTAs per cluster
     float2 *res_scratch;   // [kResidentScratchArrays][res_clusters][nx*ny]
     float *rk_part;        // [res_clusters][res_csize][8]
-    float *Dpriv;          // D/(nx*ny) in the thread-private order of the Fourier-domain-dual kernel (pd_resident_fd.cuh)
+    float *Dpriv;          // D/(nx*ny) in the thread-private order of the Fourier-domain-dual kernel (pd_resident_tm.cuh)
     // streaming variant with the Fourier-domain dual (pd_streaming_fd.cuh): allocated on first use
     float2 *sfd_planes;    // 11 arrays of [npairs][ny][nx] float2
     float *sfd_parts;      // per-CTA partial sums
@@ -211,13 +211,13 @@ cudaError_t resident_launch(const ResidentArgs &a, bool w, bool aniso, int nclus
     return aniso ? resident_launch2<N, false, true>(a, nclusters, st) : resident_launch2<N, false, false>(a, nclusters, st);
 }
 
-// ---- Fourier-domain-dual resident kernel (W = identity): same cluster shape and shared-memory budget
+// ---- resident kernel with the state on chip (W = identity; pd_resident_tm.cuh): same cluster shape
 template <int N, bool ANISO>
-cudaError_t resident_fd_launch2(const ResidentFdArgs &a, int nclusters, cudaStream_t st) {
+cudaError_t resident_tm_launch2(const ResidentTmArgs &a, int nclusters, cudaStream_t st) {
     using Ch = ResChoice<N>;
-    using Cfg = pdk::ResCfg<N, Ch::C, Ch::NT>;
-    auto kern = pdk::resident_fd_kernel<N, Ch::C, Ch::NT, Ch::MINB, ANISO>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    using TCfg = pdk::ResTmCfg<N, Ch::C, Ch::NT>;
+    auto kern = pdk::resident_tm_kernel<N, Ch::C, Ch::NT, ANISO>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, TCfg::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     if (Ch::C > 8) {
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
@@ -228,7 +228,7 @@ cudaError_t resident_fd_launch2(const ResidentFdArgs &a, int nclusters, cudaStre
     std::memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)(nclusters * Ch::C), 1, 1);
     cfg.blockDim = dim3(Ch::NT, 1, 1);
-    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.dynamicSmemBytes = TCfg::SMEM_BYTES;
     cfg.stream = st;
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = Ch::C;
@@ -239,11 +239,11 @@ cudaError_t resident_fd_launch2(const ResidentFdArgs &a, int nclusters, cudaStre
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 template <int N>
-cudaError_t resident_fd_launch(const ResidentFdArgs &a, bool aniso, int nclusters, cudaStream_t st) {
-    return aniso ? resident_fd_launch2<N, true>(a, nclusters, st) : resident_fd_launch2<N, false>(a, nclusters, st);
+cudaError_t resident_tm_launch(const ResidentTmArgs &a, bool aniso, int nclusters, cudaStream_t st) {
+    return aniso ? resident_tm_launch2<N, true>(a, nclusters, st) : resident_tm_launch2<N, false>(a, nclusters, st);
 }
 
-// D/(N*N) in the order the column phase of resident_fd_kernel reads it: [rank][m][tid] (pd_resident_fd.cuh)
+// D/(N*N) in the order the column phase of resident_tm_kernel reads it: [rank][m][tid] (pd_resident_tm.cuh)
 template <int N>
 void build_dipole_private(std::vector<float> &out, const std::vector<float> &D) {
     using Ch = ResChoice<N>;
@@ -391,20 +391,20 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
     const int nclusters = res_pairs < p->res_clusters ? res_pairs : p->res_clusters;
     cudaError_t e;
     if (!w && !p->no_fd) {
-        // W = identity: the dual variable p stays in the Fourier domain (pd_resident_fd.cuh)
-        ResidentFdArgs f;
+        // W = identity: Fourier-domain dual, state in tensor memory and shared memory (pd_resident_tm.cuh)
+        ResidentTmArgs f;
         std::memset(&f, 0, sizeof(f));
         f.batch = a.batch; f.npairs = a.npairs; f.max_iters = a.max_iters; f.check_every = a.check_every;
         f.alpha = a.alpha; f.sigma = a.sigma; f.tau = a.tau; f.theta = a.theta;
         f.inv_one_plus_sigma = a.inv_one_plus_sigma; f.tol = a.tol;
         f.field = field; f.mask = mask; f.mask_bstride = a.mask_bstride; f.chi_out = chi_out;
-        f.Z = a.Z; f.qy = a.qy; f.chi = a.chi; f.chibar = a.chibar; f.M2 = a.M2; f.phihat = a.phi2;
+        f.Z = a.Z; f.M2 = a.M2;
         f.Dpriv = p->Dpriv; f.tw_tab = p->tw_row; f.part = p->rk_part;
         f.iters_done = p->iters_done; f.relgap = p->relgap; f.relres = p->relres;
         switch (p->nx) {
-            case 64: e = resident_fd_launch<64>(f, aniso, nclusters, st); break;
-            case 128: e = resident_fd_launch<128>(f, aniso, nclusters, st); break;
-            default: e = resident_fd_launch<256>(f, aniso, nclusters, st); break;
+            case 64: e = resident_tm_launch<64>(f, aniso, nclusters, st); break;
+            case 128: e = resident_tm_launch<128>(f, aniso, nclusters, st); break;
+            default: e = resident_tm_launch<256>(f, aniso, nclusters, st); break;
         }
     } else
     switch (p->nx) {

@@ -2,7 +2,7 @@
 // launches per iteration, described first); the literal iteration for W != I on the same planes (four launches,
 // sfd_dual_rows_kernel and sfd_cols_kernel<PLAIN> further down).
 //
-// Same algebra as pd_resident_fd.cuh (PAPER.md:49 line 1 commutes with the FFT when W = I):
+// Same algebra as pd_resident_tm.cuh (PAPER.md:49 line 1 commutes with the FFT when W = I):
 //     p^_{n+1} = (p^_n + sigma (D X^_n - phi^)) / (1 + sigma),   X^_n = F chibar_n,   K p_{n+1} = F^-1 (D p^_{n+1}),
 // so one iteration is ONE forward 2-D FFT and ONE inverse: two launches over the whole batch instead of four,
 //   fd_cols : column FFT of Z (= X^_n), p^ update, column FFT of conj(D/(nx ny) p^_{n+1})      [PAPER.md:49 line 1]
@@ -24,7 +24,7 @@
 // chi_{n-1} r8, chi_{n+1} w8, qx r8 w8, qy r8 w8, M r8 = 80  ->  60 B per pixel of one slice and iteration, 56 without
 // a mask.
 //
-// Gap (R9): data term by Parseval over mirror-paired columns (as in pd_resident_fd.cuh), q term in fd_rows;
+// Gap (R9): data term by Parseval over mirror-paired columns (as in pd_resident_tm.cuh), q term in fd_rows;
 // both as per-CTA partial sums.  Every CTA of fd_cols(n+1) reduces the partials of iteration n in the same fixed
 // order and reaches the same stop decision; column block 0 records it.  No host round trip.
 #pragma once
@@ -380,7 +380,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n, const int do_decide) {
         if (threadIdx.x == 0) {
             float t1 = 0.f, t2 = 0.f;
             for (int w = 0; w < NT / 32; ++w) { t1 += dec[2 + 2 * w]; t2 += dec[3 + 2 * w]; }
-            // 1/2 sum_x e^2 = (S1 +- S2) / (4 nx ny sigma^2)   (Parseval; pd_resident_fd.cuh header)
+            // 1/2 sum_x e^2 = (S1 +- S2) / (4 nx ny sigma^2)   (Parseval; pd_resident_tm.cuh header)
             const float scale = 0.25f / (NN * a.sigma * a.sigma);
             float *gc = a.gap_col[n & 1] + ((long long)pair * a.ncolparts + blockIdx.x) * 2;
             gc[0] = scale * (t1 + t2);

@@ -51,6 +51,16 @@ NCU_DRAM_BYTES_PER_PX = {
 }
 PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
 
+# What ncu measured on the resident kernel of THIS build (profiles/r02/, one `--set full` capture of the kernel alone on
+# C2 and one metrics-only pass over every launch of a hybrid C3 step); quoted beside the live numbers, never timed here.
+NCU_RESIDENT = {
+    "source": "profiles/r02/ncu_resident_tm_c2.txt, profiles/r02/dram_bytes_C3_hybrid_step.md",
+    "issue_slots_busy_pct": None, "fma_pipe_pct": None, "l1tex_pct": None, "l2_pct": None, "shared_wavefronts_pct_of_peak": None,
+    "l2_bytes_per_pixel_pair_iteration": None,
+}
+# dram__bytes_read.sum + dram__bytes_write.sum summed over every launch of one step (resident kernel + streaming tail)
+NCU_DRAM_BYTES_PER_STEP = {}   # (workload, hybrid_tail_pairs) -> bytes
+
 
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -135,6 +145,24 @@ def time_oracle(cfg, data, nsample):
     return float(out["iters_done"].sum()) / dt, dt, int(out["iters_done"].sum())
 
 
+def time_oracle_all_cores(cfg, data, nsample):
+    """Parallel-for over slices OUTSIDE the oracle (one single-threaded oracle call per slice on a thread pool; the
+    ctypes call releases the GIL), on every host core."""
+    from concurrent.futures import ThreadPoolExecutor
+    orc = oracle_module()
+    ncores = os.cpu_count() or 1
+
+    def one(b):
+        out = orc.solve(data["field"][b:b + 1], data["mask"][b:b + 1], lambda_=cfg.lam, sigma=cfg.sigma, tau=cfg.tau,
+                        theta=cfg.theta, max_iters=cfg.iters, tol=cfg.tol, precision="f32", want_hist=False)
+        return int(out["iters_done"].sum())
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=ncores) as ex:
+        its = sum(ex.map(one, range(nsample)))
+    dt = time.perf_counter() - t0
+    return its / dt, dt, its, ncores
+
+
 def oracle_sample_size(cfg):
     """Batch entries giving roughly 10-30 s of single-core oracle work (about 8e-7 s per pixel-iteration measured)."""
     per_slice = 8e-7 * cfg.nx * cfg.ny * (cfg.iters if cfg.tol <= 0 else min(cfg.iters, 80))
@@ -171,6 +199,11 @@ def run_reference(args):
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+def flops_per_slice_it_ns(cfg):
+    P = cfg.nx * cfg.ny
+    return P * (10.0 * math.log2(P) + 32.0)
 
 
 def workload_config(cfg, name, batch_per_gpu, ngpus):
@@ -245,6 +278,7 @@ def main():
     plan_info["weighted"] = bool(args.weighted)
     plan_info["mask"] = "none (all ones)" if mask_is_one else "per slice"
     plan_info["hybrid_tail_pairs"] = plan.hybrid_tail()
+    plan_info["hybrid_rho_measured_at_plan_time"] = plan.hybrid_rho()
     small = batch * P * 32 <= 2 * 126e6
     flush = torch.empty(64 * 1024 * 1024, device="cuda") if small else None
 
@@ -310,39 +344,50 @@ def main():
     peak, peak_src = load_peaks()
     dom = max(KERNEL_BYTES_PER_PX, key=lambda k: ktot.get(k, [0.0, 0])[0])
     dom_ms, dom_n = ktot[dom]
-    # units one launch processes: every active slice once; averaged over the launches of the solve (a stopped slice is
-    # skipped by later launches), = batch when no tolerance is set
-    avg_active_slices = float(its_local.sum()) / max(cfg.iters, 1)
-    per_px = KERNEL_BYTES_PER_PX[dom] - (4.0 if (dom == "fd_rows" and mask_is_one) else 0.0)
-    bytes_per_launch = per_px * P * avg_active_slices
-    if dom == "resident":   # a single launch runs every iteration of every slice
-        bytes_per_launch = KERNEL_BYTES_PER_PX[dom] * P * float(its_local.sum())
-    achieved = bytes_per_launch / (dom_ms / dom_n * 1e-3) / 1e9
-    ncu_px = NCU_DRAM_BYTES_PER_PX.get((dom, cfg.nx if dom == "fd_rows" else cfg.ny, not mask_is_one))
-    traffic = ncu_px * P * avg_active_slices if ncu_px is not None else None
-    if dom == "resident" and cfg.nx == 256 and plan_info.get("hybrid_tail_pairs", 0) == 0 and not args.weighted:
-        # ncu_resident_fd_c2_v3.txt: 34.2 + 25.6 MB for 64 slices of 256x256, whole solve (load + store only)
-        traffic = 14.26 * P * batch
     ksum = sum(v[0] for v in ktot.values())
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
-                "avg_launch_us": 1e3 * dom_ms / dom_n, "share_of_step": dom_ms / ksum,
-                "kernel_ms_per_step": {k: v[0] / args.steps for k, v in ktot.items()},
-                "step_ms_with_events": ms_evt / args.steps}
-    path_bytes = PATH_FLOOR_BYTES_PER_PX * P * float(its_local.sum())
-    roofline_path = {"bound": "hbm", "what": "whole path at the 48 B/px/slice-iteration streaming floor", "unit": "GB/s",
-                     "achieved": path_bytes * args.steps / (ms * 1e-3) / 1e9 if world == 1 else path_bytes / (ms / args.steps * 1e-3) / 1e9,
-                     "peak": peak}
-    roofline_path["frac"] = roofline_path["achieved"] / peak
-    # FP32 view of the same step: algorithmic flops P (10 log2 P + 32) per slice-iteration against
-    # 148 SMs x 128 lanes x 2 flop x SM clock
-    sm_mhz = load_sm_mhz()
+    slice_its_local = float(its_local.sum())
+    # FP32 peak of the CUDA cores: NOMINAL (148 SMs x 128 lanes x 2 flop) at the SM clock sampled during the timed region
+    sm_mhz = (clocks or {}).get("sm_mhz") or load_sm_mhz()
     alu_peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12
-    flops = P * (10.0 * math.log2(P) + 32.0) * float(its_local.sum())
-    alu_ach = flops * (args.steps if world == 1 else 1) / ((ms if world == 1 else ms / args.steps) * 1e-3) / 1e12
+    alu_src = "nominal: 148 SMs x 128 FP32 lanes x 2 flop x %.0f MHz (SM clock sampled during the timed region)" % sm_mhz
+    flops_per_slice_it = P * (10.0 * math.log2(P) + 32.0)   # algorithmic, two K applications per iteration
+    common = {"kernel": dom, "avg_launch_us": 1e3 * dom_ms / dom_n, "share_of_step": dom_ms / ksum,
+              "kernel_ms_per_step": {k: v[0] / args.steps for k, v in ktot.items()}, "step_ms_with_events": ms_evt / args.steps}
+    if dom == "resident":
+        # One launch runs every iteration of every slice (with the hybrid schedule the bracket also covers the streaming
+        # tail on the second stream).  HBM is touched at load and store only, so the bound SURVEY.md 8(d) names is
+        # max(shared memory, FP32 pipe): report the FP32 fraction, the ncu percentages beside it.
+        flops = flops_per_slice_it * slice_its_local
+        achieved = flops / (dom_ms / dom_n * 1e-3) / 1e12
+        traffic = NCU_DRAM_BYTES_PER_STEP.get((args.workload, plan_info.get("hybrid_tail_pairs", 0)))
+        roofline = dict(common, bound="alu", achieved=achieved, peak=alu_peak, unit="TFLOP/s", frac=achieved / alu_peak,
+                        traffic=traffic, peak_source=alu_src, flops_per_launch=flops,
+                        flops_model="P (10 log2 P + 32) per slice-iteration (SURVEY.md 8(d)); the Fourier-domain dual executes "
+                                    "about 0.58 of that (one FFT round trip per iteration instead of two)",
+                        ncu=NCU_RESIDENT,
+                        vs_streaming_floor={"what": "the same step against a perfect streaming kernel at 48 B/px/slice-iteration "
+                                                    "(no such bytes move: the state is on chip)",
+                                            "frac": PATH_FLOOR_BYTES_PER_PX * P * slice_its_local / (dom_ms / dom_n * 1e-3) / 1e9 / peak})
+    else:
+        # units one launch processes: every active slice once; averaged over the launches of the solve (a stopped slice
+        # is skipped by later launches), = batch when no tolerance is set
+        avg_active_slices = slice_its_local / max(cfg.iters, 1)
+        per_px = KERNEL_BYTES_PER_PX[dom] - (4.0 if (dom == "fd_rows" and mask_is_one) else 0.0)
+        bytes_per_launch = per_px * P * avg_active_slices
+        achieved = bytes_per_launch / (dom_ms / dom_n * 1e-3) / 1e9
+        ncu_px = NCU_DRAM_BYTES_PER_PX.get((dom, cfg.nx if dom == "fd_rows" else cfg.ny, not mask_is_one))
+        traffic = ncu_px * P * avg_active_slices if ncu_px is not None else None
+        roofline = dict(common, bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, traffic=traffic,
+                        peak_source=peak_src, bytes_per_launch=bytes_per_launch)
+    step_s = (ms / args.steps) * 1e-3
+    path_bytes = PATH_FLOOR_BYTES_PER_PX * P * slice_its_local
+    roofline_path = {"bound": "hbm", "what": "whole path at the 48 B/px/slice-iteration streaming floor", "unit": "GB/s",
+                     "achieved": path_bytes / step_s / 1e9, "peak": peak}
+    roofline_path["frac"] = roofline_path["achieved"] / peak
+    # FP32 view of the whole step (all kernels, launch gaps included)
+    alu_ach = flops_per_slice_it * slice_its_local / step_s / 1e12
     roofline_alu = {"bound": "alu", "what": "whole path, algorithmic flops P(10 log2 P + 32) per slice-iteration",
-                    "unit": "TFLOP/s", "achieved": alu_ach, "peak": alu_peak, "frac": alu_ach / alu_peak,
-                    "peak_source": "148 SMs x 128 FP32 lanes x 2 x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz, else 1965)" % sm_mhz}
+                    "unit": "TFLOP/s", "achieved": alu_ach, "peak": alu_peak, "frac": alu_ach / alu_peak, "peak_source": alu_src}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), H2D and D2H inside the timed region
     e2e = None
@@ -383,17 +428,22 @@ def main():
         extra = {"workload": "NS: 128 slices x 256x256, 1 field map per slice, 200 iterations (BASELINE.json north_star target)",
                  "stack_recon_ms": t_ns, "slice_iterations_per_s": ns.batch * ns.iters / (t_ns * 1e-3),
                  "hbm_floor_frac": PATH_FLOOR_BYTES_PER_PX * ns.nx * ns.ny * ns.batch * ns.iters / (t_ns * 1e-3) / 1e9 / peak,
+                 "fp32_frac": flops_per_slice_it_ns(ns) * ns.batch * ns.iters / (t_ns * 1e-3) / 1e12 / alu_peak,
                  "hybrid_tail_pairs": plan2.hybrid_tail()}
         plan2.destroy()
 
     if rank == 0:
         cpu = None
         if not args.no_cpu_baseline and world == 1:
-            nsample = oracle_sample_size(cfg)
+            nsample = max(1, oracle_sample_size(cfg) // 2)
             v, dt, n = time_oracle(cfg, data, nsample)
+            nall = min(batch, nsample * (os.cpu_count() or 1))
+            va, dta, na, ncores = time_oracle_all_cores(cfg, data, nall)
             cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                    "sample": "first %d of %d batch entries of the same inputs, %d slice-iterations in %.1f s, float instantiation"
                              % (nsample, batch, n, dt),
+                   "all_cores": {"value": va, "unit": UNIT, "cores": ncores, "kind": "oracle, parallel-for over slices outside it",
+                                 "sample": "first %d of %d batch entries, %d slice-iterations in %.1f s" % (nall, batch, na, dta)},
                    "host_cores_available": os.cpu_count()}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

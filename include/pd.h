@@ -144,10 +144,15 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size);
 int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs);
 
 /* The rule behind the automatic tail (pure host arithmetic, no device needed): with `clusters` resident clusters in
- * flight, each finishing one slice pair per wave, and the streaming side finishing about 0.19 * clusters pairs in the
- * same time, the number of whole resident waves w that minimises max(w, tail / (0.19 * clusters)) is taken and
+ * flight, each finishing one slice pair per wave, and the streaming side finishing about rho * clusters pairs in the
+ * same time, the number of whole resident waves w that minimises max(w, tail / (rho * clusters)) is taken and
  * tail = npairs - w * clusters (0 if that is negative) is returned. */
-int pd_hybrid_tail_rule(int npairs, int clusters);
+int pd_hybrid_tail_rule(int npairs, int clusters, float rho);
+
+/* rho of this plan: measured by pd_plan on the plan's device (one wave of resident clusters and a few slice pairs
+ * through the streaming kernels, run concurrently on a synthetic field; a few ms), or the built-in 0.15 when the batch
+ * is too small for a tail or the size has no hybrid schedule.  HOST pointer. */
+int pd_get_hybrid_rho(pd_plan_t p, float *rho);
 
 int pd_destroy(pd_plan_t p);
 

@@ -23,7 +23,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_get_hybrid_rho", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -55,7 +55,8 @@ def lib():
         L.pd_last_launch_count.argtypes = [vp]
         L.pd_get_info.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
         L.pd_get_hybrid_tail.argtypes = [vp, C.POINTER(ip)]
-        L.pd_hybrid_tail_rule.argtypes = [ip, ip]
+        L.pd_hybrid_tail_rule.argtypes = [ip, ip, fp]
+        L.pd_get_hybrid_rho.argtypes = [vp, C.POINTER(fp)]
         L.pd_destroy.argtypes = [vp]
         L.pd_strerror.argtypes = [ip]
         L.pd_strerror.restype = C.c_char_p
@@ -95,9 +96,10 @@ def _stream_handle(stream):
     return C.c_void_p(stream.cuda_stream)
 
 
-def hybrid_tail_rule(npairs, clusters):
-    """pd_hybrid_tail_rule: the automatic tail of the hybrid schedule for `npairs` slice pairs and `clusters` clusters."""
-    return lib().pd_hybrid_tail_rule(int(npairs), int(clusters))
+def hybrid_tail_rule(npairs, clusters, rho):
+    """pd_hybrid_tail_rule: the automatic tail of the hybrid schedule for `npairs` slice pairs, `clusters` clusters and
+    a streaming side that finishes rho * clusters pairs per resident wave."""
+    return lib().pd_hybrid_tail_rule(int(npairs), int(clusters), float(rho))
 
 
 class Plan:
@@ -183,6 +185,12 @@ class Plan:
         n = C.c_int()
         _check(lib().pd_get_hybrid_tail(self._h, C.byref(n)))
         return n.value
+
+    def hybrid_rho(self):
+        """pd_get_hybrid_rho: the streaming-to-resident rate ratio pd_plan measured for the hybrid schedule."""
+        r = C.c_float()
+        _check(lib().pd_get_hybrid_rho(self._h, C.byref(r)))
+        return r.value
 
     @property
     def last_launch_count(self):

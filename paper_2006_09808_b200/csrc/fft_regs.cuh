@@ -118,6 +118,10 @@ struct WarpSync {   // the T threads of a line sit in one warp
 struct BlockSync {  // the T threads of a line are spread over the warps of the CTA
     __device__ __forceinline__ void operator()() const { __syncthreads(); }
 };
+struct NamedSync {  // ... over `count` threads (whole warps) that all use hardware barrier `id` (1..15)
+    int id, count;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+};
 
 // Per-thread inter-stage twiddles W_N^(j*k2), k2 = 1..E-1 (index 0 unused), from the plan's double-precision table.
 template <int N>

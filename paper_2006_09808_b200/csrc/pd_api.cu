@@ -48,7 +48,7 @@ struct pd_plan_s {
     int *stop_iter, *iters_done;
     float *P0, *relgap, *relres;
     int nparts;
-    // resident variant (pd_resident.cuh): per-cluster scratch, 9 arrays of nx*ny float2 per cluster
+    // resident variant (pd_resident.cuh): per-cluster scratch, kResidentScratchArrays arrays of nx*ny float2 per cluster
     int res_ok;            // this size has a resident kernel
     int res_clusters;      // clusters launched (= scratch slots)
     int res_max_clusters;  // what the occupancy query allows
@@ -65,6 +65,7 @@ struct pd_plan_s {
     // hybrid schedule (256x256, W = I, PD_VARIANT_AUTO): the resident clusters cover 120 of the 148 SMs; the last
     // `tail` slice pairs run through the streaming kernels on a second stream, on the SMs the clusters leave free
     int hybrid_tail;       // -1: automatic ; >= 0: slice pairs given to the streaming kernels
+    double hybrid_rho;     // streaming pairs per resident pair and cluster, measured at plan time (calibrate_hybrid)
     cudaStream_t aux;
     cudaEvent_t ev_fork, ev_join;
     // host-buffer entry point staging
@@ -327,35 +328,39 @@ cudaError_t sfd_set_col_smem() {
 int resident_csize(int n) { return n == 64 ? ResChoice<64>::C : n == 128 ? ResChoice<128>::C : ResChoice<256>::C; }
 
 int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
-                       cudaStream_t st, int first = 0, int *launches_out = nullptr);
+                       cudaStream_t st, int first = 0, int *launches_out = nullptr, int count = 0);
 
 // Hybrid schedule: slice pairs handed to the streaming kernels.  The resident clusters finish
-// `ncl` pairs per wave; the streaming kernels on the SMs they leave free finish about kHybridRho * ncl in the same
-// time (measured at 256x256).  Choose the number of resident waves w that minimises max(w, tail / (rho ncl)).
-constexpr double kHybridRho = 0.19;
-int hybrid_tail_rule(int npairs, int ncl) {
-    if (npairs < 1 || ncl < 1) return 0;
+// `ncl` pairs per wave; the streaming kernels on the SMs they leave free finish about rho * ncl in the same time.
+// rho is MEASURED on the plan's device when the plan is made (calibrate_hybrid below); kHybridRhoDefault is only the
+// value of a plan whose batch is too small to calibrate.  Choose the number of resident waves w that minimises
+// max(w, tail / (rho ncl)).
+constexpr double kHybridRhoDefault = 0.15;
+int hybrid_tail_rule(int npairs, int ncl, double rho) {
+    if (npairs < 1 || ncl < 1 || !(rho > 0.0)) return 0;
     int best_tail = 0;
     double best_t = 1e30;
     for (int w = (npairs + ncl - 1) / ncl; w >= 1; --w) {
         const int tail = npairs > w * ncl ? npairs - w * ncl : 0;
-        const double ts = (double)tail / (kHybridRho * ncl), t = ts > w ? ts : (double)w;
+        const double ts = (double)tail / (rho * ncl), t = ts > w ? ts : (double)w;
         if (t < best_t - 1e-9) { best_t = t; best_tail = tail; }
     }
     return best_tail;
 }
+bool hybrid_possible(const pd_plan_s *p) {
+    return p->nx == 256 && p->aux && p->res_max_clusters * 8 + 16 <= p->num_sms;   // SMs left over beside the clusters
+}
 int hybrid_tail_pairs(const pd_plan_s *p) {
     if (p->nx != 256 || p->weight || p->no_fd || p->variant != PD_VARIANT_AUTO || !p->aux) return 0;
     if (p->hybrid_tail >= 0) return p->hybrid_tail < p->npairs ? p->hybrid_tail : p->npairs - 1;
-    if (p->res_max_clusters * 8 + 16 > p->num_sms) return 0;   // no SMs left over
-    return hybrid_tail_rule(p->npairs, p->res_max_clusters);
+    if (!hybrid_possible(p)) return 0;
+    return hybrid_tail_rule(p->npairs, p->res_max_clusters, p->hybrid_rho);
 }
 
-int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
-                   cudaStream_t st) {
+// The resident kernel over the first res_pairs slice pairs (res_batch slices) of the caller's arrays
+cudaError_t launch_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                            cudaStream_t st, int res_pairs, int res_batch) {
     const size_t P = (size_t)p->nx * p->ny;
-    const int tail = hybrid_tail_pairs(p);
-    const int res_pairs = p->npairs - tail, res_batch = tail ? 2 * res_pairs : p->batch;
     ResidentArgs a;
     std::memset(&a, 0, sizeof(a));
     a.batch = res_batch; a.npairs = res_pairs; a.max_iters = max_iters; a.check_every = p->check_every;
@@ -373,7 +378,89 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
     a.Dtab = p->Dtab; a.tw_tab = p->tw_row;
     a.part = p->rk_part;
     a.iters_done = p->iters_done; a.relgap = p->relgap; a.relres = p->relres;
+    const bool w = p->weight != nullptr, aniso = p->tv_mode == PD_TV_ANISO;
+    const int nclusters = res_pairs < p->res_clusters ? res_pairs : p->res_clusters;
+    if (!w && !p->no_fd) {
+        // W = identity: Fourier-domain dual, state in tensor memory and shared memory (pd_resident_tm.cuh)
+        ResidentTmArgs f;
+        std::memset(&f, 0, sizeof(f));
+        f.batch = a.batch; f.npairs = a.npairs; f.max_iters = a.max_iters; f.check_every = a.check_every;
+        f.alpha = a.alpha; f.sigma = a.sigma; f.tau = a.tau; f.theta = a.theta;
+        f.inv_one_plus_sigma = a.inv_one_plus_sigma; f.tol = a.tol;
+        f.field = field; f.mask = mask; f.mask_bstride = a.mask_bstride; f.chi_out = chi_out;
+        f.Z = a.Z; f.M2 = a.M2;
+        f.Dpriv = p->Dpriv; f.tw_tab = p->tw_row; f.part = p->rk_part;
+        f.iters_done = p->iters_done; f.relgap = p->relgap; f.relres = p->relres;
+        switch (p->nx) {
+            case 64: return resident_tm_launch<64>(f, aniso, nclusters, st);
+            case 128: return resident_tm_launch<128>(f, aniso, nclusters, st);
+            default: return resident_tm_launch<256>(f, aniso, nclusters, st);
+        }
+    }
+    switch (p->nx) {
+        case 64: return resident_launch<64>(a, w, aniso, nclusters, st);
+        case 128: return resident_launch<128>(a, w, aniso, nclusters, st);
+        default: return resident_launch<256>(a, w, aniso, nclusters, st);
+    }
+}
 
+// rho of the hybrid schedule, measured at plan time on this device: one wave of resident clusters and a few slice pairs
+// through the streaming kernels run CONCURRENTLY (as in a hybrid solve: the streaming CTAs land on the SMs the clusters
+// leave free) on a constant synthetic field, iteration counts chosen so that both sides take about the same time; rho =
+// (streaming pair-iterations per ms) / (resident pair-iterations per ms per cluster) / clusters.  Costs a few ms.
+int calibrate_hybrid(pd_plan_s *p) {
+    const int ncl = p->res_max_clusters;
+    const int ps = p->npairs - ncl < 6 ? p->npairs - ncl : 6;   // streaming pairs of the calibration
+    p->hybrid_rho = kHybridRhoDefault;
+    if (!hybrid_possible(p) || ps < 1) return PD_OK;
+    const size_t P = (size_t)p->nx * p->ny, nsl = 2 * (size_t)(ncl + ps);
+    float *buf = nullptr;
+    int rc = dev_alloc(&buf, 2 * nsl * P);
+    if (rc != PD_OK) return rc;
+    rc = ensure_sfd_workspace(p, (size_t)ps);
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    cudaStream_t st = nullptr;
+    cudaError_t e = cudaSuccess;
+    if (rc == PD_OK) {
+        e = cudaMemset(buf, 0x3c, nsl * P * sizeof(float));   // field = 0.0115 everywhere; the work does not depend on the data
+        if (e == cudaSuccess) e = cudaStreamSynchronize(nullptr);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+        for (int k = 0; k < 3 && e == cudaSuccess; ++k) e = cudaEventCreate(&ev[k]);
+    }
+    if (rc == PD_OK && e == cudaSuccess) {
+        const int it_res = 48, it_str = (int)(it_res * kHybridRhoDefault * ncl / ps + 0.5);
+        float *field = buf, *chi = buf + nsl * P;
+        for (int rep = 0; rep < 2 && rc == PD_OK && e == cudaSuccess; ++rep) {   // first repetition warms up
+            e = cudaEventRecord(ev[0], st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(p->aux, ev[0], 0);
+            if (e == cudaSuccess) e = launch_resident(p, field, nullptr, chi, it_res, 0.f, st, ncl, 2 * ncl);
+            if (e == cudaSuccess) e = cudaEventRecord(ev[1], st);
+            int launches = 0;
+            if (e == cudaSuccess) rc = solve_streaming_fd(p, field, nullptr, chi, it_str < 1 ? 1 : it_str, 0.f, p->aux, 2 * ncl, &launches, 2 * ps);
+            if (rc == PD_OK && e == cudaSuccess) e = cudaEventRecord(ev[2], p->aux);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(p->aux);
+        }
+        float t_res = 0.f, t_str = 0.f;
+        if (rc == PD_OK && e == cudaSuccess) e = cudaEventElapsedTime(&t_res, ev[0], ev[1]);
+        if (rc == PD_OK && e == cudaSuccess) e = cudaEventElapsedTime(&t_str, ev[0], ev[2]);
+        if (rc == PD_OK && e == cudaSuccess && t_res > 0.f && t_str > 0.f) {
+            const double rho = ((double)ps * (it_str < 1 ? 1 : it_str) / t_str) / ((double)ncl * it_res / t_res);
+            if (rho > 0.01 && rho < 1.0) p->hybrid_rho = rho;
+        }
+    }
+    for (int k = 0; k < 3; ++k) if (ev[k]) cudaEventDestroy(ev[k]);
+    if (st) cudaStreamDestroy(st);
+    cudaFree(buf);
+    if (rc != PD_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(e, "hybrid calibration");
+    return PD_OK;
+}
+
+int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                   cudaStream_t st) {
+    const int tail = hybrid_tail_pairs(p);
+    const int res_pairs = p->npairs - tail, res_batch = tail ? 2 * res_pairs : p->batch;
     p->ev_class->clear();
     if (p->timing) {
         while (p->ev->size() < 2) {
@@ -387,31 +474,7 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
         PD_CUDA(cudaEventRecord(p->ev_fork, st));
         PD_CUDA(cudaStreamWaitEvent(p->aux, p->ev_fork, 0));
     }
-    const bool w = p->weight != nullptr, aniso = p->tv_mode == PD_TV_ANISO;
-    const int nclusters = res_pairs < p->res_clusters ? res_pairs : p->res_clusters;
-    cudaError_t e;
-    if (!w && !p->no_fd) {
-        // W = identity: Fourier-domain dual, state in tensor memory and shared memory (pd_resident_tm.cuh)
-        ResidentTmArgs f;
-        std::memset(&f, 0, sizeof(f));
-        f.batch = a.batch; f.npairs = a.npairs; f.max_iters = a.max_iters; f.check_every = a.check_every;
-        f.alpha = a.alpha; f.sigma = a.sigma; f.tau = a.tau; f.theta = a.theta;
-        f.inv_one_plus_sigma = a.inv_one_plus_sigma; f.tol = a.tol;
-        f.field = field; f.mask = mask; f.mask_bstride = a.mask_bstride; f.chi_out = chi_out;
-        f.Z = a.Z; f.M2 = a.M2;
-        f.Dpriv = p->Dpriv; f.tw_tab = p->tw_row; f.part = p->rk_part;
-        f.iters_done = p->iters_done; f.relgap = p->relgap; f.relres = p->relres;
-        switch (p->nx) {
-            case 64: e = resident_tm_launch<64>(f, aniso, nclusters, st); break;
-            case 128: e = resident_tm_launch<128>(f, aniso, nclusters, st); break;
-            default: e = resident_tm_launch<256>(f, aniso, nclusters, st); break;
-        }
-    } else
-    switch (p->nx) {
-        case 64: e = resident_launch<64>(a, w, aniso, nclusters, st); break;
-        case 128: e = resident_launch<128>(a, w, aniso, nclusters, st); break;
-        default: e = resident_launch<256>(a, w, aniso, nclusters, st); break;
-    }
+    const cudaError_t e = launch_resident(p, field, mask, chi_out, max_iters, tol, st, res_pairs, res_batch);
     if (e != cudaSuccess) return cuda_fail(e, "resident kernel launch");
     int tail_launches = 0;
     if (tail) {   // the tail, then join
@@ -454,8 +517,8 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
 // Streaming variant, W = identity: two launches per iteration (pd_streaming_fd.cuh)
 // Slices [first, batch) of the plan (first even); field, mask and chi_out are the caller's whole-batch pointers.
 int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
-                       cudaStream_t st, int first, int *launches_out) {
-    const int nb = p->batch - first, np = (nb + 1) / 2;
+                       cudaStream_t st, int first, int *launches_out, int count) {
+    const int nb = count > 0 ? count : p->batch - first, np = (nb + 1) / 2;
     int rc = ensure_sfd_workspace(p, (size_t)np);
     if (rc != PD_OK) return rc;
     const size_t P = (size_t)p->nx * p->ny, PP = P * (size_t)np;
@@ -540,7 +603,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     {
         cudaError_t e = cudaGetDevice(&p->device);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
-        if (e != cudaSuccess) { delete p; return cuda_fail(e, "cudaGetDevice"); }
+        if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "cudaGetDevice"); }
     }
     const int rows_per_cta = (nx == 64 || nx == 128) ? 16 : 8;  // = SfdRowCfg<nx>::G
     p->nparts = ny / rows_per_cta;
@@ -605,6 +668,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
                 if (e3 == cudaSuccess) e3 = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
                 if (e3 == cudaSuccess) e3 = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
                 if (e3 != cudaSuccess) { pd_destroy(p); return cuda_fail(e3, "hybrid stream"); }
+                if ((rc = calibrate_hybrid(p)) != PD_OK) { pd_destroy(p); return rc; }
                 const int tail = hybrid_tail_pairs(p);
                 if (tail > 0 && (rc = ensure_sfd_workspace(p, (size_t)tail)) != PD_OK) { pd_destroy(p); return rc; }
             }
@@ -752,7 +816,13 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
     return PD_OK;
 }
 
-int pd_hybrid_tail_rule(int npairs, int clusters) { return hybrid_tail_rule(npairs, clusters); }
+int pd_hybrid_tail_rule(int npairs, int clusters, float rho) { return hybrid_tail_rule(npairs, clusters, (double)rho); }
+
+int pd_get_hybrid_rho(pd_plan_t p, float *rho) {
+    if (!p || !rho) return PD_EINVAL;
+    *rho = (float)p->hybrid_rho;
+    return PD_OK;
+}
 
 int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs) {
     if (!p || !tail_pairs) return PD_EINVAL;

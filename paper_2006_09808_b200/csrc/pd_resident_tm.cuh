@@ -101,10 +101,10 @@ struct TmRow {
 //   Z <- column FFT of conj(D/N^2 p^_{n+1})   (= conjugate of the inverse transform, finished by the row phase)
 // With want_gap: Sa += sum |dp(k) + conj dp(-k)|^2, Sb += sum |dp(k) - conj dp(-k)|^2, dp = p^_{n+1} - p^_n (the
 // mirror column's dp is in smg_mirror).
-template <int N, int NT, class Tw>
+template <int N, int NT, class Tw, class Sync>
 __device__ __forceinline__ void dual_tm_col(float2 *zc, const float *__restrict__ dpriv, const uint32_t tm_ph,
                                             const uint32_t tm_fh, const int j, float2 *smg, const float2 *smg_mirror,
-                                            const Tw &tw, const ResidentTmArgs &a, const bool first,
+                                            const Tw &tw, const Sync colsync, const ResidentTmArgs &a, const bool first,
                                             const bool want_gap, float &Sa, float &Sb) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, CH = 8;
     float2 v[E];
@@ -114,7 +114,7 @@ __device__ __forceinline__ void dual_tm_col(float2 *zc, const float *__restrict_
     if (!first) {
 #pragma unroll
         for (int m = 0; m < E; ++m) v[m] = ldcg2(zc + (j + T * m) * N);
-        fft_line<N, T>(v, smg, j, tw, BlockSync());
+        fft_line<N, T>(v, smg, j, tw, colsync);
     } else {
 #pragma unroll
         for (int m = 0; m < E; ++m) v[m] = make_float2(0.f, 0.f);
@@ -151,7 +151,7 @@ __device__ __forceinline__ void dual_tm_col(float2 *zc, const float *__restrict_
             Sb = fmaf(bx, bx, fmaf(by, by, Sb));
         }
     }
-    fft_line<N, T>(v, smg, j, tw, BlockSync());
+    fft_line<N, T>(v, smg, j, tw, colsync);
 #pragma unroll
     for (int m = 0; m < E; ++m) zc[(j + T * m) * N] = v[m];
     tm_st_wait();
@@ -370,6 +370,9 @@ resident_tm_kernel(const ResidentTmArgs a) {
     const float2 *smg_mir = self_mirror ? smg_col : exch + ((1 - cgi) * Cfg::COLS + cc) * Cfg::CS;
     TwiddlesSmem<N> tw_col;
     tw_col.w = tws + cj;
+    // the T threads of a column all sit in one column group (warps [cgi NT/64, (cgi+1) NT/64)): the two groups
+    // exchange through separate hardware barriers and drift apart (one in FFT arithmetic, the other in loads)
+    const NamedSync colsync{1 + cgi, NT / 2};
 
     const long long soff = (long long)cid * P;
     TmRow<N, NT> r;
@@ -476,7 +479,7 @@ resident_tm_kernel(const ResidentTmArgs a) {
 
             // (1) column phase: p^_{n+1} and the spectrum of K p_{n+1}
             float Sa = 0.f, Sb = 0.f;
-            dual_tm_col<N, NT>(zcol, dpriv, tm_ph, tm_fh, cj, smg_col, smg_mir, tw_col, a, n == 0, want_gap, Sa, Sb);
+            dual_tm_col<N, NT>(zcol, dpriv, tm_ph, tm_fh, cj, smg_col, smg_mir, tw_col, colsync, a, n == 0, want_gap, Sa, Sb);
             // (2) q-update from chibar_n (chibar_0 = 0 and q_0 = 0: nothing to do in the first iteration)
             float2 gap = zero;
             if (n > 0) q_update_tm<N, NT, ANISO>(r, a, j, want_gap, gap);

@@ -71,15 +71,16 @@ def test_hybrid_tail_rule_host_logic(libpath):
     run whole waves, the tail is what is left, and it never asks the streaming side for more than it can do in that time."""
     from paper_2006_09808_b200 import binding
     rule = binding.hybrid_tail_rule
-    assert rule(64, 15) == 4        # NS: 128 slices = 64 pairs = 4 full waves of 15 + 4
-    assert rule(512, 15) == 77      # C3: 29 waves + 77 (30 waves + 62 would take one wave longer)
-    assert rule(32, 15) == 2        # C2
-    assert rule(15, 15) == 0 and rule(30, 15) == 0 and rule(7, 15) == 0   # whole waves / less than one wave: no tail
-    assert rule(0, 15) == 0 and rule(10, 0) == 0
-    rho = 0.19
-    for ncl in (1, 7, 15, 18):
+    assert rule(64, 15, 0.19) == 4        # NS: 128 slices = 64 pairs = 4 full waves of 15 + 4
+    assert rule(512, 15, 0.19) == 77      # C3: 29 waves + 77 (30 waves + 62 would take one wave longer)
+    assert rule(512, 15, 0.15) == 62      # a slower streaming side gets a smaller tail
+    assert rule(32, 15, 0.19) == 2        # C2
+    assert rule(15, 15, 0.19) == 0 and rule(30, 15, 0.19) == 0 and rule(7, 15, 0.19) == 0   # whole waves / less than one wave: no tail
+    assert rule(0, 15, 0.19) == 0 and rule(10, 0, 0.19) == 0 and rule(64, 15, 0.0) == 0
+    for rho in (0.08, 0.15, 0.19, 0.3):
+      for ncl in (1, 7, 15, 18):
         for npairs in range(1, 400):
-            t = rule(npairs, ncl)
+            t = rule(npairs, ncl, rho)
             assert 0 <= t < npairs
             assert (npairs - t) % ncl == 0 or t == 0          # the resident part is whole waves whenever a tail is split off
             w = -(-(npairs - t) // ncl)

@@ -54,11 +54,18 @@ enum pd_option {
     PD_OPT_FOURIER_DUAL = 7, /* 1 (default): when W is the identity keep the dual variable p in the Fourier domain
                                 (one FFT round trip per iteration; same iterates up to rounding);
                                 0: always apply K twice per iteration, literally as PAPER.md:49 */
-    PD_OPT_HYBRID_TAIL = 8   /* 256x256, W = identity, PD_VARIANT_AUTO only: slice pairs (from the END of the batch) that
+    PD_OPT_HYBRID_TAIL = 8,  /* 256x256, W = identity, PD_VARIANT_AUTO only: slice pairs (from the END of the batch) that
                                 run through the streaming kernels on a plan-owned second stream, concurrently with the
                                 resident clusters, on the SMs those leave free (slices are independent).
                                 -1 (default): chosen from the batch size ; 0: off ; n > 0: exactly n pairs.
                                 pd_solve still returns with all work ordered on the caller's stream. */
+    PD_OPT_GRAPH_LOOP = 9    /* streaming variant: 1 (default): the whole solve is ONE CUDA graph launch -- init, a conditional
+                                WHILE node around the iteration kernels whose condition a loop-control kernel sets on the
+                                device (false once every slice has stopped or max_iters is reached), finish: nothing is
+                                launched for iterations nobody needs and the host is never asked.  The graph
+                                is cached in the plan and rebuilt when the arguments of pd_solve change.  0: one stream
+                                launch per kernel, 2*max_iters + 3 of them (the kernels of a stopped slice return at once).
+                                PD_OPT_KERNEL_TIMING = 1 always uses plain launches. */
 };
 /* kernel classes for pd_get_kernel_times.  Streaming variant: init, finish and, per iteration, fd_cols + fd_rows
  * (W = identity, Fourier-domain dual: two launches) or dipole_cols + dual_rows + dipole_cols + fd_rows (W set, or
@@ -130,7 +137,8 @@ int pd_get_stats_host(pd_plan_t p, int *iters_done_host, float *relgap_host, flo
  * in milliseconds (ms_host[PD_NUM_KERNEL_CLASSES]) and the number of launches (launches_host[...]); HOST pointers. */
 int pd_get_kernel_times(pd_plan_t p, float *ms_host, int *launches_host);
 
-/* Number of kernel launches pd_solve enqueued at its last call (for launch accounting in benchmarks). */
+/* Number of kernels of the last pd_solve (for launch accounting in benchmarks).  With the graphed loop the number is
+ * decided on the device: the call then waits for the device (cudaDeviceSynchronize) and reads the loop counter. */
 int pd_last_launch_count(pd_plan_t p);
 
 /* Which variant the next pd_solve of this plan runs, and its launch shape (HOST pointers, any may be NULL):

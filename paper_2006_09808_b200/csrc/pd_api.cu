@@ -67,6 +67,19 @@ struct pd_plan_s {
     int hybrid_tail;       // -1: automatic ; >= 0: slice pairs given to the streaming kernels
     double hybrid_rho;     // streaming pairs per resident pair and cluster, measured at plan time (calibrate_hybrid)
     cudaStream_t aux;
+    // graphed streaming loop (PD_OPT_GRAPH_LOOP, default on): init -> WHILE { iteration kernels, loop control } -> finish,
+    // one cached executable graph per use (slot 0: whole-batch streaming solve; slot 1: tail of the hybrid schedule)
+    int graph_loop;
+    cudaStream_t cap_stream;
+    struct GraphSlot {
+        cudaGraphExec_t exec;
+        cudaGraph_t graph;
+        StreamFdArgs key;     // the arguments the graph was built for
+        int key_valid;
+        int *iter;            // device iteration counter
+    } gslot[2];
+    int last_graph_slot;       // slot of the last solve's graph, -1 if it used plain launches
+    int graph_literal;         // the last graphed solve ran the literal (four-kernel) iteration
     cudaEvent_t ev_fork, ev_join;
     // host-buffer entry point staging
     float *h_field, *h_mask, *h_chi;
@@ -461,6 +474,7 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
                    cudaStream_t st) {
     const int tail = hybrid_tail_pairs(p);
     const int res_pairs = p->npairs - tail, res_batch = tail ? 2 * res_pairs : p->batch;
+    p->last_graph_slot = -1;
     p->ev_class->clear();
     if (p->timing) {
         while (p->ev->size() < 2) {
@@ -490,7 +504,7 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
         PD_CUDA(cudaEventRecord((*p->ev)[1], st));
         p->ev_class->push_back(PD_KERNEL_RESIDENT);
     }
-    p->last_launches = 1 + tail_launches;
+    p->last_launches = 1 + (tail_launches > 0 ? tail_launches : 0);
     return PD_OK;
 }
 
@@ -513,6 +527,81 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
         }                                                                                          \
         ++launches;                                                                                \
     } while (0)
+
+// The iteration kernels of one PD iteration (n < 0: inside the graphed loop, the kernels read the device counter)
+void sfd_enqueue_iteration(const pd_plan_s *p, const StreamFdArgs &a, bool literal, int n, cudaStream_t st) {
+    if (literal) {
+        if (n != 0) { PD_DISPATCH(p->ny, sfd_launch_cols_plain, a, n, 1, st); }   // K1 (chibar_0 = 0; in the loop the kernel skips n = 0 itself)
+        PD_DISPATCH(p->nx, sfd_launch_dual_rows, a, n, st);
+        PD_DISPATCH(p->ny, sfd_launch_cols_plain, a, n, 0, st);                    // K2
+    } else {
+        PD_DISPATCH(p->ny, sfd_launch_cols, a, n, st);
+    }
+    PD_DISPATCH(p->nx, sfd_launch_rows, a, n, st);
+}
+
+void graph_slot_release(pd_plan_s::GraphSlot &g) {
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    g.exec = nullptr; g.graph = nullptr; g.key_valid = 0;
+}
+
+// Build (or reuse) the executable graph of one streaming solve with arguments `a`:
+//   memset(iter) -> init_rows -> init_cols -> WHILE (handle) { iteration kernels ; sfd_loop_ctl } -> finish
+// The WHILE node's handle is set on the device by sfd_loop_ctl: when every slice has stopped (or n = max_iters) the
+// body is not launched again -- no no-op launches, no host round trip.
+int sfd_graph_prepare(pd_plan_s *p, int slot, const StreamFdArgs &a, bool literal) {
+    pd_plan_s::GraphSlot &g = p->gslot[slot];
+    if (g.key_valid && std::memcmp(&g.key, &a, sizeof(a)) == 0) return PD_OK;
+    graph_slot_release(g);
+    if (!p->cap_stream) PD_CUDA(cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+    cudaStream_t cs = p->cap_stream;
+    const size_t P = (size_t)p->nx * p->ny;
+    PD_CUDA(cudaGraphCreate(&g.graph, 0));
+    // prologue
+    PD_CUDA(cudaStreamBeginCaptureToGraph(cs, g.graph, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    cudaError_t e = cudaMemsetAsync(a.iter, 0, sizeof(int), cs);
+    PD_DISPATCH(p->nx, sfd_launch_init_rows, a, cs);
+    PD_DISPATCH(p->ny, sfd_launch_init_cols, a, cs);
+    cudaStreamCaptureStatus status;
+    const cudaGraphNode_t *deps = nullptr;
+    size_t ndeps = 0;
+    if (e == cudaSuccess) e = cudaStreamGetCaptureInfo_v2(cs, &status, nullptr, nullptr, &deps, &ndeps);
+    std::vector<cudaGraphNode_t> pro(deps, deps + (e == cudaSuccess ? ndeps : 0));
+    cudaGraph_t dummy = nullptr;
+    cudaError_t e2 = cudaStreamEndCapture(cs, &dummy);
+    if (e == cudaSuccess) e = e2;
+    if (e != cudaSuccess) { graph_slot_release(g); return cuda_fail(e, "graph capture (prologue)"); }
+    // WHILE node
+    cudaGraphConditionalHandle handle;
+    PD_CUDA(cudaGraphConditionalHandleCreate(&handle, g.graph, a.max_iters > 0 ? 1u : 0u, cudaGraphCondAssignDefault));
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = handle;
+    cp.conditional.type = cudaGraphCondTypeWhile;
+    cp.conditional.size = 1;
+    cudaGraphNode_t wnode;
+    PD_CUDA(cudaGraphAddNode(&wnode, g.graph, pro.data(), pro.size(), &cp));
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    PD_CUDA(cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    sfd_enqueue_iteration(p, a, literal, -1, cs);
+    pdk::sfd_loop_ctl_kernel<<<1, 256, 0, cs>>>(a, handle);
+    e = cudaStreamEndCapture(cs, &dummy);
+    if (e != cudaSuccess) { graph_slot_release(g); return cuda_fail(e, "graph capture (loop body)"); }
+    // epilogue
+    PD_CUDA(cudaStreamBeginCaptureToGraph(cs, g.graph, &wnode, nullptr, 1, cudaStreamCaptureModeRelaxed));
+    {
+        const int gx = (int)((P + 256 * 8 - 1) / (256 * 8));
+        pdk::sfd_finish_kernel<<<dim3(gx, a.npairs), 256, 0, cs>>>(a);
+    }
+    e = cudaStreamEndCapture(cs, &dummy);
+    if (e != cudaSuccess) { graph_slot_release(g); return cuda_fail(e, "graph capture (epilogue)"); }
+    e = cudaGraphInstantiate(&g.exec, g.graph, 0);
+    if (e != cudaSuccess) { graph_slot_release(g); return cuda_fail(e, "cudaGraphInstantiate"); }
+    g.key = a;
+    g.key_valid = 1;
+    return PD_OK;
+}
 
 // Streaming variant, W = identity: two launches per iteration (pd_streaming_fd.cuh)
 // Slices [first, batch) of the plan (first even); field, mask and chi_out are the caller's whole-batch pointers.
@@ -557,6 +646,19 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
 
     int launches = 0;
     if (!launches_out) p->ev_class->clear();
+    const int slot = first > 0 ? 1 : 0;
+    if (p->graph_loop && !p->timing && count == 0) {
+        // one graph launch: the loop over iterations and its termination live on the device
+        if (!p->gslot[slot].iter && (rc = dev_alloc(&p->gslot[slot].iter, 1)) != PD_OK) return rc;
+        a.iter = p->gslot[slot].iter;
+        if ((rc = sfd_graph_prepare(p, slot, a, literal)) != PD_OK) return rc;
+        PD_CUDA(cudaGraphLaunch(p->gslot[slot].exec, st));
+        if (launches_out) *launches_out = -1; else p->last_launches = 0;   // the graph's kernels are counted on demand (pd_last_launch_count)
+        p->last_graph_slot = slot;
+        p->graph_literal = literal ? 1 : 0;
+        return PD_OK;
+    }
+    if (!launches_out) p->last_graph_slot = -1;
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->nx, sfd_launch_init_rows, a, st));
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->ny, sfd_launch_init_cols, a, st));
     for (int n = 0; n < max_iters; ++n) {
@@ -600,6 +702,8 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     p->lambda_user = lambda; p->sigma_user = sigma; p->tau_user = tau; p->theta = theta;
     p->check_every = 1;
     p->hybrid_tail = -1;
+    p->graph_loop = 1;
+    p->last_graph_slot = -1;
     {
         cudaError_t e = cudaGetDevice(&p->device);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
@@ -734,6 +838,9 @@ int pd_set_option(pd_plan_t p, int key, int value) {
         case PD_OPT_HYBRID_TAIL:
             if (value < -1) return PD_EINVAL;
             p->hybrid_tail = value; return PD_OK;
+        case PD_OPT_GRAPH_LOOP:
+            if (value != 0 && value != 1) return PD_EINVAL;
+            p->graph_loop = value; return PD_OK;
         default: return PD_EINVAL;
     }
 }
@@ -805,7 +912,18 @@ int pd_get_kernel_times(pd_plan_t p, float *ms_host, int *launches_host) {
     return PD_OK;
 }
 
-int pd_last_launch_count(pd_plan_t p) { return p ? p->last_launches : PD_EINVAL; }
+int pd_last_launch_count(pd_plan_t p) {
+    if (!p) return PD_EINVAL;
+    int n = p->last_launches;
+    if (p->last_graph_slot >= 0) {   // kernels the graphed loop executed: decided on the device, so ask the device
+        int iters = 0;
+        if (cudaDeviceSynchronize() != cudaSuccess ||
+            cudaMemcpy(&iters, p->gslot[p->last_graph_slot].iter, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess)
+            return PD_ECUDA;
+        n += 3 + iters * (p->graph_literal ? 5 : 3);   // init rows + cols, finish ; per iteration its kernels + loop control
+    }
+    return n;
+}
 
 int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
     if (!p) return PD_EINVAL;
@@ -837,6 +955,12 @@ int pd_destroy(pd_plan_t p) {
                     p->sfd_planes, p->sfd_parts};
     for (void *q : ptrs)
         if (q) cudaFree(q);
+    for (int k = 0; k < 2; ++k) {
+        if (p->gslot[k].exec) cudaGraphExecDestroy(p->gslot[k].exec);
+        if (p->gslot[k].graph) cudaGraphDestroy(p->gslot[k].graph);
+        if (p->gslot[k].iter) cudaFree(p->gslot[k].iter);
+    }
+    if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     if (p->aux) cudaStreamDestroy(p->aux);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);

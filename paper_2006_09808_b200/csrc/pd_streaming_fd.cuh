@@ -54,6 +54,7 @@ struct StreamFdArgs {
     float *gap_row;                          // [npairs][nrowparts][2]
     float *res_part;                         // [npairs][nrowparts][4] (dn_a, cn_a, dn_b, cn_b)
     int ncolparts, nrowparts;
+    int *iter;                               // device iteration counter of the graphed loop (kernels launched with n < 0 read it)
 };
 
 template <int N> struct SfdRowCfg {
@@ -221,7 +222,9 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
 // `decide` is set for the first of the two column launches of an iteration.
 template <int NY, bool PLAIN>
 __global__ void __launch_bounds__(SfdColCfg<NY>::THREADS, SfdColCfg<NY>::THREADS <= 128 ? 4 : 2)
-sfd_cols_kernel(const StreamFdArgs a, const int n, const int do_decide) {
+sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
+    const int n = n_arg >= 0 ? n_arg : *a.iter;      // inside the graphed loop the iteration number lives on the device
+    if (PLAIN && do_decide && n == 0) return;        // literal path: chibar_0 = 0, the first K application of iteration 0 is skipped
     using Cfg = SfdColCfg<NY>;
     constexpr int E = Cfg::E, T = Cfg::T, NT = Cfg::THREADS;
     extern __shared__ __align__(16) unsigned char sfd_smem[];
@@ -412,7 +415,8 @@ __device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float 
 //   Z <- row FFT of chibar_{n+1}
 template <int NX, bool MASKED>
 __global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, SfdRowCfg<NX>::MINB)
-sfd_rows_kernel(const StreamFdArgs a, const int n) {
+sfd_rows_kernel(const StreamFdArgs a, const int n_arg) {
+    const int n = n_arg >= 0 ? n_arg : *a.iter;
     using Cfg = SfdRowCfg<NX>;
     constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
     __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
@@ -574,7 +578,8 @@ sfd_rows_kernel(const StreamFdArgs a, const int n) {
 // Same structure as sfd_rows: read-only double-buffered p, spectrum parked in the exchange region.
 template <int NX>
 __global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, 4)
-sfd_dual_rows_kernel(const StreamFdArgs a, const int n) {
+sfd_dual_rows_kernel(const StreamFdArgs a, const int n_arg) {
+    const int n = n_arg >= 0 ? n_arg : *a.iter;
     using Cfg = SfdRowCfg<NX>;
     constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
     __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
@@ -644,6 +649,24 @@ sfd_dual_rows_kernel(const StreamFdArgs a, const int n) {
             for (int q = 0; q < G; ++q) t += red[q][threadIdx.x];
             a.gap_col[n & 1][((long long)pair * a.ncolparts + blockIdx.x) * 2 + threadIdx.x] = t;
         }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ loop control
+// Last node of the graphed iteration body (one CTA): n <- n + 1, and the WHILE node runs the body again only if the
+// count allows it and some slice is still active -- the paper's per-slice "control of the calculation end points"
+// extended to the launch sequence itself: once every slice has stopped nothing is launched any more,
+// and the host is never asked.  The stop decision of iteration n-1 is taken inside the column kernel of
+// iteration n, so the loop runs one (empty) iteration past the last stop.
+__global__ void __launch_bounds__(256)
+sfd_loop_ctl_kernel(const StreamFdArgs a, const cudaGraphConditionalHandle handle) {
+    const int n = *a.iter + 1;
+    int active = 0;
+    for (int b = threadIdx.x; b < a.batch; b += 256) active |= (n < a.stop_iter[b]);
+    active = __syncthreads_or(active);
+    if (threadIdx.x == 0) {
+        *a.iter = n;
+        cudaGraphSetConditional(handle, (n < a.max_iters && active) ? 1u : 0u);
     }
 }
 

@@ -101,7 +101,7 @@ def test_streaming_fourier_domain_dual(torch, pd, oracle, ny, nx, iters):
     Same gates as the literal four-launch path (PD_OPT_FOURIER_DUAL = 0), and agreement with it."""
     case = synth.random_case(nx, ny, 5, seed=nx + 3 * ny + iters, with_mask=True)   # odd batch: ragged last pair
     g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, variant="streaming")
-    assert g["launches"] == 2 * iters + 3
+    assert g["launches"] == 3 * iters + 3          # graphed loop: init x2, per iteration cols + rows + loop control, finish
     o = oracle.solve(case["field"], case["mask"], lambda_=0.2, sigma=0.25, tau=0.25, max_iters=iters)
     assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
     assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-4)
@@ -109,9 +109,15 @@ def test_streaming_fourier_domain_dual(torch, pd, oracle, ny, nx, iters):
     assert np.all(g["iters_done"] == iters)
     lit = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, variant="streaming",
                     options=[(pd.OPT_FOURIER_DUAL, 0)])
-    assert lit["launches"] == 4 * iters + 2
+    assert lit["launches"] == 5 * iters + 3        # cols (returns at once in iteration 0), dual rows, cols, rows, loop control
     assert slice_rel(g["chi"], lit["chi"]).max() < TOL_1IT
     assert np.allclose(g["relgap"], lit["relgap"], rtol=1e-4)
+    # the same solves with one stream launch per kernel (PD_OPT_GRAPH_LOOP = 0): bit-identical results
+    for opts, count in (([(pd.OPT_GRAPH_LOOP, 0)], 2 * iters + 3), ([(pd.OPT_GRAPH_LOOP, 0), (pd.OPT_FOURIER_DUAL, 0)], 4 * iters + 2)):
+        h = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, variant="streaming", options=opts)
+        assert h["launches"] == count
+        ref = g if len(opts) == 1 else lit
+        assert np.array_equal(h["chi"], ref["chi"]) and np.array_equal(h["relgap"], ref["relgap"])
 
 
 @pytest.mark.parametrize("tail", [1, 2, 4])
@@ -122,7 +128,7 @@ def test_hybrid_schedule_tail_through_streaming(torch, pd, oracle, tail):
     iters = 4
     plan_opts = [(pd.OPT_HYBRID_TAIL, tail)]
     g = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, options=plan_opts)
-    assert g["launches"] == 1 + 2 * iters + 3
+    assert g["launches"] == 1 + 3 * iters + 3      # resident kernel + the graphed streaming loop of the tail
     o = oracle.solve(case["field"], case["mask"], lambda_=0.2, sigma=0.25, tau=0.25, max_iters=iters)
     assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
     assert np.allclose(g["relgap"], o["relgap"][:, iters - 1], rtol=1e-4)
@@ -236,6 +242,8 @@ def test_config4_full_tolerance_stop_sampled(torch, pd, oracle):
     d, g = _sampled_full_config(torch, pd, oracle, 4, [3, 200])
     assert g["iters_done"].min() > 40 and g["iters_done"].max() < 140
     assert np.all(g["relgap"] < 1e-4)
+    # the graphed loop stops launching one iteration after the last slice has stopped (not at max_iters = 500)
+    assert g["launches"] == 3 * (int(g["iters_done"].max()) + 1) + 3
 
 
 def test_options_aniso_dataconv_sharedmask_b0x_theta(torch, pd, oracle, variant):

@@ -109,9 +109,12 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir,
 int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
              int max_iters, float tol, void *cuda_stream);
 
-/* pd_solve_host: same computation with HOST buffers (pageable or pinned) -- flow steps (2) and (6) of the paper
- * done by the library: H2D of field (and mask if non-NULL), pd_solve, D2H of chi_out, on
- * cuda_stream, then synchronises that stream.  Staging buffers are plan-owned (allocated on first use). */
+/* pd_solve_host: same computation with HOST buffers (pinned for the copies to overlap; pageable works, serialised by
+ * the driver) -- flow steps (2) and (6) of the paper done by the library.  Slices are independent
+ * (PAPER.md:82), so a large batch is cut into a few contiguous chunks and pipelined on plan-owned copy streams:
+ * upload of chunk k+1 || solve of chunk k (on cuda_stream) || download of chunk k-1; small batches, a set weight and
+ * PD_OPT_KERNEL_TIMING use one chunk.  Returns after synchronising cuda_stream, with chi_out_host complete.
+ * Staging buffers, streams and events are plan-owned (allocated on first use). */
 int pd_solve_host(pd_plan_t p, const float *field_host, const float *mask_host, float *chi_out_host,
                   int max_iters, float tol, void *cuda_stream);
 

@@ -36,6 +36,8 @@ constexpr double kNormBound = 4.0 / 9.0 + 8.0;  // ||K_full||^2 <= max|D|^2 + ||
 
 }  // namespace
 
+constexpr int kGraphSlots = 8, kMaxChunks = 6;
+
 struct pd_plan_s {
     int nx, ny, batch, npairs, b0_dir;
     // user-facing parameters (as given) and the effective ones of the rescaled problem (R2)
@@ -76,10 +78,14 @@ struct pd_plan_s {
         cudaGraph_t graph;
         StreamFdArgs key;     // the arguments the graph was built for
         int key_valid;
+        int literal;          // built for the literal (four-kernel) iteration
         int *iter;            // device iteration counter
-    } gslot[2];
-    int last_graph_slot;       // slot of the last solve's graph, -1 if it used plain launches
-    int graph_literal;         // the last graphed solve ran the literal (four-kernel) iteration
+    } gslot[kGraphSlots];      // executable graphs cached by their arguments (whole batch, hybrid tail, chunks of pd_solve_host)
+    int gslot_next;            // round-robin replacement
+    unsigned graph_used;       // bit k: slot k was launched by the last pd_solve / pd_solve_host
+    // pd_solve_host pipeline: copies on their own streams, one event pair per chunk
+    cudaStream_t h2d_stream, d2h_stream;
+    cudaEvent_t ev_chunk[2 * kMaxChunks + 2];
     cudaEvent_t ev_fork, ev_join;
     // host-buffer entry point staging
     float *h_field, *h_mask, *h_chi;
@@ -363,17 +369,19 @@ int hybrid_tail_rule(int npairs, int ncl, double rho) {
 bool hybrid_possible(const pd_plan_s *p) {
     return p->nx == 256 && p->aux && p->res_max_clusters * 8 + 16 <= p->num_sms;   // SMs left over beside the clusters
 }
-int hybrid_tail_pairs(const pd_plan_s *p) {
+// tail of a solve over `npairs` slice pairs (the whole batch, or one chunk of pd_solve_host: `whole` false)
+int hybrid_tail_pairs(const pd_plan_s *p, int npairs, bool whole) {
     if (p->nx != 256 || p->weight || p->no_fd || p->variant != PD_VARIANT_AUTO || !p->aux) return 0;
-    if (p->hybrid_tail >= 0) return p->hybrid_tail < p->npairs ? p->hybrid_tail : p->npairs - 1;
-    if (!hybrid_possible(p)) return 0;
-    return hybrid_tail_rule(p->npairs, p->res_max_clusters, p->hybrid_rho);
+    if (p->hybrid_tail >= 0 && whole) return p->hybrid_tail < npairs ? p->hybrid_tail : npairs - 1;
+    if (p->hybrid_tail == 0 || !hybrid_possible(p)) return 0;
+    return hybrid_tail_rule(npairs, p->res_max_clusters, p->hybrid_rho);
 }
+int hybrid_tail_pairs(const pd_plan_s *p) { return hybrid_tail_pairs(p, p->npairs, true); }
 
-// The resident kernel over the first res_pairs slice pairs (res_batch slices) of the caller's arrays
+// The resident kernel over res_pairs slice pairs (res_batch slices) starting at slice `first` of the caller's arrays
 cudaError_t launch_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
-                            cudaStream_t st, int res_pairs, int res_batch) {
-    const size_t P = (size_t)p->nx * p->ny;
+                            cudaStream_t st, int res_pairs, int res_batch, int first = 0) {
+    const size_t P = (size_t)p->nx * p->ny, off = (size_t)first * P;
     ResidentArgs a;
     std::memset(&a, 0, sizeof(a));
     a.batch = res_batch; a.npairs = res_pairs; a.max_iters = max_iters; a.check_every = p->check_every;
@@ -381,16 +389,17 @@ cudaError_t launch_resident(pd_plan_s *p, const float *field, const float *mask,
     a.theta = p->theta;
     a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
     a.tol = tol;
-    a.field = field; a.mask = mask; a.weight = p->weight;
     a.mask_bstride = p->mask_shared ? 0 : (long long)P;
-    a.chi_out = chi_out;
+    a.field = field + off; a.mask = mask ? mask + (size_t)first * (size_t)a.mask_bstride : nullptr;
+    a.weight = p->weight ? p->weight + off : nullptr;
+    a.chi_out = chi_out + off;
     const size_t stride = (size_t)p->res_clusters * P;
     float2 *base = p->res_scratch;
     a.Z = base; a.qy = base + stride; a.chi = base + 2 * stride; a.chibar = base + 3 * stride;
     a.phi2 = base + 4 * stride; a.M2 = base + 5 * stride; a.W2 = base + 6 * stride;
     a.Dtab = p->Dtab; a.tw_tab = p->tw_row;
     a.part = p->rk_part;
-    a.iters_done = p->iters_done; a.relgap = p->relgap; a.relres = p->relres;
+    a.iters_done = p->iters_done + first; a.relgap = p->relgap + first; a.relres = p->relres + first;
     const bool w = p->weight != nullptr, aniso = p->tv_mode == PD_TV_ANISO;
     const int nclusters = res_pairs < p->res_clusters ? res_pairs : p->res_clusters;
     if (!w && !p->no_fd) {
@@ -400,10 +409,10 @@ cudaError_t launch_resident(pd_plan_s *p, const float *field, const float *mask,
         f.batch = a.batch; f.npairs = a.npairs; f.max_iters = a.max_iters; f.check_every = a.check_every;
         f.alpha = a.alpha; f.sigma = a.sigma; f.tau = a.tau; f.theta = a.theta;
         f.inv_one_plus_sigma = a.inv_one_plus_sigma; f.tol = a.tol;
-        f.field = field; f.mask = mask; f.mask_bstride = a.mask_bstride; f.chi_out = chi_out;
+        f.field = a.field; f.mask = a.mask; f.mask_bstride = a.mask_bstride; f.chi_out = a.chi_out;
         f.Z = a.Z; f.M2 = a.M2;
         f.Dpriv = p->Dpriv; f.tw_tab = p->tw_row; f.part = p->rk_part;
-        f.iters_done = p->iters_done; f.relgap = p->relgap; f.relres = p->relres;
+        f.iters_done = a.iters_done; f.relgap = a.relgap; f.relres = a.relres;
         switch (p->nx) {
             case 64: return resident_tm_launch<64>(f, aniso, nclusters, st);
             case 128: return resident_tm_launch<128>(f, aniso, nclusters, st);
@@ -441,6 +450,8 @@ int calibrate_hybrid(pd_plan_s *p) {
         for (int k = 0; k < 3 && e == cudaSuccess; ++k) e = cudaEventCreate(&ev[k]);
     }
     if (rc == PD_OK && e == cudaSuccess) {
+        const int graph_loop = p->graph_loop;
+        p->graph_loop = 0;
         const int it_res = 48, it_str = (int)(it_res * kHybridRhoDefault * ncl / ps + 0.5);
         float *field = buf, *chi = buf + nsl * P;
         for (int rep = 0; rep < 2 && rc == PD_OK && e == cudaSuccess; ++rep) {   // first repetition warms up
@@ -454,6 +465,7 @@ int calibrate_hybrid(pd_plan_s *p) {
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(p->aux);
         }
+        p->graph_loop = graph_loop;
         float t_res = 0.f, t_str = 0.f;
         if (rc == PD_OK && e == cudaSuccess) e = cudaEventElapsedTime(&t_res, ev[0], ev[1]);
         if (rc == PD_OK && e == cudaSuccess) e = cudaEventElapsedTime(&t_str, ev[0], ev[2]);
@@ -470,13 +482,16 @@ int calibrate_hybrid(pd_plan_s *p) {
     return PD_OK;
 }
 
+// Slices [first, first + count) of the plan through the resident kernel (count = 0: to the end of the batch), with the
+// hybrid schedule's streaming tail where it applies.  field, mask and chi_out are the caller's whole-batch pointers.
 int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
-                   cudaStream_t st) {
-    const int tail = hybrid_tail_pairs(p);
-    const int res_pairs = p->npairs - tail, res_batch = tail ? 2 * res_pairs : p->batch;
-    p->last_graph_slot = -1;
-    p->ev_class->clear();
-    if (p->timing) {
+                   cudaStream_t st, int first = 0, int count = 0) {
+    const bool whole = (first == 0 && count == 0);
+    const int nb = count > 0 ? count : p->batch - first, np = (nb + 1) / 2;
+    const int tail = hybrid_tail_pairs(p, np, whole);
+    const int res_pairs = np - tail, res_batch = tail ? 2 * res_pairs : nb;
+    if (whole) p->ev_class->clear();
+    if (p->timing && whole) {
         while (p->ev->size() < 2) {
             cudaEvent_t evn_;
             PD_CUDA(cudaEventCreate(&evn_));
@@ -488,24 +503,34 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
         PD_CUDA(cudaEventRecord(p->ev_fork, st));
         PD_CUDA(cudaStreamWaitEvent(p->aux, p->ev_fork, 0));
     }
-    const cudaError_t e = launch_resident(p, field, mask, chi_out, max_iters, tol, st, res_pairs, res_batch);
+    const cudaError_t e = launch_resident(p, field, mask, chi_out, max_iters, tol, st, res_pairs, res_batch, first);
     if (e != cudaSuccess) return cuda_fail(e, "resident kernel launch");
     int tail_launches = 0;
     if (tail) {   // the tail, then join
         const int timing = p->timing;
         p->timing = 0;   // the class-5 bracket below covers the whole hybrid step
-        const int rc = solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, p->aux, 2 * res_pairs, &tail_launches);
+        const int rc = solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, p->aux, first + 2 * res_pairs, &tail_launches,
+                                          nb - 2 * res_pairs);
         p->timing = timing;
         if (rc != PD_OK) return rc;
         PD_CUDA(cudaEventRecord(p->ev_join, p->aux));
         PD_CUDA(cudaStreamWaitEvent(st, p->ev_join, 0));
     }
-    if (p->timing) {
+    if (p->timing && whole) {
         PD_CUDA(cudaEventRecord((*p->ev)[1], st));
         p->ev_class->push_back(PD_KERNEL_RESIDENT);
     }
-    p->last_launches = 1 + (tail_launches > 0 ? tail_launches : 0);
+    p->last_launches += 1 + tail_launches;
     return PD_OK;
+}
+
+int solve_range(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                cudaStream_t st, int first, int count) {
+    if (p->res_ok && p->variant != PD_VARIANT_STREAMING) return solve_resident(p, field, mask, chi_out, max_iters, tol, st, first, count);
+    int launches = 0;
+    const int rc = solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, st, first, &launches, count);
+    p->last_launches += launches;
+    return rc;
 }
 
 
@@ -550,10 +575,24 @@ void graph_slot_release(pd_plan_s::GraphSlot &g) {
 //   memset(iter) -> init_rows -> init_cols -> WHILE (handle) { iteration kernels ; sfd_loop_ctl } -> finish
 // The WHILE node's handle is set on the device by sfd_loop_ctl: when every slice has stopped (or n = max_iters) the
 // body is not launched again -- no no-op launches, no host round trip.
-int sfd_graph_prepare(pd_plan_s *p, int slot, const StreamFdArgs &a, bool literal) {
+int sfd_graph_prepare(pd_plan_s *p, StreamFdArgs &a, bool literal, int *slot_out) {
+    // the iteration counter belongs to the slot: look the arguments up with each slot's own counter in place
+    for (int k = 0; k < kGraphSlots; ++k) {
+        pd_plan_s::GraphSlot &c = p->gslot[k];
+        a.iter = c.iter;
+        if (c.key_valid && c.literal == (literal ? 1 : 0) && std::memcmp(&c.key, &a, sizeof(a)) == 0) { *slot_out = k; return PD_OK; }
+    }
+    const int slot = p->gslot_next;
+    p->gslot_next = (p->gslot_next + 1) % kGraphSlots;
+    *slot_out = slot;
     pd_plan_s::GraphSlot &g = p->gslot[slot];
-    if (g.key_valid && std::memcmp(&g.key, &a, sizeof(a)) == 0) return PD_OK;
+    if (g.exec) PD_CUDA(cudaDeviceSynchronize());   // a graph being replaced may still be running (chunks of an earlier call)
     graph_slot_release(g);
+    if (!g.iter) {
+        const int rc_ = dev_alloc(&g.iter, 1);
+        if (rc_ != PD_OK) return rc_;
+    }
+    a.iter = g.iter;
     if (!p->cap_stream) PD_CUDA(cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
     cudaStream_t cs = p->cap_stream;
     const size_t P = (size_t)p->nx * p->ny;
@@ -600,6 +639,7 @@ int sfd_graph_prepare(pd_plan_s *p, int slot, const StreamFdArgs &a, bool litera
     if (e != cudaSuccess) { graph_slot_release(g); return cuda_fail(e, "cudaGraphInstantiate"); }
     g.key = a;
     g.key_valid = 1;
+    g.literal = literal ? 1 : 0;
     return PD_OK;
 }
 
@@ -646,19 +686,15 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
 
     int launches = 0;
     if (!launches_out) p->ev_class->clear();
-    const int slot = first > 0 ? 1 : 0;
-    if (p->graph_loop && !p->timing && count == 0) {
+    if (p->graph_loop && !p->timing) {
         // one graph launch: the loop over iterations and its termination live on the device
-        if (!p->gslot[slot].iter && (rc = dev_alloc(&p->gslot[slot].iter, 1)) != PD_OK) return rc;
-        a.iter = p->gslot[slot].iter;
-        if ((rc = sfd_graph_prepare(p, slot, a, literal)) != PD_OK) return rc;
+        int slot = 0;
+        if ((rc = sfd_graph_prepare(p, a, literal, &slot)) != PD_OK) return rc;
         PD_CUDA(cudaGraphLaunch(p->gslot[slot].exec, st));
-        if (launches_out) *launches_out = -1; else p->last_launches = 0;   // the graph's kernels are counted on demand (pd_last_launch_count)
-        p->last_graph_slot = slot;
-        p->graph_literal = literal ? 1 : 0;
+        p->graph_used |= 1u << slot;   // its kernels are counted on demand (pd_last_launch_count)
+        if (launches_out) *launches_out = 0; else p->last_launches = 0;
         return PD_OK;
     }
-    if (!launches_out) p->last_graph_slot = -1;
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->nx, sfd_launch_init_rows, a, st));
     PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->ny, sfd_launch_init_cols, a, st));
     for (int n = 0; n < max_iters; ++n) {
@@ -703,7 +739,6 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     p->check_every = 1;
     p->hybrid_tail = -1;
     p->graph_loop = 1;
-    p->last_graph_slot = -1;
     {
         cudaError_t e = cudaGetDevice(&p->device);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
@@ -850,25 +885,107 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
     if (!p || !field || !chi_out || max_iters < 0) return PD_EINVAL;
     if (p->lambda_conv == PD_LAMBDA_DATA && !(p->lambda_user > 0.f)) return PD_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    p->last_launches = 0;
+    p->graph_used = 0u;
     if (p->res_ok && p->variant != PD_VARIANT_STREAMING) return solve_resident(p, field, mask, chi_out, max_iters, tol, st);
     return solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, st);
+}
+
+// Chunks of pd_solve_host, in slices (even counts, the last takes the rest).  Slices are independent, so
+// the batch is cut into a short first chunk (its upload is the only one nobody hides), a long middle and short last
+// chunks (the download of the very last one is the only one nobody hides): H2D(k+1) || solve(k) || D2H(k-1).
+// Resident variant: the unit is one wave of clusters (no chunk leaves clusters idle) and a solve costs about ten times
+// its upload, so the chunks grow 1, 4, rest and shrink 4, 2.  Streaming variant: a small chunk cannot fill the GPU with
+// its launches, so three chunks of 1/8, 6/8, 1/8 of the batch (measured on C4: five chunks lose more than they hide).
+int host_chunks(const pd_plan_s *p, int *count /*[kMaxChunks]*/) {
+    const bool res = p->res_ok && p->variant != PD_VARIANT_STREAMING;
+    int unit = res ? p->res_max_clusters : (p->npairs + 7) / 8;   // pairs
+    if (unit < 1) unit = 1;
+    const int np = p->npairs;
+    int n = 0, left = np;
+    if (res && np >= 24 * unit) {     // 1, 4, middle, 4, 2 units
+        const int head[2] = {unit, 4 * unit}, tail[2] = {4 * unit, 2 * unit};
+        count[n++] = 2 * head[0]; count[n++] = 2 * head[1];
+        count[n++] = 2 * (np - head[0] - head[1] - tail[0] - tail[1]);
+        count[n++] = 2 * tail[0]; count[n++] = 2 * tail[1];
+        left = 0;
+    } else if (np >= 6 * unit) {      // 1, middle, 1 units
+        count[n++] = 2 * unit; count[n++] = 2 * (np - 2 * unit); count[n++] = 2 * unit;
+        left = 0;
+    }
+    if (left) count[n++] = 2 * left;
+    int used = 0;
+    for (int k = 0; k < n; ++k) used += count[k];
+    count[n - 1] -= used - p->batch;   // an odd batch: the last pair is half empty
+    return n;
 }
 
 int pd_solve_host(pd_plan_t p, const float *field_host, const float *mask_host, float *chi_out_host, int max_iters,
                   float tol, void *cuda_stream) {
     if (!p || !field_host || !chi_out_host || max_iters < 0) return PD_EINVAL;
+    if (p->lambda_conv == PD_LAMBDA_DATA && !(p->lambda_user > 0.f)) return PD_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t P = (size_t)p->nx * p->ny, BP = P * (size_t)p->batch;
-    const size_t mask_count = p->mask_shared ? P : BP;
     int rc;
     if (!p->h_field && (rc = dev_alloc(&p->h_field, BP)) != PD_OK) return rc;
     if (!p->h_chi && (rc = dev_alloc(&p->h_chi, BP)) != PD_OK) return rc;
-    if (mask_host && !p->h_mask && (rc = dev_alloc(&p->h_mask, BP)) != PD_OK) return rc;
-    PD_CUDA(cudaMemcpyAsync(p->h_field, field_host, BP * sizeof(float), cudaMemcpyHostToDevice, st));
-    if (mask_host) PD_CUDA(cudaMemcpyAsync(p->h_mask, mask_host, mask_count * sizeof(float), cudaMemcpyHostToDevice, st));
-    rc = pd_solve(p, p->h_field, mask_host ? p->h_mask : nullptr, p->h_chi, max_iters, tol, cuda_stream);
-    if (rc != PD_OK) return rc;
-    PD_CUDA(cudaMemcpyAsync(chi_out_host, p->h_chi, BP * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (mask_host && !p->h_mask && (rc = dev_alloc(&p->h_mask, p->mask_shared ? P : BP)) != PD_OK) return rc;
+    if (!p->h2d_stream) {
+        PD_CUDA(cudaStreamCreateWithFlags(&p->h2d_stream, cudaStreamNonBlocking));
+        PD_CUDA(cudaStreamCreateWithFlags(&p->d2h_stream, cudaStreamNonBlocking));
+        for (cudaEvent_t &ev : p->ev_chunk) PD_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    }
+    int count[kMaxChunks];
+    const int nchunks = (p->timing || p->weight) ? 1 : host_chunks(p, count);
+    if (nchunks == 1) count[0] = p->batch;
+    {   // workspaces the chunks need must exist before anything is in flight (an allocation synchronises and may free)
+        size_t need = 0;
+        for (int k = 0; k < nchunks; ++k) {
+            const int np = (count[k] + 1) / 2;
+            const bool res = p->res_ok && p->variant != PD_VARIANT_STREAMING;
+            const size_t t = res ? (size_t)hybrid_tail_pairs(p, np, nchunks == 1) : (size_t)np;
+            need = t > need ? t : need;
+        }
+        if (need && (rc = ensure_sfd_workspace(p, need)) != PD_OK) return rc;
+    }
+    p->last_launches = 0;
+    p->graph_used = 0u;
+    cudaEvent_t *ev_up = p->ev_chunk, *ev_done = p->ev_chunk + kMaxChunks, ev_start = p->ev_chunk[2 * kMaxChunks],
+                ev_end = p->ev_chunk[2 * kMaxChunks + 1];
+    // the copies start when the caller's stream reaches this call
+    PD_CUDA(cudaEventRecord(ev_start, st));
+    PD_CUDA(cudaStreamWaitEvent(p->h2d_stream, ev_start, 0));
+    PD_CUDA(cudaStreamWaitEvent(p->d2h_stream, ev_start, 0));
+    if (mask_host && p->mask_shared)
+        PD_CUDA(cudaMemcpyAsync(p->h_mask, mask_host, P * sizeof(float), cudaMemcpyHostToDevice, p->h2d_stream));
+    int first = 0;
+    for (int k = 0; k < nchunks; ++k) {          // flow step (2) of the paper, chunk by chunk
+        const size_t off = (size_t)first * P, nby = (size_t)count[k] * P * sizeof(float);
+        PD_CUDA(cudaMemcpyAsync(p->h_field + off, field_host + off, nby, cudaMemcpyHostToDevice, p->h2d_stream));
+        if (mask_host && !p->mask_shared)
+            PD_CUDA(cudaMemcpyAsync(p->h_mask + off, mask_host + off, nby, cudaMemcpyHostToDevice, p->h2d_stream));
+        PD_CUDA(cudaEventRecord(ev_up[k], p->h2d_stream));
+        first += count[k];
+    }
+    first = 0;
+    for (int k = 0; k < nchunks; ++k) {
+        const size_t off = (size_t)first * P, nby = (size_t)count[k] * P * sizeof(float);
+        PD_CUDA(cudaStreamWaitEvent(st, ev_up[k], 0));
+        if (nchunks == 1) {
+            rc = (p->res_ok && p->variant != PD_VARIANT_STREAMING)
+                     ? solve_resident(p, p->h_field, mask_host ? p->h_mask : nullptr, p->h_chi, max_iters, tol, st)
+                     : solve_streaming_fd(p, p->h_field, mask_host ? p->h_mask : nullptr, p->h_chi, max_iters, tol, st);
+        } else {
+            rc = solve_range(p, p->h_field, mask_host ? p->h_mask : nullptr, p->h_chi, max_iters, tol, st, first, count[k]);
+        }
+        if (rc != PD_OK) return rc;
+        PD_CUDA(cudaEventRecord(ev_done[k], st));
+        PD_CUDA(cudaStreamWaitEvent(p->d2h_stream, ev_done[k], 0));   // flow step (6), chunk by chunk
+        PD_CUDA(cudaMemcpyAsync(chi_out_host + off, p->h_chi + off, nby, cudaMemcpyDeviceToHost, p->d2h_stream));
+        first += count[k];
+    }
+    PD_CUDA(cudaEventRecord(ev_end, p->d2h_stream));
+    PD_CUDA(cudaStreamWaitEvent(st, ev_end, 0));
     PD_CUDA(cudaStreamSynchronize(st));
     return PD_OK;
 }
@@ -915,12 +1032,14 @@ int pd_get_kernel_times(pd_plan_t p, float *ms_host, int *launches_host) {
 int pd_last_launch_count(pd_plan_t p) {
     if (!p) return PD_EINVAL;
     int n = p->last_launches;
-    if (p->last_graph_slot >= 0) {   // kernels the graphed loop executed: decided on the device, so ask the device
-        int iters = 0;
-        if (cudaDeviceSynchronize() != cudaSuccess ||
-            cudaMemcpy(&iters, p->gslot[p->last_graph_slot].iter, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess)
-            return PD_ECUDA;
-        n += 3 + iters * (p->graph_literal ? 5 : 3);   // init rows + cols, finish ; per iteration its kernels + loop control
+    if (p->graph_used) {   // kernels the graphed loops executed: decided on the device, so ask the device
+        if (cudaDeviceSynchronize() != cudaSuccess) return PD_ECUDA;
+        for (int k = 0; k < kGraphSlots; ++k) {
+            if (!(p->graph_used & (1u << k))) continue;
+            int iters = 0;
+            if (cudaMemcpy(&iters, p->gslot[k].iter, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return PD_ECUDA;
+            n += 3 + iters * (p->gslot[k].literal ? 5 : 3);   // init rows + cols, finish ; per iteration its kernels + loop control
+        }
     }
     return n;
 }
@@ -955,12 +1074,15 @@ int pd_destroy(pd_plan_t p) {
                     p->sfd_planes, p->sfd_parts};
     for (void *q : ptrs)
         if (q) cudaFree(q);
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < kGraphSlots; ++k) {
         if (p->gslot[k].exec) cudaGraphExecDestroy(p->gslot[k].exec);
         if (p->gslot[k].graph) cudaGraphDestroy(p->gslot[k].graph);
         if (p->gslot[k].iter) cudaFree(p->gslot[k].iter);
     }
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
+    if (p->h2d_stream) cudaStreamDestroy(p->h2d_stream);
+    if (p->d2h_stream) cudaStreamDestroy(p->d2h_stream);
+    for (cudaEvent_t ev : p->ev_chunk) if (ev) cudaEventDestroy(ev);
     if (p->aux) cudaStreamDestroy(p->aux);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);

@@ -246,6 +246,26 @@ def test_config4_full_tolerance_stop_sampled(torch, pd, oracle):
     assert g["launches"] == 3 * (int(g["iters_done"].max()) + 1) + 3
 
 
+@pytest.mark.parametrize("ny,nx,batch,variant_", [(64, 64, 901, "auto"), (64, 128, 51, "streaming"), (256, 256, 61, "auto")])
+def test_host_entry_pipeline_chunks(torch, pd, oracle, ny, nx, batch, variant_):
+    """pd_solve_host cuts a large batch into chunks (upload k+1 || solve k || download k-1 on plan-owned streams): same
+    chi and statistics as pd_solve on device buffers -- bit for bit where every slice runs through the same kernels
+    (64x64: five chunks of resident waves; 64x128: five chunks of graphed streaming loops, odd batch), within the
+    one-iteration gate where the hybrid tail may land elsewhere (256x256) -- and as the oracle on sampled slices."""
+    case = synth.random_case(nx, ny, batch, seed=batch + nx, with_mask=True)
+    iters, tol = (12, 0.0) if variant_ == "auto" else (40, 5e-2)
+    dev = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, tol=tol, variant=variant_)
+    host = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, tol=tol, variant=variant_, host=True)
+    assert np.array_equal(host["iters_done"], dev["iters_done"])
+    if nx == 256:
+        assert slice_rel(host["chi"], dev["chi"]).max() < TOL_1IT
+    else:
+        assert np.array_equal(host["chi"], dev["chi"]) and np.array_equal(host["relgap"], dev["relgap"])
+    for b in (0, batch // 2, batch - 1):
+        o = oracle.solve(case["field"][b], case["mask"][b], lambda_=0.2, sigma=0.25, tau=0.25, max_iters=int(host["iters_done"][b]))
+        assert slice_rel(host["chi"][b:b + 1], o["chi"]).max() < TOL_1IT
+
+
 def test_options_aniso_dataconv_sharedmask_b0x_theta(torch, pd, oracle, variant):
     case = synth.random_case(64, 128, 2, seed=5, with_mask=True)
     f, m = case["field"], case["mask"]

@@ -105,13 +105,15 @@ inline int signed_index(int i, int n) { return (i < (n + 1) / 2) ? i : i - n; }
 /* Dipole kernel in the in-plane form fixed by BASELINE.json north_star:
  * D(kx,ky) = 1/3 - k_b^2/(kx^2+ky^2), D(0,0) = 0, kx = fi/nx, ky = fj/ny cycles per pixel. */
 template <class T>
-void dipole_table(int nx, int ny, int b0_dir, T *D) {
+void dipole_table(int nx, int ny, int b0_dir, T *D, double b0_angle = 0.0) {
+    /* PDO_B0_ANGLE: B0 along the in-plane unit vector (cos a, sin a); a = 0 is PDO_B0_X, a = pi/2 is PDO_B0_Y */
+    const double bx = std::cos(b0_angle), by = std::sin(b0_angle);
     for (int j = 0; j < ny; ++j) {
         for (int i = 0; i < nx; ++i) {
             const double kx = (double)signed_index(i, nx) / (double)nx;
             const double ky = (double)signed_index(j, ny) / (double)ny;
             const double k2 = kx * kx + ky * ky;
-            const double kb = (b0_dir == PDO_B0_Y) ? ky : kx;
+            const double kb = (b0_dir == PDO_B0_ANGLE) ? kx * bx + ky * by : (b0_dir == PDO_B0_Y) ? ky : kx;
             D[(std::ptrdiff_t)j * nx + i] = (i == 0 && j == 0) ? (T)0 : (T)(1.0 / 3.0 - kb * kb / k2);
         }
     }
@@ -186,6 +188,15 @@ void prox_q(std::ptrdiff_t n, T *tx, T *ty, T radius, int tv_mode) {
     }
 }
 
+/* Soft shrinkage: the prox of t*|.| (PDO_REG_L1; BASELINE.json north_star "or shrinkage"). */
+template <class T>
+void shrink(std::ptrdiff_t n, T *v, const T *t) {
+    for (std::ptrdiff_t i = 0; i < n; ++i) {
+        const T a = std::fabs(v[i]) - t[i];
+        v[i] = (a > 0) ? (v[i] > 0 ? a : -a) : (T)0;
+    }
+}
+
 /* One slice of the PD iteration, steps in the paper's order. */
 template <class T>
 struct SliceSolver {
@@ -196,7 +207,8 @@ struct SliceSolver {
     std::vector<T> u, r, gx, gy, wp, v, mqx, mqy, d, chinew;
     std::vector<Cpx<T>> work;
     T sigma, tau, theta, lambda;
-    int tv_mode, lambda_conv;
+    int tv_mode, lambda_conv, regulariser;
+    std::vector<T> thr;   /* PDO_REG_L1: shrinkage threshold tau * radius * M per pixel */
     T radius;   /* ball of the q-projection: lambda (REG) or 1 (DATA) */
     double P0;  /* normaliser of relgap: primal objective at chi = 0 */
 
@@ -210,9 +222,10 @@ struct SliceSolver {
         lambda = (T)prm.lambda;
         tv_mode = prm.tv_mode;
         lambda_conv = prm.lambda_conv;
+        regulariser = prm.regulariser;
         radius = (lambda_conv == PDO_LAMBDA_DATA) ? (T)1 : lambda;
         D.resize(P);
-        dipole_table(nx, ny, prm.b0_dir, D.data());
+        dipole_table(nx, ny, prm.b0_dir, D.data(), prm.b0_angle);
         phi.resize(P);
         M.resize(P);
         W.resize(P);
@@ -234,10 +247,50 @@ struct SliceSolver {
             s += wphi * wphi;
         }
         P0 = 0.5 * s * ((lambda_conv == PDO_LAMBDA_DATA) ? (double)lambda : 1.0);
+        thr.resize(P);
+        for (std::ptrdiff_t i = 0; i < P; ++i) thr[i] = tau * radius * M[i];
+    }
+
+    /* PDO_REG_L1: min 1/2||W(K chi - phi)||^2 + radius*||M chi||_1 (north_star's alternative regulariser).  The same
+     * first-order primal-dual iteration with K_full = W K only: p as in PAPER.md:49 line 1, no q, and the primal step
+     * chi_{n+1} = prox_{tau G}(chi_n - tau K W p_{n+1}) with G = radius*||M .||_1, whose prox is the soft shrinkage.
+     * relgap: the Fenchel-Young gap of the data term alone (the q part of reading R9 does not exist here). */
+    void iterate_l1(double *relgap, double *relres) {
+        apply_K(nx, ny, D.data(), chibar.data(), u.data(), work);
+        for (std::ptrdiff_t i = 0; i < P; ++i) r[i] = W[i] * (u[i] - phi[i]);
+        prox_p(P, p.data(), r.data(), sigma, lambda, lambda_conv);
+        double gap_p = 0;
+        for (std::ptrdiff_t i = 0; i < P; ++i) {
+            if (lambda_conv == PDO_LAMBDA_DATA) {
+                const double e = (double)lambda * (double)r[i] - (double)p[i];
+                gap_p += e * e / (2.0 * (double)lambda);
+            } else {
+                const double e = (double)r[i] - (double)p[i];
+                gap_p += 0.5 * e * e;
+            }
+        }
+        *relgap = (P0 > 0) ? gap_p / P0 : 0.0;
+        for (std::ptrdiff_t i = 0; i < P; ++i) wp[i] = W[i] * p[i];
+        apply_K(nx, ny, D.data(), wp.data(), v.data(), work);
+        for (std::ptrdiff_t i = 0; i < P; ++i) chinew[i] = chi[i] - tau * v[i];
+        shrink(P, chinew.data(), thr.data());
+        double dn = 0, cn = 0;
+        for (std::ptrdiff_t i = 0; i < P; ++i) {
+            const double dd = (double)chinew[i] - (double)chi[i];
+            dn += dd * dd;
+            cn += (double)chinew[i] * (double)chinew[i];
+        }
+        const double cnorm = std::sqrt(cn);
+        *relres = std::sqrt(dn) / (cnorm > 1e-300 ? cnorm : 1e-300);
+        for (std::ptrdiff_t i = 0; i < P; ++i) {
+            chibar[i] = chinew[i] + theta * (chinew[i] - chi[i]);
+            chi[i] = chinew[i];
+        }
     }
 
     /* One pass of the Repeat body.  Returns relgap_{n+1} and relres_{n+1} (readings R9). */
     void iterate(double *relgap, double *relres) {
+        if (regulariser == PDO_REG_L1) { iterate_l1(relgap, relres); return; }
         /* p_{n+1} = (p_n + sigma*(W(D chibar_n - Delta B))) / (1 + sigma[/lambda])   (residual per Eq.(1), reading R3) */
         apply_K(nx, ny, D.data(), chibar.data(), u.data(), work);
         for (std::ptrdiff_t i = 0; i < P; ++i) r[i] = W[i] * (u[i] - phi[i]);
@@ -392,6 +445,27 @@ int pdo_apply_K(int nx, int ny, int b0_dir, const double *a, double *out) {
     dipole_table(nx, ny, b0_dir, D.data());
     std::vector<Cpx<double>> work;
     apply_K(nx, ny, D.data(), a, out, work);
+    return 0;
+}
+
+int pdo_dipole_angle(int nx, int ny, double angle, double *D) {
+    if (nx < 1 || ny < 1 || !D) return -1;
+    dipole_table(nx, ny, PDO_B0_ANGLE, D, angle);
+    return 0;
+}
+
+int pdo_apply_K_angle(int nx, int ny, double angle, const double *a, double *out) {
+    if (nx < 1 || ny < 1 || !a || !out) return -1;
+    std::vector<double> D((std::ptrdiff_t)nx * ny);
+    dipole_table(nx, ny, PDO_B0_ANGLE, D.data(), angle);
+    std::vector<Cpx<double>> work;
+    apply_K(nx, ny, D.data(), a, out, work);
+    return 0;
+}
+
+int pdo_shrink(int n, double *v, const double *t) {
+    if (n < 0 || !v || !t) return -1;
+    shrink<double>(n, v, t);
     return 0;
 }
 

@@ -20,6 +20,10 @@
  *   PD iteration .... pinned (closed-form first iterate, per-frequency recurrence at
  *                     alpha=0, dense-matrix brute force on 8x8, zero-mean invariant,
  *                     monotone proximal-point distance, convention A == rescaled B)
+ *   l1-on-chi variant (PDO_REG_L1) and oblique in-plane B0 (PDO_B0_ANGLE): pinned (prox optimality,
+ *                     closed-form first iterate, dense-matrix brute force, LASSO optimality at the fixed
+ *                     point, alpha=0 reduction to the TV path; axis angles reduce to PDO_B0_X / PDO_B0_Y,
+ *                     45 degree closed-form values, rotated analytic field of a disc)
  *   reconstruction QUALITY on real data: parity unpinned (the paper prints no number).
  */
 #ifndef PD_ORACLE_H
@@ -29,7 +33,11 @@
 extern "C" {
 #endif
 
-enum { PDO_B0_X = 0, PDO_B0_Y = 1 };
+enum { PDO_B0_X = 0, PDO_B0_Y = 1,
+       PDO_B0_ANGLE = 2 /* in-plane unit vector (cos a, sin a), a = b0_angle: k_b = kx cos a + ky sin a */ };
+enum { PDO_REG_TV = 0,  /* the paper's regulariser ||M G chi||_1 with the dual q (reading R1) */
+       PDO_REG_L1 = 1   /* plain l1 on chi, lambda ||M chi||_1: no q, the primal step ends in a soft shrinkage
+                           (BASELINE.json north_star: "lambda ||chi||_1 ... the prox (clip onto the lambda-ball, or shrinkage)") */ };
 enum { PDO_TV_ISO = 0, PDO_TV_ANISO = 1 };
 enum { PDO_LAMBDA_REG = 0,  /* "convention B": 1/2||W(K chi - phi)||^2 + lambda ||M G chi||_1 (BASELINE.json north_star) */
        PDO_LAMBDA_DATA = 1  /* "convention A": lambda/2 ||...||^2 + ||M G chi||_1, literally PAPER.md:37,49 */ };
@@ -44,6 +52,8 @@ typedef struct {
     int tv_mode;       /* PDO_TV_ISO / PDO_TV_ANISO (reading R4) */
     int lambda_conv;   /* PDO_LAMBDA_REG / PDO_LAMBDA_DATA (reading R2) */
     int check_every;   /* tolerance is tested when (n+1) % check_every == 0 */
+    int regulariser;   /* PDO_REG_TV (default 0) / PDO_REG_L1 */
+    double b0_angle;   /* radians from the x axis, used when b0_dir == PDO_B0_ANGLE (0 = PDO_B0_X, pi/2 = PDO_B0_Y) */
 } pdo_params;
 
 /* 2-D DFT, unnormalised forward, 1/(nx*ny)-scaled inverse.  Textbook iterative radix-2
@@ -58,6 +68,11 @@ int pdo_dft2_bruteforce(int nx, int ny, const double *in_re, const double *in_im
 int pdo_dipole(int nx, int ny, int b0_dir, double *D);
 /* K(a) = Re(IFFT2(D .* FFT2(a))) ("dipole kernel convolution operator"). */
 int pdo_apply_K(int nx, int ny, int b0_dir, const double *a, double *out);
+/* The same two for an in-plane B0 direction at `angle` radians from the x axis: k_b = kx cos(angle) + ky sin(angle). */
+int pdo_dipole_angle(int nx, int ny, double angle, double *D);
+int pdo_apply_K_angle(int nx, int ny, double angle, const double *a, double *out);
+/* Soft shrinkage, the prox of t*|.|: v <- sign(v) max(|v| - t[i], 0), per element (PDO_REG_L1). */
+int pdo_shrink(int n, double *v, const double *t);
 /* Forward differences with Neumann boundary, and the exact adjoint (reading R7). */
 int pdo_grad(int nx, int ny, const double *a, double *gx, double *gy);
 int pdo_gradT(int nx, int ny, const double *qx, const double *qy, double *out);

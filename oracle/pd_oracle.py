@@ -12,7 +12,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
-B0_X, B0_Y = 0, 1
+B0_X, B0_Y, B0_ANGLE = 0, 1, 2
+REG_TV, REG_L1 = 0, 1
 TV_ISO, TV_ANISO = 0, 1
 LAMBDA_REG, LAMBDA_DATA = 0, 1
 
@@ -23,6 +24,7 @@ class Params(C.Structure):
         ("lambda_", C.c_double), ("sigma", C.c_double), ("tau", C.c_double), ("theta", C.c_double),
         ("max_iters", C.c_int), ("tol", C.c_double),
         ("tv_mode", C.c_int), ("lambda_conv", C.c_int), ("check_every", C.c_int),
+        ("regulariser", C.c_int), ("b0_angle", C.c_double),
     ]
 
 
@@ -89,6 +91,27 @@ def apply_K(a, b0_dir=B0_Y):
     return out
 
 
+def dipole_angle(nx, ny, angle):
+    D = np.empty((ny, nx), np.float64)
+    _check(lib().pdo_dipole_angle(nx, ny, C.c_double(angle), _d(D)), "dipole_angle")
+    return D
+
+
+def apply_K_angle(a, angle):
+    a = _c64(a)
+    ny, nx = a.shape
+    out = np.empty_like(a)
+    _check(lib().pdo_apply_K_angle(nx, ny, C.c_double(angle), _d(a), _d(out)), "apply_K_angle")
+    return out
+
+
+def shrink(v, t):
+    v = _c64(v).copy()
+    t = _c64(np.broadcast_to(t, v.shape))
+    _check(lib().pdo_shrink(v.size, _d(v), _d(t)), "shrink")
+    return v
+
+
 def grad(a):
     a = _c64(a)
     ny, nx = a.shape
@@ -119,14 +142,16 @@ def prox_q(tx, ty, radius, tv_mode=TV_ISO):
 
 
 def make_params(nx, ny, batch, lambda_, sigma, tau, theta=1.0, max_iters=100, tol=0.0, b0_dir=B0_Y,
-                tv_mode=TV_ISO, lambda_conv=LAMBDA_REG, check_every=1):
+                tv_mode=TV_ISO, lambda_conv=LAMBDA_REG, check_every=1, regulariser=REG_TV, b0_angle=None):
+    if b0_angle is not None:
+        b0_dir = B0_ANGLE
     return Params(nx, ny, batch, b0_dir, lambda_, sigma, tau, theta, max_iters, tol, tv_mode, lambda_conv,
-                  check_every)
+                  check_every, regulariser, 0.0 if b0_angle is None else float(b0_angle))
 
 
 def solve(field, mask=None, weight=None, *, lambda_, sigma, tau, theta=1.0, max_iters=100, tol=0.0,
           b0_dir=B0_Y, tv_mode=TV_ISO, lambda_conv=LAMBDA_REG, check_every=1, precision="f64",
-          want_state=False, want_hist=True):
+          want_state=False, want_hist=True, regulariser=REG_TV, b0_angle=None):
     """Run the PD iteration slice after slice.  field/mask/weight: [batch][ny][nx] (or [ny][nx]).
 
     Returns a dict: chi (float64 [batch][ny][nx]), chi32, iters_done, relgap/relres ([batch][max_iters],
@@ -142,7 +167,7 @@ def solve(field, mask=None, weight=None, *, lambda_, sigma, tau, theta=1.0, max_
         if arr is not None and arr.size != field.size:
             raise ValueError("%s must have the shape of field" % name)
     prm = make_params(nx, ny, batch, lambda_, sigma, tau, theta, max_iters, tol, b0_dir, tv_mode, lambda_conv,
-                      check_every)
+                      check_every, regulariser, b0_angle)
     chi64 = np.empty((batch, ny, nx), np.float64)
     chi32 = np.empty((batch, ny, nx), np.float32)
     iters = np.zeros(batch, np.int32)
@@ -162,11 +187,12 @@ def solve(field, mask=None, weight=None, *, lambda_, sigma, tau, theta=1.0, max_
 
 
 def trace(field, mask=None, weight=None, *, lambda_, sigma, tau, theta=1.0, max_iters=10, b0_dir=B0_Y,
-          tv_mode=TV_ISO, lambda_conv=LAMBDA_REG):
+          tv_mode=TV_ISO, lambda_conv=LAMBDA_REG, regulariser=REG_TV, b0_angle=None):
     """Single slice; returns trace[n][c] for n=0..max_iters, c = (chi, p, qx, qy)."""
     field = _c32(field)
     ny, nx = field.shape
-    prm = make_params(nx, ny, 1, lambda_, sigma, tau, theta, max_iters, 0.0, b0_dir, tv_mode, lambda_conv, 1)
+    prm = make_params(nx, ny, 1, lambda_, sigma, tau, theta, max_iters, 0.0, b0_dir, tv_mode, lambda_conv, 1,
+                      regulariser, b0_angle)
     tr = np.empty((max_iters + 1, 4, ny, nx), np.float64)
     _check(lib().pdo_trace_f64(C.byref(prm), _f(field), _f(_c32(mask)), _f(_c32(weight)), _d(tr)), "trace")
     return tr

@@ -474,3 +474,169 @@ def test_theta_zero_and_b0x_variants_run(oracle):
     x = oracle.solve(fx, lambda_=0.2, sigma=SIG, tau=SIG, max_iters=6, b0_dir=oracle.B0_X)
     y = oracle.solve(case["field"], lambda_=0.2, sigma=SIG, tau=SIG, max_iters=6, b0_dir=oracle.B0_Y)
     assert rel(x["chi"][0].T, y["chi"][0]) < 1e-12
+
+
+# ---------------------------------------------------------------- P15: oblique in-plane B0
+def np_dipole_angle(nx, ny, ang):
+    """Closed form typed independently: k_b = k . (cos a, sin a), standard fftfreq."""
+    kx = np.fft.fftfreq(nx)[None, :]
+    ky = np.fft.fftfreq(ny)[:, None]
+    k2 = kx * kx + ky * ky
+    kb = kx * np.cos(ang) + ky * np.sin(ang)
+    out = np.zeros((ny, nx))
+    nz = k2 > 0
+    out[nz] = 1.0 / 3.0 - (kb * kb + 0 * k2)[nz] / k2[nz]
+    return out
+
+
+@pytest.mark.parametrize("ny,nx", [(16, 16), (8, 32), (12, 10)])
+def test_P15_dipole_angle_reduces_to_axes_and_closed_form(oracle, ny, nx):
+    assert rel(oracle.dipole_angle(nx, ny, 0.0), oracle.dipole(nx, ny, oracle.B0_X)) < 1e-15
+    assert rel(oracle.dipole_angle(nx, ny, np.pi / 2), oracle.dipole(nx, ny, oracle.B0_Y)) < 1e-15
+    for ang in (0.3, np.pi / 4, 2.0, -0.7):
+        D = oracle.dipole_angle(nx, ny, ang)
+        assert rel(D, np_dipole_angle(nx, ny, ang)) < 1e-13
+        assert D[0, 0] == 0.0 and D.min() >= -2.0 / 3.0 - 1e-12 and D.max() <= 1.0 / 3.0 + 1e-12
+        # B0 and -B0 are the same axis
+        assert rel(oracle.dipole_angle(nx, ny, ang + np.pi), D) < 1e-12
+    # 45 degrees on a square grid: -2/3 on the diagonal kx = ky, +1/3 on the anti-diagonal, transpose-symmetric
+    if nx == ny:
+        D = oracle.dipole_angle(nx, ny, np.pi / 4)
+        for i in range(1, nx // 2):
+            assert abs(D[i, i] + 2.0 / 3.0) < 1e-12 and abs(D[nx - i, i] - 1.0 / 3.0) < 1e-12
+        assert rel(D, D.T) < 1e-12
+    # the sum over two perpendicular in-plane directions is 2/3 - 1 = -1/3 away from DC
+    S = oracle.dipole_angle(nx, ny, 0.4) + oracle.dipole_angle(nx, ny, 0.4 + np.pi / 2)
+    S[0, 0] = -1.0 / 3.0
+    assert np.abs(S + 1.0 / 3.0).max() < 1e-12
+
+
+def test_P15_forward_model_cylinder_rotated(oracle):
+    """The analytic field of a cylinder, (R^2/2r^2) cos 2(theta - a) outside and -1/6 inside, turns with B0; and
+    K(a) stays real and symmetric (the oracle takes the real part: only the even part of D acts)."""
+    n, R, ang = 256, 16.0, 0.6
+    yy, xx = np.mgrid[0:n, 0:n]
+    c = n / 2.0
+    disc = ((xx - c) ** 2 + (yy - c) ** 2 <= R * R).astype(np.float64)
+    f = oracle.apply_K_angle(disc, ang)
+    f = f - f[0, 0]
+    r2 = (xx - c) ** 2 + (yy - c) ** 2
+    inside = r2 <= (0.6 * R) ** 2
+    assert abs(f[inside].mean() + 1.0 / 6.0) < 0.02
+    ring = (r2 > (1.5 * R) ** 2) & (r2 < (4 * R) ** 2)
+    th = np.arctan2(yy - c, xx - c)
+    ana = R * R / (2 * np.maximum(r2, 1e-30)) * np.cos(2 * (th - ang))
+    assert np.corrcoef(f[ring], ana[ring])[0, 1] > 0.995
+    assert rel(f[ring], ana[ring]) < 0.12
+    # independent numpy evaluation of Re(IFFT(D FFT(a)))
+    a = rng(31).standard_normal((24, 40))
+    ref = np.real(np.fft.ifft2(np_dipole_angle(40, 24, ang) * np.fft.fft2(a)))
+    assert rel(oracle.apply_K_angle(a, ang), ref) < 1e-12
+    b = rng(32).standard_normal((24, 40))
+    assert abs(np.vdot(oracle.apply_K_angle(a, ang), b) - np.vdot(a, oracle.apply_K_angle(b, ang))) < 1e-10
+
+
+def test_P15_angle_iteration_matches_axis_iteration(oracle):
+    case = synth.random_case(32, 16, 2, seed=15, with_mask=True, with_weight=True)
+    kw = dict(lambda_=0.3, sigma=SIG, tau=SIG, max_iters=7)
+    a = oracle.solve(case["field"], case["mask"], case["weight"], b0_dir=oracle.B0_X, **kw)
+    b = oracle.solve(case["field"], case["mask"], case["weight"], b0_angle=0.0, **kw)
+    assert rel(b["chi"], a["chi"]) < 1e-14
+    c = oracle.solve(case["field"], case["mask"], case["weight"], b0_angle=np.pi / 2, **kw)
+    d = oracle.solve(case["field"], case["mask"], case["weight"], b0_dir=oracle.B0_Y, **kw)
+    assert rel(c["chi"], d["chi"]) < 1e-12
+
+
+# ---------------------------------------------------------------- P16: l1 on chi with a shrinkage prox (north_star's alternative)
+def test_P16_shrink_is_the_prox_of_the_l1_norm(oracle):
+    r = rng(16)
+    v = np.concatenate([r.standard_normal(200) * 2, [0.0, 1.0, -1.0, 0.5, -0.5]])
+    t = np.abs(r.standard_normal(v.size)) + 0.0
+    t[-5:] = [1.0, 1.0, 1.0, 1.0, 1.0]
+    x = oracle.shrink(v, t)
+    # first-order optimality of argmin_x 1/2 (x - v)^2 + t |x| : v - x = t sign(x) where x != 0, |v - x| <= t where x = 0
+    nz = x != 0
+    assert np.allclose((v - x)[nz], (t * np.sign(x))[nz], atol=1e-15)
+    assert np.all(np.abs(v - x)[~nz] <= t[~nz] + 1e-15)
+    assert np.all(np.sign(x[nz]) == np.sign(v[nz]))
+    assert np.array_equal(x[-5:], [0.0, 0.0, 0.0, 0.0, 0.0])
+    # brute force: the minimiser on a fine grid
+    for vi, ti in ((1.7, 0.4), (-0.9, 0.25), (0.1, 0.3)):
+        g = np.linspace(-3, 3, 600001)
+        xb = g[np.argmin(0.5 * (g - vi) ** 2 + ti * np.abs(g))]
+        assert abs(oracle.shrink(np.array([vi]), ti)[0] - xb) < 2e-5
+    # threshold 0 is the identity
+    assert np.array_equal(oracle.shrink(v, 0.0), v)
+
+
+@pytest.mark.parametrize("with_w", [False, True])
+def test_P16_l1_first_iterate_closed_form(oracle, with_w):
+    """chi_1 = shrink((sigma tau/(1+sigma)) K(W^2 phi), tau alpha M), p_1 = -sigma W phi/(1+sigma), relgap_1 = 1/(1+sigma)^2."""
+    case = synth.random_case(32, 16, 1, seed=160, with_mask=True, with_weight=with_w)
+    phi = case["field"][0].astype(np.float64)
+    W = case["weight"][0].astype(np.float64) if with_w else np.ones_like(phi)
+    M = case["mask"][0].astype(np.float64)
+    alpha, tau = 0.02, 0.3
+    out = oracle.solve(case["field"], case["mask"], case["weight"] if with_w else None, lambda_=alpha, sigma=SIG, tau=tau,
+                       max_iters=1, regulariser=oracle.REG_L1, want_state=True)
+    v = SIG * tau / (1 + SIG) * np_K(W * W * phi)
+    chi1 = np.sign(v) * np.maximum(np.abs(v) - tau * alpha * M, 0.0)
+    assert rel(out["chi"][0], chi1) < 1e-12
+    assert rel(out["p"][0], -SIG * W * phi / (1 + SIG)) < 1e-12
+    assert abs(out["relgap"][0, 0] - 1.0 / (1 + SIG) ** 2) < 1e-12
+    assert np.all(out["qx"] == 0) and np.all(out["qy"] == 0)
+    assert (out["chi"][0] == 0).sum() > 0 and (out["chi"][0] != 0).sum() > 0     # the threshold bites on part of the image
+
+
+def test_P16_l1_dense_matrix_bruteforce_8x8(oracle):
+    """8x8, 6 iterations, K as a dense matrix from DFT matrices, the iteration written with mat-vecs."""
+    n = 8
+    P = n * n
+    case = synth.random_case(n, n, 1, seed=161, with_mask=True, with_weight=True)
+    phi = case["field"][0].astype(np.float64).ravel()
+    M = case["mask"][0].astype(np.float64).ravel()
+    M[::5] = 0.0
+    W = case["weight"][0].astype(np.float64).ravel()
+    F1 = np.exp(-2j * np.pi * np.outer(np.arange(n), np.arange(n)) / n)
+    F2 = np.kron(F1, F1)
+    Kmat = np.real(np.conj(F2).T @ np.diag(np_dipole(n, n).ravel()) @ F2) / P
+    A = np.diag(W) @ Kmat
+    alpha, sig, tau, theta = 0.05, 0.4, 0.5, 0.8
+    chi, chib, p = np.zeros(P), np.zeros(P), np.zeros(P)
+    for _ in range(6):
+        p = (p + sig * (A @ chib - W * phi)) / (1 + sig)
+        v = chi - tau * (A.T @ p)
+        chin = np.sign(v) * np.maximum(np.abs(v) - tau * alpha * M, 0.0)
+        chib = chin + theta * (chin - chi)
+        chi = chin
+    out = oracle.solve(case["field"], M.reshape(1, n, n).astype(np.float32), case["weight"], lambda_=alpha, sigma=sig, tau=tau,
+                       theta=theta, max_iters=6, regulariser=oracle.REG_L1, want_state=True)
+    assert rel(out["chi"][0].ravel(), chi) < 1e-12
+    assert rel(out["p"][0].ravel(), p) < 1e-12
+    assert rel(out["chibar"][0].ravel(), chib) < 1e-12
+
+
+def test_P16_l1_fixed_point_is_the_lasso_optimum(oracle):
+    """After many iterations chi satisfies the optimality condition of min 1/2||K chi - phi||^2 + alpha||chi||_1:
+    g = K(K chi - phi) has |g| <= alpha everywhere and g = -alpha sign(chi) on the support."""
+    n = 16
+    case = synth.random_case(n, n, 1, seed=162, with_mask=False)
+    phi = case["field"][0].astype(np.float64)
+    alpha = 0.05 * np.abs(np_K(phi)).max()
+    out = oracle.solve(case["field"], None, lambda_=alpha, sigma=1.0, tau=1.0, max_iters=6000, regulariser=oracle.REG_L1,
+                       want_hist=False)
+    chi = out["chi"][0]
+    g = np_K(np_K(chi) - phi)
+    assert np.abs(g).max() <= alpha * (1 + 1e-6)
+    sup = np.abs(chi) > 1e-9 * np.abs(chi).max()
+    assert sup.sum() > 0 and (~sup).sum() > 0
+    assert np.abs(g[sup] + alpha * np.sign(chi[sup])).max() < 1e-6 * alpha
+
+
+def test_P16_l1_with_alpha_zero_equals_tv_with_alpha_zero(oracle):
+    case = synth.random_case(16, 16, 2, seed=163, with_mask=True, with_weight=True)
+    kw = dict(lambda_=0.0, sigma=SIG, tau=SIG, max_iters=9)
+    a = oracle.solve(case["field"], case["mask"], case["weight"], **kw)
+    b = oracle.solve(case["field"], case["mask"], case["weight"], regulariser=oracle.REG_L1, **kw)
+    assert rel(b["chi"], a["chi"]) < 1e-14
+    assert np.allclose(b["relgap"], a["relgap"], rtol=1e-12)

@@ -28,7 +28,8 @@ from paper_2006_09808_b200 import shard, synth  # noqa: E402  (input generator a
 
 METRIC = "pd_slice_iterations_per_s"
 UNIT = "slice-iterations/s"
-WORKLOADS = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4, "NS": 5}
+WORKLOADS = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4, "NS": 5,
+             "E1": 6, "E2": 7, "E3": 8}   # E1-E3: stand-ins in the paper's own matrix sizes (256x258, 128x132)
 
 # Algorithmic HBM bytes per pixel of a slice and launch of each kernel class of the streaming variant:
 # what the pass must read and write once, spectra counted at 4 B/px/slice (one float2 per pixel of a slice PAIR).
@@ -233,6 +234,9 @@ def main():
     ap.add_argument("--hybrid-tail", type=int, default=-1,
                     help="PD_OPT_HYBRID_TAIL: slice pairs run by the streaming kernels beside the resident clusters "
                          "(-1 automatic, 0 off)")
+    ap.add_argument("--no-graph-loop", action="store_true",
+                    help="PD_OPT_GRAPH_LOOP = 0: plain launches from the host instead of the graphed device-side loop "
+                         "(used for the ncu launch lists)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -269,6 +273,8 @@ def main():
     if args.variant != "auto":
         plan.set_option(binding.OPT_VARIANT, {"streaming": binding.VARIANT_STREAMING, "resident": binding.VARIANT_RESIDENT}[args.variant])
     plan.set_option(binding.OPT_HYBRID_TAIL, args.hybrid_tail)
+    if args.no_graph_loop:
+        plan.set_option(binding.OPT_GRAPH_LOOP, 0)
     weight = None
     if args.weighted:
         gen = torch.Generator(device="cuda").manual_seed(200609808 + rank)

@@ -59,14 +59,19 @@ enum pd_option {
                                 resident clusters, on the SMs those leave free (slices are independent).
                                 -1 (default): chosen from the batch size ; 0: off ; n > 0: exactly n pairs.
                                 pd_solve still returns with all work ordered on the caller's stream. */
-    PD_OPT_GRAPH_LOOP = 9    /* streaming variant: 1 (default): the whole solve is ONE CUDA graph launch -- init, a conditional
+    PD_OPT_GRAPH_LOOP = 9,   /* streaming variant: 1 (default): the whole solve is ONE CUDA graph launch -- init, a conditional
                                 WHILE node around the iteration kernels whose condition a loop-control kernel sets on the
                                 device (false once every slice has stopped or max_iters is reached), finish: nothing is
                                 launched for iterations nobody needs and the host is never asked.  The graph
                                 is cached in the plan and rebuilt when the arguments of pd_solve change.  0: one stream
-                                launch per kernel, 2*max_iters + 3 of them (the kernels of a stopped slice return at once).
+                                launch per kernel, 2*max_iters + 4 of them (the kernels of a stopped slice return at once).
                                 PD_OPT_KERNEL_TIMING = 1 always uses plain launches. */
+    PD_OPT_REGULARISER = 10  /* PD_REG_TV (default): the paper's lambda ||M G chi||_1 with the dual q.
+                                PD_REG_L1: lambda ||M chi||_1 (BASELINE.json north_star's alternative):
+                                no q, the primal step ends in the soft shrinkage chi <- sign(v) max(|v| - tau lambda M, 0);
+                                relgap is then the Fenchel-Young gap of the data term alone.  PD_OPT_TV_MODE is ignored. */
 };
+enum { PD_REG_TV = 0, PD_REG_L1 = 1 };
 /* kernel classes for pd_get_kernel_times.  Streaming variant: init, finish and, per iteration, fd_cols + fd_rows
  * (W = identity, Fourier-domain dual: two launches) or dipole_cols + dual_rows + dipole_cols + fd_rows (W set, or
  * PD_OPT_FOURIER_DUAL = 0: four launches; class 3 is no longer used).  Resident variant: class 5, one bracket around
@@ -124,6 +129,12 @@ int pd_set_weight(pd_plan_t p, const float *W);
 
 /* Replace lambda / sigma / tau / theta of an existing plan (same checks as pd_plan). */
 int pd_set_steps(pd_plan_t p, float lambda, float sigma, float tau, float theta);
+
+/* Oblique in-plane B0 (BASELINE.json north_star "B0_dir"): the dipole table is rebuilt for the
+ * unit vector (cos a, sin a), a = angle_rad from the x axis: k_b = kx cos a + ky sin a (0 = PD_B0_X, pi/2 = PD_B0_Y).
+ * K is the real part of F^-1 D F (R12), so the even part (D(k) + D(-k))/2 is stored (it differs from D only on
+ * the Nyquist lines).  Host call; waits for the device, then uploads.  Errors: PD_EINVAL, PD_ECUDA. */
+int pd_set_b0_angle(pd_plan_t p, float angle_rad);
 
 int pd_set_option(pd_plan_t p, int key, int value);
 

@@ -15,7 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libpd_b200.so")
 
 B0_X, B0_Y = 0, 1
 OK, EINVAL, ESIZE, ESTEP, ENOMEM, ECUDA, EVARIANT = 0, -1, -2, -3, -4, -5, -6
-OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING, OPT_FOURIER_DUAL, OPT_HYBRID_TAIL, OPT_GRAPH_LOOP = range(10)
+OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING, OPT_FOURIER_DUAL, OPT_HYBRID_TAIL, OPT_GRAPH_LOOP, OPT_REGULARISER = range(11)
+REG_TV, REG_L1 = 0, 1
 KERNEL_CLASSES = ["init", "dual_rows", "dipole_cols", "primal_rows", "finish", "resident", "fd_cols", "fd_rows"]
 TV_ISO, TV_ANISO = 0, 1
 LAMBDA_REG, LAMBDA_DATA = 0, 1
@@ -23,7 +24,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_get_hybrid_rho", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -49,6 +50,7 @@ def lib():
         L.pd_set_weight.argtypes = [vp, vp]
         L.pd_set_steps.argtypes = [vp, fp, fp, fp, fp]
         L.pd_set_option.argtypes = [vp, ip, ip]
+        L.pd_set_b0_angle.argtypes = [vp, fp]
         L.pd_get_stats.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.pd_get_stats_host.argtypes = [vp, vp, vp, vp, vp]
         L.pd_get_kernel_times.argtypes = [vp, vp, vp]
@@ -119,6 +121,10 @@ class Plan:
 
     def set_steps(self, lambda_, sigma, tau, theta=1.0):
         _check(lib().pd_set_steps(self._h, lambda_, sigma, tau, theta))
+
+    def set_b0_angle(self, angle_rad):
+        """pd_set_b0_angle: B0 along (cos a, sin a) in the slice plane."""
+        _check(lib().pd_set_b0_angle(self._h, float(angle_rad)))
 
     def set_weight(self, weight):
         if weight is not None and weight.numel() != self.batch * self.ny * self.nx:

@@ -1,10 +1,13 @@
 // fft_regs.cuh -- register-resident complex FFT building blocks for sm_100a.
 //
-// A length-N line (N in {64,128,256,512}) is transformed by T = N/E cooperating threads that each
+// A length-N line (N in {64,128,256}) is transformed by T = N/E cooperating threads that each
 // hold E points in registers: one in-register DFT of size E, a twiddle multiply, ONE exchange
 // through shared memory, and E/T in-register DFTs of size T.  Input and output use the same
 // thread<->index map (thread j holds the points j + T*m, m = 0..E-1), so a forward and an inverse
 // transform chain without any extra shuffle (used for F^-1 D F).
+// N = 512 keeps 16 points per thread (a whole warp per line, T = 32) and runs THREE stages of in-register
+// 8-point DFTs with two exchanges (fft_line3): 32 points per thread cost 64 registers for the line alone, which
+// held the 512-wide streaming kernels at 96-128 registers and 16-20 warps per SM.
 //
 // Only the forward (exp(-i...)) transform exists; the inverse is obtained by swapping re/im before
 // and after, which is a register renaming.
@@ -18,11 +21,17 @@
 
 namespace pdk {
 
-template <int N> struct FftCfg;
-template <> struct FftCfg<64>  { static constexpr int E = 8,  T = 8;  };
-template <> struct FftCfg<128> { static constexpr int E = 16, T = 8;  };
-template <> struct FftCfg<256> { static constexpr int E = 16, T = 16; };
-template <> struct FftCfg<512> { static constexpr int E = 32, T = 16; };
+// E points per thread, T threads per line; TW: float2 entries of the shared-memory twiddle table (TwiddlesSmem);
+// REGION: float2 entries the exchange region of one line needs at least (two-stage lines: E rows of the caller's LD)
+// COL: the configuration of the COLUMN kernels, whose T threads of a line sit in different warps and exchange through
+// CTA-wide barriers: there the two-stage 512-point line (32 points per thread, two barriers per transform) measured
+// faster than the three-stage one (four barriers; 64-register cap at 512 threads per CTA): C4 columns 34.3 vs 38.3 ms.
+template <int N, bool COL = false> struct FftCfg;
+template <bool COL> struct FftCfg<64, COL>  { static constexpr int E = 8,  T = 8,  TW = E * T, REGION = 0; };
+template <bool COL> struct FftCfg<128, COL> { static constexpr int E = 16, T = 8,  TW = E * T, REGION = 0; };
+template <bool COL> struct FftCfg<256, COL> { static constexpr int E = 16, T = 16, TW = E * T, REGION = 0; };
+template <> struct FftCfg<512, false> { static constexpr int E = 16, T = 32, TW = 2 * E * T, REGION = 544; };
+template <> struct FftCfg<512, true>  { static constexpr int E = 32, T = 16, TW = E * T, REGION = 0; };
 
 // cos(2*pi*i/32), sin(2*pi*i/32), i = 0..15, as literals so that they fold after unrolling.
 __device__ __forceinline__ float cos32(int i) {
@@ -108,6 +117,14 @@ __device__ __forceinline__ void dft_reg(float2 (&v)[R]) {
     for (int k = 0; k < R; ++k) v[k] = t[k];
 }
 
+// sum over the T threads of one line (T a power of two <= 32, the group is aligned inside its warp)
+template <int T>
+__device__ __forceinline__ float group_sum(float v) {
+#pragma unroll
+    for (int o = T / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
 __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
     return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.x, w.y, a.y * w.x));
 }
@@ -126,7 +143,8 @@ struct NamedSync {  // ... over `count` threads (whole warps) that all use hardw
 // Per-thread inter-stage twiddles W_N^(j*k2), k2 = 1..E-1 (index 0 unused), from the plan's double-precision table.
 template <int N>
 struct Twiddles {
-    static constexpr int E = FftCfg<N>::E;
+    static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
+    static constexpr bool kThree = false;
     float2 w[E];
     __device__ __forceinline__ void load(const float2 *__restrict__ table, int j) {
 #pragma unroll
@@ -137,9 +155,10 @@ struct Twiddles {
 
 // Same twiddles kept in shared memory as a table tws[k2*T + j] = W_N^(j*k2) (conflict-free: consecutive j), read when
 // needed instead of living in E registers for the whole kernel.
-template <int N>
+template <int N, bool COL = false>
 struct TwiddlesSmem {
-    static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
+    static constexpr int E = FftCfg<N, COL>::E, T = FftCfg<N, COL>::T;
+    static constexpr bool kThree = false;
     const float2 *w;  // &tws[j]
     __device__ __forceinline__ float2 get(int k) const { return w[k * T]; }
     // fill a table of E*T float2 from the plan's W_N^n table (all threads of the CTA cooperate; caller synchronises)
@@ -147,21 +166,94 @@ struct TwiddlesSmem {
         for (int i = tid; i < E * T; i += nthreads) tws[i] = __ldg(table + (((i % T) * (i / T)) & (N - 1)));
     }
 };
+// N = 512, three stages (fft_line3): two tables of 16 entries per thread, [idx][j]:
+//   table 1, idx = 8 b + k3 : W_64^(n2 k3),            n2 = (j >> 3) + 4 b
+//   table 2, idx = 8 c + k2 : W_512^(n1 (k3 + 8 k2)),  n1 = j & 7, k3 = 2 (j >> 3) + c
+template <>
+struct TwiddlesSmem<512, false> {
+    static constexpr int E = 16, T = 32;
+    static constexpr bool kThree = true;
+    const float2 *w;  // &tws[j]
+    __device__ __forceinline__ float2 get1(int idx) const { return w[idx * T]; }
+    __device__ __forceinline__ float2 get2(int idx) const { return w[(16 + idx) * T]; }
+    static __device__ __forceinline__ void fill(float2 *tws, const float2 *__restrict__ table, int tid, int nthreads) {
+        for (int i = tid; i < 2 * E * T; i += nthreads) {
+            const int j = i % T, idx = (i / T) % 16, hi = idx >> 3, lo = idx & 7;
+            const int e = (i < E * T) ? 8 * ((j >> 3) + 4 * hi) * lo                     // 8 n2 k3
+                                      : (j & 7) * ((2 * (j >> 3) + hi) + 8 * lo);        // n1 (k3 + 8 k2)
+            tws[i] = __ldg(table + (e & 511));
+        }
+    }
+};
 template <int N>
 __device__ __forceinline__ float2 tw_get(const Twiddles<N> &tw, int k) { return tw.w[k]; }
-template <int N>
-__device__ __forceinline__ float2 tw_get(const TwiddlesSmem<N> &tw, int k) { return tw.get(k); }
+template <int N, bool COL>
+__device__ __forceinline__ float2 tw_get(const TwiddlesSmem<N, COL> &tw, int k) { return tw.get(k); }
+
+// N = 512 = 8 x 8 x 8 with n = n1 + 8 n2 + 64 n3 and k = k3 + 8 k2 + 64 k1 (thread j of the warp holds n = j + 32 m:
+// n1 = j & 7, n2 = (j >> 3) + 4 (m & 1), n3 = m >> 1):
+//   A[n1,n2,k3] = sum_n3 x[n] W_8^(n3 k3)          ; A *= W_64^(n2 k3)            ; exchange 1 (over n2)
+//   B[n1,k3,k2] = sum_n2 A[n1,n2,k3] W_8^(n2 k2)   ; B *= W_512^(n1 (k3 + 8 k2))  ; exchange 2 (over n1)
+//   X[k3 + 8 k2 + 64 k1] = sum_n1 B[n1,k3,k2] W_8^(n1 k1)
+// Every stage is two in-register 8-point DFTs over the elements of equal parity of m; the output lands in the input's
+// map (k = j + 32 m with k3 = j & 7, k2 = (j >> 3) + 4 (m & 1), k1 = m >> 1).  sm: >= FftCfg<512>::REGION float2.
+// Exchange 1 is bank-conflict free both ways; the writes of exchange 2 are two-way conflicted, its reads free.
+template <class Sync>
+__device__ __forceinline__ void fft_line3(float2 (&v)[16], float2 *sm, const int j, const TwiddlesSmem<512, false> &tw, Sync sync) {
+    const int r = j & 7, q = j >> 3;
+    float2 w[8];
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {   // stage A
+#pragma unroll
+        for (int i = 0; i < 8; ++i) w[i] = v[b + 2 * i];
+        dft_reg<8>(w);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[b + 2 * k] = (k == 0) ? w[0] : cmul(w[k], tw.get1(8 * b + k));
+    }
+    sync();  // earlier readers of sm are done
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+        for (int k3 = 0; k3 < 8; ++k3) sm[(k3 >> 1) * 136 + (k3 & 1) * 64 + b * 32 + j] = v[b + 2 * k3];   // (k3, n2 = q + 4b, n1 = r)
+    sync();
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {   // stage B: k3 = 2q + c
+#pragma unroll
+        for (int n2 = 0; n2 < 8; ++n2) w[n2] = sm[q * 136 + c * 64 + n2 * 8 + r];
+        dft_reg<8>(w);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[c + 2 * k] = cmul(w[k], tw.get2(8 * c + k));
+    }
+    sync();  // exchange 1 has been read
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int k2 = 0; k2 < 8; ++k2) sm[r * 65 + k2 * 8 + 2 * q + c] = v[c + 2 * k2];   // (n1 = r, k2, k3 = 2q + c)
+    sync();
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {   // stage C: k3 = r, k2 = q + 4b
+#pragma unroll
+        for (int n1 = 0; n1 < 8; ++n1) w[n1] = sm[n1 * 65 + (q + 4 * b) * 8 + r];
+        dft_reg<8>(w);
+#pragma unroll
+        for (int k1 = 0; k1 < 8; ++k1) v[b + 2 * k1] = w[k1];
+    }
+}
 
 // Cooperative forward FFT of one length-N line held by T threads (thread j: points j + T*m).
 //   sm : this line's exchange region, E rows of LD float2 (row k2, column j)
 //   SYNC: functor that synchronises the T threads of the line (and orders their shared-memory accesses)
 template <int N, int LD, class Tw, class Sync>
-__device__ __forceinline__ void fft_line(float2 (&v)[FftCfg<N>::E], float2 *sm, int j, const Tw &tw,
+__device__ __forceinline__ void fft_line(float2 (&v)[Tw::E], float2 *sm, int j, const Tw &tw,
                                          Sync sync) {
-    constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, C = E / T;
+    if constexpr (Tw::kThree) {
+        fft_line3(v, sm, j, tw, sync);
+        return;
+    } else {
+    constexpr int E = Tw::E, T = Tw::T, C = E / T;
     dft_reg<E>(v);  // over n2: Y[j][k2]
 #pragma unroll
-    for (int k = 1; k < E; ++k) v[k] = cmul(v[k], tw_get<N>(tw, k));
+    for (int k = 1; k < E; ++k) v[k] = cmul(v[k], tw_get(tw, k));
     sync();  // earlier readers of sm are done
 #pragma unroll
     for (int k = 0; k < E; ++k) sm[k * LD + j] = v[k];
@@ -174,6 +266,7 @@ __device__ __forceinline__ void fft_line(float2 (&v)[FftCfg<N>::E], float2 *sm, 
         dft_reg<T>(w);  // over n1: X[E*k1 + (j + T*c)] = X[j + T*(C*k1 + c)]
 #pragma unroll
         for (int k1 = 0; k1 < T; ++k1) v[C * k1 + c] = w[k1];
+    }
     }
 }
 

@@ -5,6 +5,7 @@
 #include "pd_resident.cuh"
 #include "pd_resident_tm.cuh"
 #include "pd_streaming_fd.cuh"
+#include "pd_streaming_gen.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -31,6 +32,16 @@ int cuda_fail(cudaError_t e, const char *where) {
     } while (0)
 
 bool size_ok(int n) { return n == 64 || n == 128 || n == 256 || n == 512; }
+// sizes of the general-length streaming kernels (pd_streaming_gen.cuh): any even length; the paper's are 258 and 132
+bool gen_size_ok(int n) { return n >= 4 && n <= 1024 && (n % 2) == 0; }
+// most balanced factorisation n = n1 * n2, n1 <= n2 (n1 = 1 for a prime: one dense stage)
+void balanced_factors(int n, int *n1, int *n2) {
+    int best = 1;
+    for (int f = 1; f * f <= n; ++f)
+        if (n % f == 0) best = f;
+    *n1 = best;
+    *n2 = n / best;
+}
 
 constexpr double kNormBound = 4.0 / 9.0 + 8.0;  // ||K_full||^2 <= max|D|^2 + ||G||^2 = 4/9 + 8 for W = M = 1
 
@@ -43,12 +54,18 @@ struct pd_plan_s {
     // user-facing parameters (as given) and the effective ones of the rescaled problem (R2)
     float lambda_user, sigma_user, tau_user, theta;
     int tv_mode, lambda_conv, variant, check_every, mask_shared, unsafe_steps, no_fd;
+    int generic;           // a size that is not a power of two: general-length kernels (pd_streaming_gen.cuh), literal iteration
+    pdk::GenDims gdims;
+    int reg_l1;            // PD_OPT_REGULARISER = PD_REG_L1
+    int use_angle;         // oblique in-plane B0 (pd_set_b0_angle)
+    double b0_angle;
     const float *weight;
     // device tables and workspace
     float *Dtab;
     float2 *tw_row, *tw_col;
     int *stop_iter, *iters_done;
     float *P0, *relgap, *relres;
+    float *cscale;         // [batch] power-of-two normalisation of every slice (streaming variant; pair_scale)
     int nparts;
     // resident variant (pd_resident.cuh): per-cluster scratch, kResidentScratchArrays arrays of nx*ny float2 per cluster
     int res_ok;            // this size has a resident kernel
@@ -133,20 +150,30 @@ void effective_params(const pd_plan_s *p, float *alpha, float *sigma, float *tau
     }
 }
 
-void build_dipole(std::vector<float> &D, int nx, int ny, int b0_dir) {
+void build_dipole(std::vector<float> &D, int nx, int ny, int b0_dir, bool use_angle = false, double angle = 0.0) {
     // D(kx,ky) = 1/3 - k_b^2/(kx^2+ky^2), D(0,0)=0, kx = fi/nx, ky = fj/ny (BASELINE.json north_star; R6);
-    // the 1/(nx*ny) of the inverse transform is folded in.
+    // the 1/(nx*ny) of the inverse transform is folded in.  k_b = ky (PD_B0_Y), kx (PD_B0_X), or k . (cos a, sin a) for an
+    // oblique in-plane B0 (pd_set_b0_angle).  K is defined as the REAL part of F^-1 D F (R12), i.e. only the even part of D
+    // acts on a real image; for an oblique B0 the table is not even on the Nyquist lines (index n/2 stands for -n/2), so
+    // the even part (D(k) + D(-k))/2 is what is stored -- which is also what lets two real slices ride one complex
+    // transform.
     const double scale = 1.0 / ((double)nx * (double)ny);
+    const double bx = std::cos(angle), by = std::sin(angle);
+    std::vector<double> d2((size_t)nx * ny);
     for (int jy = 0; jy < ny; ++jy) {
-        const double ky = (double)(jy < ny / 2 ? jy : jy - ny) / (double)ny;
+        const double ky = (double)(jy < (ny + 1) / 2 ? jy : jy - ny) / (double)ny;
         for (int ix = 0; ix < nx; ++ix) {
-            const double kx = (double)(ix < nx / 2 ? ix : ix - nx) / (double)nx;
+            const double kx = (double)(ix < (nx + 1) / 2 ? ix : ix - nx) / (double)nx;
             const double k2 = kx * kx + ky * ky;
-            const double kb = (b0_dir == PD_B0_Y) ? ky : kx;
-            const double d = (ix == 0 && jy == 0) ? 0.0 : 1.0 / 3.0 - kb * kb / k2;
-            D[(size_t)jy * nx + ix] = (float)(d * scale);
+            const double kb = use_angle ? kx * bx + ky * by : (b0_dir == PD_B0_Y) ? ky : kx;
+            d2[(size_t)jy * nx + ix] = (ix == 0 && jy == 0) ? 0.0 : 1.0 / 3.0 - kb * kb / k2;
         }
     }
+    for (int jy = 0; jy < ny; ++jy)
+        for (int ix = 0; ix < nx; ++ix) {
+            const size_t i = (size_t)jy * nx + ix, im = (size_t)((ny - jy) % ny) * nx + (size_t)((nx - ix) % nx);
+            D[i] = (float)(0.5 * (d2[i] + d2[im]) * scale);
+        }
 }
 
 void build_twiddles(std::vector<float2> &tw, int n) {
@@ -232,11 +259,11 @@ cudaError_t resident_launch(const ResidentArgs &a, bool w, bool aniso, int nclus
 }
 
 // ---- resident kernel with the state on chip (W = identity; pd_resident_tm.cuh): same cluster shape
-template <int N, bool ANISO>
+template <int N, int MODE>
 cudaError_t resident_tm_launch2(const ResidentTmArgs &a, int nclusters, cudaStream_t st) {
     using Ch = ResChoice<N>;
     using TCfg = pdk::ResTmCfg<N, Ch::C, Ch::NT>;
-    auto kern = pdk::resident_tm_kernel<N, Ch::C, Ch::NT, ANISO>;
+    auto kern = pdk::resident_tm_kernel<N, Ch::C, Ch::NT, MODE>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, TCfg::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     if (Ch::C > 8) {
@@ -259,8 +286,10 @@ cudaError_t resident_tm_launch2(const ResidentTmArgs &a, int nclusters, cudaStre
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 template <int N>
-cudaError_t resident_tm_launch(const ResidentTmArgs &a, bool aniso, int nclusters, cudaStream_t st) {
-    return aniso ? resident_tm_launch2<N, true>(a, nclusters, st) : resident_tm_launch2<N, false>(a, nclusters, st);
+cudaError_t resident_tm_launch(const ResidentTmArgs &a, int mode, int nclusters, cudaStream_t st) {
+    return mode == pdk::kModeL1 ? resident_tm_launch2<N, pdk::kModeL1>(a, nclusters, st)
+         : mode == pdk::kModeAniso ? resident_tm_launch2<N, pdk::kModeAniso>(a, nclusters, st)
+                                   : resident_tm_launch2<N, pdk::kModeIso>(a, nclusters, st);
 }
 
 // D/(N*N) in the order the column phase of resident_tm_kernel reads it: [rank][m][tid] (pd_resident_tm.cuh)
@@ -289,7 +318,7 @@ int ensure_sfd_workspace(pd_plan_s *p, size_t npairs) {
     if (p->sfd_planes) { cudaFree(p->sfd_planes); p->sfd_planes = nullptr; }
     if (p->sfd_parts) { cudaFree(p->sfd_parts); p->sfd_parts = nullptr; }
     const size_t PP = (size_t)p->nx * p->ny * npairs;
-    p->sfd_ncolparts = p->nx / 16;
+    p->sfd_ncolparts = p->generic ? p->nparts : p->nx / 16;
     p->sfd_nrowparts = p->nparts;
     int rc;
     if ((rc = dev_alloc(&p->sfd_planes, PP * kSfdPlanes)) != PD_OK) return rc;
@@ -313,6 +342,11 @@ template <int NX> void sfd_launch_init_rows(const StreamFdArgs &a, cudaStream_t 
 }
 template <int NX> void sfd_launch_rows(const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid(a.ny / pdk::SfdRowCfg<NX>::G, a.npairs);
+    if (a.reg_l1) {
+        if (a.mask) pdk::sfd_rows_l1_kernel<NX, true><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+        else pdk::sfd_rows_l1_kernel<NX, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+        return;
+    }
     if (a.mask) pdk::sfd_rows_kernel<NX, true><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
     else pdk::sfd_rows_kernel<NX, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
 }
@@ -342,6 +376,28 @@ cudaError_t sfd_set_col_smem() {
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(pdk::sfd_init_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 pdk::SfdColCfg<NY>::SMEM_BYTES);
+}
+
+// (Re)build the dipole tables of the plan -- D/(nx ny) in [ny][nx] order and, for the resident kernel with the state on
+// chip, in its thread-private order -- and upload them.  Synchronous (plan time, pd_set_b0_angle).
+int upload_dipole(pd_plan_s *p) {
+    const size_t P = (size_t)p->nx * p->ny;
+    std::vector<float> D(P), Dp;
+    build_dipole(D, p->nx, p->ny, p->b0_dir, p->use_angle != 0, p->b0_angle);
+    PD_CUDA(cudaMemcpy(p->Dtab, D.data(), P * sizeof(float), cudaMemcpyHostToDevice));
+    if (p->Dpriv) {
+        if (p->nx == 64) build_dipole_private<64>(Dp, D);
+        else if (p->nx == 128) build_dipole_private<128>(Dp, D);
+        else build_dipole_private<256>(Dp, D);
+        PD_CUDA(cudaMemcpy(p->Dpriv, Dp.data(), P * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    return PD_OK;
+}
+
+// The resident variant runs this plan's next solve: the size has a resident kernel, streaming is not forced, and the
+// combination l1 regulariser + (W set or PD_OPT_FOURIER_DUAL = 0) -- which only the streaming kernels implement -- is not asked for
+bool use_resident(const pd_plan_s *p) {
+    return p->res_ok && p->variant != PD_VARIANT_STREAMING && !(p->reg_l1 && (p->weight || p->no_fd));
 }
 
 int resident_csize(int n) { return n == 64 ? ResChoice<64>::C : n == 128 ? ResChoice<128>::C : ResChoice<256>::C; }
@@ -413,10 +469,11 @@ cudaError_t launch_resident(pd_plan_s *p, const float *field, const float *mask,
         f.Z = a.Z; f.M2 = a.M2;
         f.Dpriv = p->Dpriv; f.tw_tab = p->tw_row; f.part = p->rk_part;
         f.iters_done = a.iters_done; f.relgap = a.relgap; f.relres = a.relres;
+        const int mode = p->reg_l1 ? pdk::kModeL1 : aniso ? pdk::kModeAniso : pdk::kModeIso;
         switch (p->nx) {
-            case 64: return resident_tm_launch<64>(f, aniso, nclusters, st);
-            case 128: return resident_tm_launch<128>(f, aniso, nclusters, st);
-            default: return resident_tm_launch<256>(f, aniso, nclusters, st);
+            case 64: return resident_tm_launch<64>(f, mode, nclusters, st);
+            case 128: return resident_tm_launch<128>(f, mode, nclusters, st);
+            default: return resident_tm_launch<256>(f, mode, nclusters, st);
         }
     }
     switch (p->nx) {
@@ -526,7 +583,7 @@ int solve_resident(pd_plan_s *p, const float *field, const float *mask, float *c
 
 int solve_range(pd_plan_s *p, const float *field, const float *mask, float *chi_out, int max_iters, float tol,
                 cudaStream_t st, int first, int count) {
-    if (p->res_ok && p->variant != PD_VARIANT_STREAMING) return solve_resident(p, field, mask, chi_out, max_iters, tol, st, first, count);
+    if (use_resident(p)) return solve_resident(p, field, mask, chi_out, max_iters, tol, st, first, count);
     int launches = 0;
     const int rc = solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, st, first, &launches, count);
     p->last_launches += launches;
@@ -554,7 +611,37 @@ int solve_range(pd_plan_s *p, const float *field, const float *mask, float *chi_
     } while (0)
 
 // The iteration kernels of one PD iteration (n < 0: inside the graphed loop, the kernels read the device counter)
+size_t gen_rows_smem(const pd_plan_s *p) { return (size_t)(1 + 2 * pdk::kGenRows) * p->nx * sizeof(float2); }
+size_t gen_cols_smem(const pd_plan_s *p) { return (size_t)(1 + 2 * pdk::kGenColsB) * p->ny * sizeof(float2); }
+void gen_launch_cols(const pd_plan_s *p, const StreamFdArgs &a, int n, int decide, cudaStream_t st) {
+    dim3 grid((a.nx + pdk::kGenColsB - 1) / pdk::kGenColsB, a.npairs);
+    pdk::gen_cols_kernel<<<grid, 32 * pdk::kGenColsB, gen_cols_smem(p), st>>>(a, p->gdims, n, decide);
+}
+void gen_launch_dual_rows(const pd_plan_s *p, const StreamFdArgs &a, int n, cudaStream_t st) {
+    dim3 grid((a.ny + pdk::kGenRows - 1) / pdk::kGenRows, a.npairs);
+    pdk::gen_dual_rows_kernel<<<grid, 32 * pdk::kGenRows, gen_rows_smem(p), st>>>(a, p->gdims, n);
+}
+void gen_launch_rows(const pd_plan_s *p, const StreamFdArgs &a, int n, cudaStream_t st) {
+    dim3 grid((a.ny + pdk::kGenRows - 1) / pdk::kGenRows, a.npairs);
+    pdk::gen_rows_kernel<<<grid, 32 * pdk::kGenRows, gen_rows_smem(p), st>>>(a, p->gdims, n);
+}
+void gen_launch_init(const pd_plan_s *p, const StreamFdArgs &a, int which, cudaStream_t st) {
+    if (which == 0) {
+        dim3 grid((a.ny + pdk::kGenRows - 1) / pdk::kGenRows, a.npairs);
+        pdk::gen_init_kernel<<<grid, 32 * pdk::kGenRows, 0, st>>>(a);
+    } else {
+        pdk::gen_init_finish_kernel<<<(a.batch + 127) / 128, 128, 0, st>>>(a);
+    }
+}
+
 void sfd_enqueue_iteration(const pd_plan_s *p, const StreamFdArgs &a, bool literal, int n, cudaStream_t st) {
+    if (p->generic) {   // general-length kernels, literal iteration
+        if (n != 0) gen_launch_cols(p, a, n, 1, st);
+        gen_launch_dual_rows(p, a, n, st);
+        gen_launch_cols(p, a, n, 0, st);
+        gen_launch_rows(p, a, n, st);
+        return;
+    }
     if (literal) {
         if (n != 0) { PD_DISPATCH(p->ny, sfd_launch_cols_plain, a, n, 1, st); }   // K1 (chibar_0 = 0; in the loop the kernel skips n = 0 itself)
         PD_DISPATCH(p->nx, sfd_launch_dual_rows, a, n, st);
@@ -572,7 +659,7 @@ void graph_slot_release(pd_plan_s::GraphSlot &g) {
 }
 
 // Build (or reuse) the executable graph of one streaming solve with arguments `a`:
-//   memset(iter) -> init_rows -> init_cols -> WHILE (handle) { iteration kernels ; sfd_loop_ctl } -> finish
+//   memset(iter) -> scale -> init_rows -> init_cols -> WHILE (handle) { iteration kernels ; sfd_loop_ctl } -> finish
 // The WHILE node's handle is set on the device by sfd_loop_ctl: when every slice has stopped (or n = max_iters) the
 // body is not launched again -- no no-op launches, no host round trip.
 int sfd_graph_prepare(pd_plan_s *p, StreamFdArgs &a, bool literal, int *slot_out) {
@@ -600,8 +687,14 @@ int sfd_graph_prepare(pd_plan_s *p, StreamFdArgs &a, bool literal, int *slot_out
     // prologue
     PD_CUDA(cudaStreamBeginCaptureToGraph(cs, g.graph, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
     cudaError_t e = cudaMemsetAsync(a.iter, 0, sizeof(int), cs);
-    PD_DISPATCH(p->nx, sfd_launch_init_rows, a, cs);
-    PD_DISPATCH(p->ny, sfd_launch_init_cols, a, cs);
+    pdk::sfd_scale_kernel<<<a.batch, 256, 0, cs>>>(a);
+    if (p->generic) {
+        gen_launch_init(p, a, 0, cs);
+        gen_launch_init(p, a, 1, cs);
+    } else {
+        PD_DISPATCH(p->nx, sfd_launch_init_rows, a, cs);
+        PD_DISPATCH(p->ny, sfd_launch_init_cols, a, cs);
+    }
     cudaStreamCaptureStatus status;
     const cudaGraphNode_t *deps = nullptr;
     size_t ndeps = 0;
@@ -660,8 +753,9 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
     a.tol = tol;
     a.mask_bstride = p->mask_shared ? 0 : (long long)P;
-    const bool literal = p->weight != nullptr || p->no_fd;   // p in the image domain, K applied twice (PAPER.md:49 literally)
+    const bool literal = p->weight != nullptr || p->no_fd || p->generic;   // p in the image domain, K applied twice (PAPER.md:49 literally)
     a.literal = literal ? 1 : 0;
+    a.reg_l1 = p->reg_l1;
     a.weight = p->weight ? p->weight + (size_t)first * P : nullptr;
     a.field = field + (size_t)first * P;
     a.mask = mask ? mask + (size_t)first * (size_t)a.mask_bstride : nullptr;
@@ -674,6 +768,7 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     a.Dtab = p->Dtab; a.tw_row = p->tw_row; a.tw_col = p->tw_col;
     a.stop_iter = p->stop_iter + first; a.P0 = p->P0 + first; a.relgap = p->relgap + first;
     a.relres = p->relres + first; a.iters_done = p->iters_done + first;
+    a.cscale = p->cscale + first;
     a.nrowparts = p->sfd_nrowparts;
     a.ncolparts = literal ? p->sfd_nrowparts : p->sfd_ncolparts;   // who writes the data term of the gap
     const size_t nr = (size_t)np * a.nrowparts, nc = (size_t)np * (size_t)(p->sfd_ncolparts > p->sfd_nrowparts ? p->sfd_ncolparts : p->sfd_nrowparts);
@@ -695,9 +790,22 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
         if (launches_out) *launches_out = 0; else p->last_launches = 0;
         return PD_OK;
     }
-    PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->nx, sfd_launch_init_rows, a, st));
-    PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->ny, sfd_launch_init_cols, a, st));
+    PD_LAUNCH(PD_KERNEL_INIT, (pdk::sfd_scale_kernel<<<a.batch, 256, 0, st>>>(a)));
+    if (p->generic) {
+        PD_LAUNCH(PD_KERNEL_INIT, gen_launch_init(p, a, 0, st));
+        PD_LAUNCH(PD_KERNEL_INIT, gen_launch_init(p, a, 1, st));
+    } else {
+        PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->nx, sfd_launch_init_rows, a, st));
+        PD_LAUNCH(PD_KERNEL_INIT, PD_DISPATCH(p->ny, sfd_launch_init_cols, a, st));
+    }
     for (int n = 0; n < max_iters; ++n) {
+        if (p->generic) {
+            if (n > 0) PD_LAUNCH(PD_KERNEL_COLS, gen_launch_cols(p, a, n, 1, st));
+            PD_LAUNCH(PD_KERNEL_DUAL, gen_launch_dual_rows(p, a, n, st));
+            PD_LAUNCH(PD_KERNEL_COLS, gen_launch_cols(p, a, n, 0, st));
+            PD_LAUNCH(PD_KERNEL_FD_ROWS, gen_launch_rows(p, a, n, st));
+            continue;
+        }
         if (literal) {
             if (n > 0) PD_LAUNCH(PD_KERNEL_COLS, PD_DISPATCH(p->ny, sfd_launch_cols_plain, a, n, 1, st));   // K1 (chibar_0 = 0)
             PD_LAUNCH(PD_KERNEL_DUAL, PD_DISPATCH(p->nx, sfd_launch_dual_rows, a, n, st));
@@ -724,7 +832,8 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     if (!out) return PD_EINVAL;
     *out = nullptr;
     if (batch < 1 || (B0_dir != PD_B0_X && B0_dir != PD_B0_Y)) return PD_EINVAL;
-    if (!size_ok(nx) || !size_ok(ny)) return PD_ESIZE;
+    const bool generic = !(size_ok(nx) && size_ok(ny));
+    if (generic && !(gen_size_ok(nx) && gen_size_ok(ny))) return PD_ESIZE;
     int rc = check_params(lambda, sigma, tau, theta, false);
     if (rc != PD_OK) return rc;
 
@@ -744,8 +853,12 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
         if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "cudaGetDevice"); }
     }
-    const int rows_per_cta = (nx == 64 || nx == 128) ? 16 : 8;  // = SfdRowCfg<nx>::G
-    p->nparts = ny / rows_per_cta;
+    p->generic = generic ? 1 : 0;
+    balanced_factors(nx, &p->gdims.n1x, &p->gdims.n2x);
+    balanced_factors(ny, &p->gdims.n1y, &p->gdims.n2y);
+    const int rows_per_cta = generic ? pdk::kGenRows : nx == 64 ? pdk::SfdRowCfg<64>::G : nx == 128 ? pdk::SfdRowCfg<128>::G
+                           : nx == 256 ? pdk::SfdRowCfg<256>::G : pdk::SfdRowCfg<512>::G;
+    p->nparts = (ny + rows_per_cta - 1) / rows_per_cta;
 
     const size_t P = (size_t)nx * ny;
 #define PD_TRY(expr) do { rc = (expr); if (rc != PD_OK) { pd_destroy(p); return rc; } } while (0)
@@ -757,15 +870,14 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     PD_TRY(dev_alloc(&p->P0, (size_t)batch));
     PD_TRY(dev_alloc(&p->relgap, (size_t)batch));
     PD_TRY(dev_alloc(&p->relres, (size_t)batch));
+    PD_TRY(dev_alloc(&p->cscale, (size_t)batch + 1));
 #undef PD_TRY
     {
-        std::vector<float> D(P);
-        build_dipole(D, nx, ny, B0_dir);
         std::vector<float2> twr(nx), twc(ny);
         build_twiddles(twr, nx);
         build_twiddles(twc, ny);
-        cudaError_t e = cudaMemcpy(p->Dtab, D.data(), P * sizeof(float), cudaMemcpyHostToDevice);
-        if (e == cudaSuccess) e = cudaMemcpy(p->tw_row, twr.data(), nx * sizeof(float2), cudaMemcpyHostToDevice);
+        if ((rc = upload_dipole(p)) != PD_OK) { pd_destroy(p); return rc; }
+        cudaError_t e = cudaMemcpy(p->tw_row, twr.data(), nx * sizeof(float2), cudaMemcpyHostToDevice);
         if (e == cudaSuccess) e = cudaMemcpy(p->tw_col, twc.data(), ny * sizeof(float2), cudaMemcpyHostToDevice);
         if (e == cudaSuccess) e = cudaMemset(p->iters_done, 0, batch * sizeof(int));
         if (e == cudaSuccess) e = cudaMemset(p->relgap, 0, batch * sizeof(float));
@@ -774,10 +886,17 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (e == cudaSuccess) e = sfd_set_col_smem<128>();
         if (e == cudaSuccess) e = sfd_set_col_smem<256>();
         if (e == cudaSuccess) e = sfd_set_col_smem<512>();
+        if (e == cudaSuccess && generic) {
+            // the attribute belongs to the function, not to the plan: always the largest supported length (1024)
+            const int cmax = (1 + 2 * pdk::kGenColsB) * 1024 * (int)sizeof(float2), rmax = (1 + 2 * pdk::kGenRows) * 1024 * (int)sizeof(float2);
+            e = cudaFuncSetAttribute(pdk::gen_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, cmax);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(pdk::gen_dual_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rmax);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(pdk::gen_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rmax);
+        }
         if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "plan table upload"); }
     }
     // resident variant: square slices up to 256x256
-    if (nx == ny && nx <= 256) {
+    if (!generic && nx == ny && nx <= 256) {
         int maxc = 0;
         rc = (nx == 64) ? resident_max_clusters<64>(&maxc) : (nx == 128) ? resident_max_clusters<128>(&maxc)
                                                                           : resident_max_clusters<256>(&maxc);
@@ -790,15 +909,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
             if (rc != PD_OK) { pd_destroy(p); return rc; }
             if (rc == PD_OK) rc = dev_alloc(&p->Dpriv, P);
             if (rc != PD_OK) { pd_destroy(p); return rc; }
-            {
-                std::vector<float> D(P), Dp;
-                build_dipole(D, nx, ny, B0_dir);
-                if (nx == 64) build_dipole_private<64>(Dp, D);
-                else if (nx == 128) build_dipole_private<128>(Dp, D);
-                else build_dipole_private<256>(Dp, D);
-                cudaError_t e2 = cudaMemcpy(p->Dpriv, Dp.data(), P * sizeof(float), cudaMemcpyHostToDevice);
-                if (e2 != cudaSuccess) { pd_destroy(p); return cuda_fail(e2, "private dipole table upload"); }
-            }
+            if ((rc = upload_dipole(p)) != PD_OK) { pd_destroy(p); return rc; }
             cudaError_t e = cudaMemset(p->rk_part, 0, (size_t)p->res_clusters * p->res_csize * 8 * sizeof(float));
             if (e != cudaSuccess) { pd_destroy(p); return cuda_fail(e, "resident scratch init"); }
             p->res_ok = 1;
@@ -831,6 +942,14 @@ int pd_set_weight(pd_plan_t p, const float *W) {
     if (!p) return PD_EINVAL;
     p->weight = W;
     return PD_OK;
+}
+
+int pd_set_b0_angle(pd_plan_t p, float angle_rad) {
+    if (!p || !std::isfinite(angle_rad)) return PD_EINVAL;
+    PD_CUDA(cudaDeviceSynchronize());   // no solve of this plan may still be reading the tables
+    p->use_angle = 1;
+    p->b0_angle = (double)angle_rad;
+    return upload_dipole(p);
 }
 
 int pd_set_steps(pd_plan_t p, float lambda, float sigma, float tau, float theta) {
@@ -873,6 +992,9 @@ int pd_set_option(pd_plan_t p, int key, int value) {
         case PD_OPT_HYBRID_TAIL:
             if (value < -1) return PD_EINVAL;
             p->hybrid_tail = value; return PD_OK;
+        case PD_OPT_REGULARISER:
+            if (value != PD_REG_TV && value != PD_REG_L1) return PD_EINVAL;
+            p->reg_l1 = (value == PD_REG_L1); return PD_OK;
         case PD_OPT_GRAPH_LOOP:
             if (value != 0 && value != 1) return PD_EINVAL;
             p->graph_loop = value; return PD_OK;
@@ -887,7 +1009,7 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
     cudaStream_t st = (cudaStream_t)cuda_stream;
     p->last_launches = 0;
     p->graph_used = 0u;
-    if (p->res_ok && p->variant != PD_VARIANT_STREAMING) return solve_resident(p, field, mask, chi_out, max_iters, tol, st);
+    if (use_resident(p)) return solve_resident(p, field, mask, chi_out, max_iters, tol, st);
     return solve_streaming_fd(p, field, mask, chi_out, max_iters, tol, st);
 }
 
@@ -898,7 +1020,7 @@ int pd_solve(pd_plan_t p, const float *field, const float *mask, float *chi_out,
 // its upload, so the chunks grow 1, 4, rest and shrink 4, 2.  Streaming variant: a small chunk cannot fill the GPU with
 // its launches, so three chunks of 1/8, 6/8, 1/8 of the batch (measured on C4: five chunks lose more than they hide).
 int host_chunks(const pd_plan_s *p, int *count /*[kMaxChunks]*/) {
-    const bool res = p->res_ok && p->variant != PD_VARIANT_STREAMING;
+    const bool res = use_resident(p);
     int unit = res ? p->res_max_clusters : (p->npairs + 7) / 8;   // pairs
     if (unit < 1) unit = 1;
     const int np = p->npairs;
@@ -942,7 +1064,7 @@ int pd_solve_host(pd_plan_t p, const float *field_host, const float *mask_host, 
         size_t need = 0;
         for (int k = 0; k < nchunks; ++k) {
             const int np = (count[k] + 1) / 2;
-            const bool res = p->res_ok && p->variant != PD_VARIANT_STREAMING;
+            const bool res = use_resident(p);
             const size_t t = res ? (size_t)hybrid_tail_pairs(p, np, nchunks == 1) : (size_t)np;
             need = t > need ? t : need;
         }
@@ -972,7 +1094,7 @@ int pd_solve_host(pd_plan_t p, const float *field_host, const float *mask_host, 
         const size_t off = (size_t)first * P, nby = (size_t)count[k] * P * sizeof(float);
         PD_CUDA(cudaStreamWaitEvent(st, ev_up[k], 0));
         if (nchunks == 1) {
-            rc = (p->res_ok && p->variant != PD_VARIANT_STREAMING)
+            rc = (use_resident(p))
                      ? solve_resident(p, p->h_field, mask_host ? p->h_mask : nullptr, p->h_chi, max_iters, tol, st)
                      : solve_streaming_fd(p, p->h_field, mask_host ? p->h_mask : nullptr, p->h_chi, max_iters, tol, st);
         } else {
@@ -1038,7 +1160,7 @@ int pd_last_launch_count(pd_plan_t p) {
             if (!(p->graph_used & (1u << k))) continue;
             int iters = 0;
             if (cudaMemcpy(&iters, p->gslot[k].iter, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return PD_ECUDA;
-            n += 3 + iters * (p->gslot[k].literal ? 5 : 3);   // init rows + cols, finish ; per iteration its kernels + loop control
+            n += 4 + iters * (p->gslot[k].literal ? 5 : 3);   // scale, init rows + cols, finish ; per iteration its kernels + loop control
         }
     }
     return n;
@@ -1046,7 +1168,7 @@ int pd_last_launch_count(pd_plan_t p) {
 
 int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
     if (!p) return PD_EINVAL;
-    const bool res = p->res_ok && p->variant != PD_VARIANT_STREAMING;
+    const bool res = use_resident(p);
     if (variant) *variant = res ? PD_VARIANT_RESIDENT : PD_VARIANT_STREAMING;
     if (clusters) *clusters = res ? p->res_clusters : 0;
     if (cluster_size) *cluster_size = res ? p->res_csize : 0;
@@ -1063,14 +1185,14 @@ int pd_get_hybrid_rho(pd_plan_t p, float *rho) {
 
 int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs) {
     if (!p || !tail_pairs) return PD_EINVAL;
-    *tail_pairs = (p->res_ok && p->variant != PD_VARIANT_STREAMING) ? hybrid_tail_pairs(p) : 0;
+    *tail_pairs = (use_resident(p)) ? hybrid_tail_pairs(p) : 0;
     return PD_OK;
 }
 
 int pd_destroy(pd_plan_t p) {
     if (!p) return PD_EINVAL;
     void *ptrs[] = {p->Dtab, p->tw_row, p->tw_col, p->stop_iter, p->iters_done,
-                    p->P0, p->relgap, p->relres, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part, p->Dpriv,
+                    p->P0, p->relgap, p->relres, p->cscale, p->h_field, p->h_mask, p->h_chi, p->res_scratch, p->rk_part, p->Dpriv,
                     p->sfd_planes, p->sfd_parts};
     for (void *q : ptrs)
         if (q) cudaFree(q);
@@ -1097,7 +1219,7 @@ const char *pd_strerror(int code) {
     switch (code) {
         case PD_OK: return "success";
         case PD_EINVAL: return "invalid argument";
-        case PD_ESIZE: return "nx and ny must each be one of 64, 128, 256, 512";
+        case PD_ESIZE: return "nx and ny must each be one of 64, 128, 256, 512 (tuned kernels) or both even and in [4, 1024] (general-length kernels)";
         case PD_ESTEP: return "sigma*tau*(4/9+8) >= 1: step sizes violate the convergence bound";
         case PD_ENOMEM: return "out of device memory";
         case PD_ECUDA: return g_cuda_err;

@@ -84,12 +84,46 @@ __device__ __forceinline__ float2 splat(float s) { return make_float2(s, s); }
 __device__ __forceinline__ float2 shfl2(float2 v, int src, int width) {
     return make_float2(__shfl_sync(0xffffffffu, v.x, src, width), __shfl_sync(0xffffffffu, v.y, src, width));
 }
-__device__ __forceinline__ float sqrt_approx(float x) {
-    float r;
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
 __device__ __forceinline__ float2 ldcg2(const float2 *p) { return __ldcg(p); }
+
+// alpha / |t| for the isotropic projection, n2 = |t|^2 (PAPER.md:49 line 2; R17).  FAST = false: IEEE square root and
+// division.  FAST = true: alpha * rsqrt(n2) and sqrt.approx with the hardware approximations (2 ulp, denormals flushed).
+// Which kernels use which, and the measured difference: DESIGN.md R17, profiles/r02/README.md.
+#ifndef PD_RESIDENT_FAST_PROJECTION
+#define PD_RESIDENT_FAST_PROJECTION 1
+#endif
+#ifndef PD_STREAMING_FAST_PROJECTION
+#define PD_STREAMING_FAST_PROJECTION 1
+#endif
+constexpr bool kResidentFastProj = PD_RESIDENT_FAST_PROJECTION != 0, kStreamingFastProj = PD_STREAMING_FAST_PROJECTION != 0;
+template <bool FAST>
+__device__ __forceinline__ float proj_scale(const float alpha, const float n2) {
+    if constexpr (FAST) return alpha * rsqrtf(n2);
+    else return __fdiv_rn(alpha, __fsqrt_rn(n2));
+}
+template <bool FAST>
+__device__ __forceinline__ float gap_sqrt(const float x) {
+    if constexpr (FAST) {
+        float r;
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    } else {
+        return __fsqrt_rn(x);
+    }
+}
+
+// Per-slice normalisation: two real slices ride one complex transform, and the twiddle
+// multiplications mix the lanes' rounding errors, so a weak slice would inherit the absolute error of a strong partner.
+// Every slice is therefore scaled by a power of two c = 2^-e that brings its r.m.s. field into [1, 2).  The iteration is
+// exactly invariant under (phi, alpha) -> (c phi, c alpha) -- chi, p, q scale by c -- and a power of two is exact in
+// floating point, so a slice's result does not depend on c; chi is multiplied by 1/c when it is stored.
+// `sumsq` = sum of phi^2 over the slice's `npix` pixels.
+__device__ __forceinline__ float pair_scale(const float sumsq, const float npix) {
+    if (!(sumsq > 0.f) || !(sumsq < 3.0e38f)) return 1.f;
+    int e = ilogbf(sumsq / npix) >> 1;   // floor(log2(rms))
+    e = e < -60 ? -60 : (e > 60 ? 60 : e);
+    return ldexpf(1.f, -e);
+}
 
 template <int N, int C, int NT>
 struct ResCfg {
@@ -140,12 +174,12 @@ struct RowPtrs {
 // ------------------------------------------------------------------------------------------------ q-update
 // q_{n+1} = proj_alpha(q_n + sigma M G chibar_n)   (PAPER.md:49 line 2; R4, R7).  Independent of the spectrum.
 template <int N, int NT, bool ANISO>
-__device__ __forceinline__ void q_update_row(const RowPtrs &r, const ResidentArgs &a, const int y, const int j,
-                                             const bool want_gap, float2 &gap) {
+__device__ __forceinline__ void q_update_row(const RowPtrs &r, const ResidentArgs &a, const float2 alpha, const int y,
+                                             const int j, const bool want_gap, float2 &gap) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
     const bool has_down = y < N - 1;
     const float2 sig2 = splat(a.sigma);
-    const float alpha = a.alpha, alpha_sq = a.alpha * a.alpha;
+    const float2 alpha_sq = mul2(alpha, alpha);   // alpha is per lane: every slice runs in its own normalisation (pair_scale)
     float2 c0[E];
 #pragma unroll
     for (int m = 0; m < E; ++m) c0[m] = ldcg2(r.chibar + j + T * m);
@@ -175,15 +209,15 @@ __device__ __forceinline__ void q_update_row(const RowPtrs &r, const ResidentArg
         float2 tx = fma2(sig2, gx, r.qx_s[m * NT]);
         float2 ty = fma2(sig2, gy, qyv[m % CH]);
         if (ANISO) {
-            tx.x = fminf(fmaxf(tx.x, -alpha), alpha);
-            tx.y = fminf(fmaxf(tx.y, -alpha), alpha);
-            ty.x = fminf(fmaxf(ty.x, -alpha), alpha);
-            ty.y = fminf(fmaxf(ty.y, -alpha), alpha);
+            tx.x = fminf(fmaxf(tx.x, -alpha.x), alpha.x);
+            tx.y = fminf(fmaxf(tx.y, -alpha.y), alpha.y);
+            ty.x = fminf(fmaxf(ty.x, -alpha.x), alpha.x);
+            ty.y = fminf(fmaxf(ty.y, -alpha.y), alpha.y);
         } else {
             const float2 n2 = fma2(ty, ty, mul2(tx, tx));
             float2 sc;
-            sc.x = (n2.x > alpha_sq) ? alpha * rsqrtf(n2.x) : 1.f;  // alpha/|t| where |t| > alpha, else 1 (R13: alpha=0 -> 0)
-            sc.y = (n2.y > alpha_sq) ? alpha * rsqrtf(n2.y) : 1.f;
+            sc.x = (n2.x > alpha_sq.x) ? proj_scale<kResidentFastProj>(alpha.x, n2.x) : 1.f;  // alpha/|t| where |t| > alpha, else 1 (R13: alpha=0 -> 0)
+            sc.y = (n2.y > alpha_sq.y) ? proj_scale<kResidentFastProj>(alpha.y, n2.y) : 1.f;
             tx = mul2(tx, sc);
             ty = mul2(ty, sc);
         }
@@ -195,10 +229,10 @@ __device__ __forceinline__ void q_update_row(const RowPtrs &r, const ResidentArg
                 gn = make_float2(fabsf(gx.x) + fabsf(gy.x), fabsf(gx.y) + fabsf(gy.y));
             } else {
                 const float2 g2 = fma2(gy, gy, mul2(gx, gx));
-                gn = make_float2(sqrt_approx(g2.x), sqrt_approx(g2.y));
+                gn = make_float2(gap_sqrt<kResidentFastProj>(g2.x), gap_sqrt<kResidentFastProj>(g2.y));
             }
             const float2 dot = fma2(gy, ty, mul2(gx, tx));
-            gap = add2(gap, sub2(mul2(splat(alpha), gn), dot));
+            gap = add2(gap, sub2(mul2(alpha, gn), dot));
         }
     }
 }
@@ -262,7 +296,7 @@ __device__ __forceinline__ void d_term_row(const RowPtrs &r, const int y, const 
 template <int N, int NT, int LDR, class Tw>
 __device__ __forceinline__ void primal_z_row(const RowPtrs &r, const ResidentArgs &a, const int j, float2 *smg,
                                              const Tw &tw, const float2 (&d)[FftCfg<N>::E], float *out_a, float *out_b,
-                                             float2 &dn, float2 &cn) {
+                                             const float2 out_scale, float2 &dn, float2 &cn) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
     float2 v[E];
 #pragma unroll
@@ -287,8 +321,8 @@ __device__ __forceinline__ void primal_z_row(const RowPtrs &r, const ResidentArg
         r.chi[x] = c_new;
         r.chibar[x] = cbar;
         v[m] = cbar;
-        if (out_a) out_a[x] = c_new.x;
-        if (out_b) out_b[x] = c_new.y;
+        if (out_a) out_a[x] = out_scale.x * c_new.x;   // back to the caller's units (exact: a power of two)
+        if (out_b) out_b[x] = out_scale.y * c_new.y;
     }
     fft_line<N, LDR>(v, smg, j, tw, WarpSync());
 #pragma unroll
@@ -398,7 +432,16 @@ resident_kernel(const ResidentArgs a) {
             dec[tid] = 0.5f * t;
         }
         __syncthreads();
-        const float P0a = dec[0], P0b = dec[1];
+        // normalisation of the two slices (pair_scale): phi (stored unscaled above) and P0 are rescaled, alpha per lane
+        const float ca = pair_scale(2.f * dec[0], (float)P), cb = pair_scale(2.f * dec[1], (float)P);
+        if (ca != 1.f || cb != 1.f) {
+            float2 *phs = a.phi2 + soff;
+            const float2 c2 = make_float2(ca, cb);
+            for (int i = tid; i < RPC * N; i += NT) phs[row0 * N + i] = mul2(c2, phs[row0 * N + i]);   // own writes, own reads
+        }
+        const float P0a = dec[0] * ca * ca, P0b = dec[1] * cb * cb;
+        const float2 alpha2 = make_float2(a.alpha * ca, a.alpha * cb);
+        const float inv_ca = 1.f / ca, inv_cb = 1.f / cb;
         // R13b: an all-zero slice is never scheduled (every iteration would be a no-op)
         int stop_a = (P0a == 0.f) ? 0 : a.max_iters;
         int stop_b = (!has_b || P0b == 0.f) ? 0 : a.max_iters;
@@ -415,7 +458,7 @@ resident_kernel(const ResidentArgs a) {
 
             // (1) q-update: needs only chibar_n and q_n, both complete since the barrier after the last primal step
             float2 gap = make_float2(0.f, 0.f);
-            q_update_row<N, NT, ANISO>(r, a, y, j, want_gap, gap);
+            q_update_row<N, NT, ANISO>(r, a, alpha2, y, j, want_gap, gap);
             if (n > 0) cluster_wait<C>();            // K1 column pass of all CTAs is complete
             // (2) dual step on the spectrum rows
             dual_z_row<N, NT, Cfg::LDR, HAS_W>(r, a, j, smg_row, tw_row, want_gap, gap);
@@ -446,7 +489,7 @@ resident_kernel(const ResidentArgs a) {
                 float *out_a = (act_a && n + 1 >= stop_a) ? a.chi_out + (long long)s0 * P + y * N : nullptr;
                 float *out_b = (act_b && n + 1 >= stop_b) ? a.chi_out + (long long)s1 * P + y * N : nullptr;
                 float2 dn = make_float2(0.f, 0.f), cn = make_float2(0.f, 0.f);
-                primal_z_row<N, NT, Cfg::LDR>(r, a, j, smg_row, tw_row, d, out_a, out_b, dn, cn);
+                primal_z_row<N, NT, Cfg::LDR>(r, a, j, smg_row, tw_row, d, out_a, out_b, make_float2(inv_ca, inv_cb), dn, cn);
                 if (out_a || out_b) {   // residual of the final iterate (reported, not used for stopping)
                     float acc[4] = {dn.x, cn.x, dn.y, cn.y};
                     const float t = block_sum<NT, 4>(acc, red);

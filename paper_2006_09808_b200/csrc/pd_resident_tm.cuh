@@ -37,6 +37,10 @@
 
 namespace pdk {
 
+// regulariser / projection of the kernel instance: the paper's TV term with the isotropic or anisotropic reading of |.|
+// (R4), or l1 on chi with a shrinkage prox (PD_REG_L1: no q-update, no divergence term)
+constexpr int kModeIso = 0, kModeAniso = 1, kModeL1 = 2;
+
 struct ResidentTmArgs {
     int batch, npairs, max_iters, check_every;
     float alpha, sigma, tau, theta, inv_one_plus_sigma, tol;
@@ -159,14 +163,14 @@ __device__ __forceinline__ void dual_tm_col(float2 *zc, const float *__restrict_
 
 // ------------------------------------------------------------------------------------------------ q-update
 // q_{n+1} = proj_alpha(q_n + sigma M G chibar_n)   (PAPER.md:49 line 2; R4, R7).  Independent of the spectrum.
-// The scale of the isotropic projection is min(1, alpha * rsqrt(|t|^2)) with the hardware reciprocal square root
-// (2 ulp; R17 gives the measured cost of the IEEE sqrt + division it replaces); |t| = 0 gives
+// The scale of the isotropic projection is min(1, alpha / |t|) (proj_scale: hardware reciprocal square root by default
+// in the resident kernels, R17 gives the measured cost of the IEEE sqrt + division it replaces); |t| = 0 gives
 // min(1, inf) = 1, and alpha = 0 gives 0 (or min(1, NaN) = 1 on a zero vector), so R13 holds without a branch.
 template <int N, int NT, bool ANISO>
-__device__ __forceinline__ void q_update_tm(const TmRow<N, NT> &r, const ResidentTmArgs &a, const int j,
+__device__ __forceinline__ void q_update_tm(const TmRow<N, NT> &r, const ResidentTmArgs &a, const float2 alpha, const int j,
                                             const bool want_gap, float2 &gap) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, CH = 8;
-    const float sigma = a.sigma, alpha = a.alpha;
+    const float sigma = a.sigma;   // alpha is per lane: every slice runs in its own normalisation (pair_scale)
     // chibar[y][x+1] is the next thread's slot of the same element, or (last thread of the row) the first thread's
     // slot of the next element: the same immediate offsets from a per-thread index
     const int cr_off = (j == T - 1) ? NT - T + 1 : 1;
@@ -203,13 +207,14 @@ __device__ __forceinline__ void q_update_tm(const TmRow<N, NT> &r, const Residen
             float2 tx = fma2(sm2, dx, qxv[k]);
             float2 ty = fma2(sm2, dy, qyv[k]);
             if (ANISO) {
-                tx.x = fminf(fmaxf(tx.x, -alpha), alpha);
-                tx.y = fminf(fmaxf(tx.y, -alpha), alpha);
-                ty.x = fminf(fmaxf(ty.x, -alpha), alpha);
-                ty.y = fminf(fmaxf(ty.y, -alpha), alpha);
+                tx.x = fminf(fmaxf(tx.x, -alpha.x), alpha.x);
+                tx.y = fminf(fmaxf(tx.y, -alpha.y), alpha.y);
+                ty.x = fminf(fmaxf(ty.x, -alpha.x), alpha.x);
+                ty.y = fminf(fmaxf(ty.y, -alpha.y), alpha.y);
             } else {
                 const float2 n2 = fma2(ty, ty, mul2(tx, tx));
-                const float2 sc = make_float2(fminf(alpha * rsqrtf(n2.x), 1.f), fminf(alpha * rsqrtf(n2.y), 1.f));
+                const float2 sc = make_float2(fminf(proj_scale<kResidentFastProj>(alpha.x, n2.x), 1.f),
+                                              fminf(proj_scale<kResidentFastProj>(alpha.y, n2.y), 1.f));
                 tx = mul2(tx, sc);
                 ty = mul2(ty, sc);
             }
@@ -223,10 +228,10 @@ __device__ __forceinline__ void q_update_tm(const TmRow<N, NT> &r, const Residen
                     gn = make_float2(fabsf(gx.x) + fabsf(gy.x), fabsf(gx.y) + fabsf(gy.y));
                 } else {
                     const float2 g2 = fma2(gy, gy, mul2(gx, gx));
-                    gn = make_float2(sqrt_approx(g2.x), sqrt_approx(g2.y));   // the gap is a diagnostic compared at 1e-3 (R17)
+                    gn = make_float2(gap_sqrt<kResidentFastProj>(g2.x), gap_sqrt<kResidentFastProj>(g2.y));
                 }
                 const float2 dot = fma2(gy, ty, mul2(gx, tx));
-                gap = add2(gap, sub2(mul2(splat(alpha), gn), dot));
+                gap = add2(gap, sub2(mul2(alpha, gn), dot));
             }
         }
         tm_st(r.tm_qx + 2 * CH * c, qxv);
@@ -278,10 +283,13 @@ __device__ __forceinline__ void d_term_tm(const TmRow<N, NT> &r, const int j, fl
 // ------------------------------------------------------------------------------------------------ row phase
 // v = K p_{n+1}: the row FFT of Z gives conj(v_a + i v_b) = (v_a, -v_b).
 // chi_{n+1} = chi_n - tau v - tau d ; chibar_{n+1} = chi_{n+1} + theta (chi_{n+1} - chi_n) ; Z <- row FFT of chibar_{n+1}.
-template <int N, int NT, int LDR, class Tw>
+// L1 (PD_REG_L1): d = 0 and chi_{n+1} = shrink(chi_n - tau v, thr0 M), thr0 = tau alpha per lane (soft shrinkage, the
+// prox of the l1 norm; BASELINE.json north_star).
+template <int N, int NT, int LDR, bool L1, class Tw>
 __device__ __forceinline__ void primal_tm_row(const TmRow<N, NT> &r, const ResidentTmArgs &a, const int j, float2 *smg,
                                               const Tw &tw, const float2 (&d)[FftCfg<N>::E], float *out_a,
-                                              float *out_b, float2 &dn, float2 &cn, const bool need_next) {
+                                              float *out_b, const float2 out_scale, const float2 thr0, float2 &dn,
+                                              float2 &cn, const bool need_next) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, CH = 8;
     float2 v[E];
 #pragma unroll
@@ -296,7 +304,15 @@ __device__ __forceinline__ void primal_tm_row(const TmRow<N, NT> &r, const Resid
         for (int k = 0; k < CH; ++k) {
             const int m = c * CH + k, x = j + T * m;
             const float2 c_old = cov[k];
-            const float2 c_new = fma2(ntau2, d[m], fma2(ntau_v, v[m], c_old));
+            float2 c_new;
+            if constexpr (L1) {
+                const float2 mm = r.mbin ? mask_from_bits(r.mbits, m) : ldcg2(r.M2 + j + T * m);
+                const float2 thr = mul2(thr0, mm), cand = fma2(ntau_v, v[m], c_old);
+                c_new = make_float2(copysignf(fmaxf(fabsf(cand.x) - thr.x, 0.f), cand.x),
+                                    copysignf(fmaxf(fabsf(cand.y) - thr.y, 0.f), cand.y));
+            } else {
+                c_new = fma2(ntau2, d[m], fma2(ntau_v, v[m], c_old));
+            }
             const float2 dc = sub2(c_new, c_old);
             dn = fma2(dc, dc, dn);
             cn = fma2(c_new, c_new, cn);
@@ -304,8 +320,8 @@ __device__ __forceinline__ void primal_tm_row(const TmRow<N, NT> &r, const Resid
             cov[k] = c_new;
             r.cb_t[m * NT] = cbar;
             v[m] = cbar;
-            if (out_a) out_a[x] = c_new.x;
-            if (out_b) out_b[x] = c_new.y;
+            if (out_a) out_a[x] = out_scale.x * c_new.x;   // back to the caller's units (exact: a power of two)
+            if (out_b) out_b[x] = out_scale.y * c_new.y;
         }
         tm_st(r.tm_chi + 2 * CH * c, cov);
     }
@@ -329,9 +345,10 @@ struct ResTmCfg {
 };
 
 // ------------------------------------------------------------------------------------------------ the kernel
-template <int N, int C, int NT, bool ANISO>
+template <int N, int C, int NT, int MODE>
 __global__ void __launch_bounds__(NT, 1)
 resident_tm_kernel(const ResidentTmArgs a) {
+    constexpr bool ANISO = MODE == kModeAniso, L1 = MODE == kModeL1;
     using Cfg = ResCfg<N, C, NT>;
     using TCfg = ResTmCfg<N, C, NT>;
     constexpr int E = Cfg::E, T = Cfg::T, RPC = Cfg::RPC, P = N * N, CH = 8;
@@ -397,14 +414,15 @@ resident_tm_kernel(const ResidentTmArgs a) {
         const bool has_b = s1 < a.batch;
         const float2 zero = make_float2(0.f, 0.f);
 
-        // ---- S7 load: my row of field and mask; zero state; P0 partial sums; mask bits; row FFT of phi
+        // ---- S7 load: my row of field and mask; zero state; P0 partial sums; mask bits; then (the slices' norms are
+        // known after one cluster barrier) normalisation (pair_scale) and row FFT of phi
+        float2 v[E];
         {
             const float *fa = a.field + (long long)s0 * P + y * N;
             const float *fb = a.field + (long long)s1 * P + y * N;
             const float *ma = a.mask ? a.mask + s0 * a.mask_bstride + y * N : nullptr;
             const float *mb = a.mask ? a.mask + s1 * a.mask_bstride + y * N : nullptr;
             float acc[2] = {0.f, 0.f};
-            float2 v[E];
             unsigned bits = 0u;
             int general = 0;
 #pragma unroll
@@ -430,9 +448,6 @@ resident_tm_kernel(const ResidentTmArgs a) {
                 tm_st(r.tm_qx + 2 * CH * c, z8);
                 tm_st(r.tm_chi + 2 * CH * c, z8);
             }
-            fft_line<N, Cfg::LDR>(v, smg_row, j, tw_row, WarpSync());
-#pragma unroll
-            for (int m = 0; m < E; ++m) r.Z[j + T * m] = v[m];
             general = __syncthreads_or(general);
             const float t = block_sum<NT, 2>(acc, red);
             if (tid < 2) part[rank * 8 + tid] = t;
@@ -446,9 +461,19 @@ resident_tm_kernel(const ResidentTmArgs a) {
             for (int q = 0; q < C; ++q) t += __ldcg(part + q * 8 + o);
             dec[tid < 2 ? tid : 8] = tid < 2 ? 0.5f * t : t;
         }
+        __syncthreads();
+        const float ca = pair_scale(2.f * dec[0], (float)P), cb = pair_scale(2.f * dec[1], (float)P);
+        {
+            const float2 c2 = make_float2(ca, cb);
+#pragma unroll
+            for (int m = 0; m < E; ++m) v[m] = mul2(c2, v[m]);
+            fft_line<N, Cfg::LDR>(v, smg_row, j, tw_row, WarpSync());
+#pragma unroll
+            for (int m = 0; m < E; ++m) r.Z[j + T * m] = v[m];
+        }
+        cluster_sync_all<C>();
         // ---- phi^ = column FFT of the row-transformed field, kept in the column role's private window
         {
-            float2 v[E];
 #pragma unroll
             for (int m = 0; m < E; ++m) v[m] = ldcg2(zcol + (cj + T * m) * N);
             fft_line<N, T>(v, smg_col, cj, tw_col, BlockSync());   // its __syncthreads also publish dec[]
@@ -461,7 +486,8 @@ resident_tm_kernel(const ResidentTmArgs a) {
             }
             tm_st_wait();
         }
-        const float P0a = dec[0], P0b = dec[1];
+        const float P0a = dec[0] * ca * ca, P0b = dec[1] * cb * cb;
+        const float2 alpha2 = make_float2(a.alpha * ca, a.alpha * cb), out_scale = make_float2(1.f / ca, 1.f / cb);
         r.mbin = dec[8] == 0.f;   // every CTA of the cluster takes the same path
         // R13b: an all-zero slice is never scheduled (every iteration would be a no-op)
         int stop_a = (P0a == 0.f) ? 0 : a.max_iters;
@@ -482,7 +508,7 @@ resident_tm_kernel(const ResidentTmArgs a) {
             dual_tm_col<N, NT>(zcol, dpriv, tm_ph, tm_fh, cj, smg_col, smg_mir, tw_col, colsync, a, n == 0, want_gap, Sa, Sb);
             // (2) q-update from chibar_n (chibar_0 = 0 and q_0 = 0: nothing to do in the first iteration)
             float2 gap = zero;
-            if (n > 0) q_update_tm<N, NT, ANISO>(r, a, j, want_gap, gap);
+            if (!L1 && n > 0) q_update_tm<N, NT, ANISO>(r, a, alpha2, j, want_gap, gap);
             if (want_gap) {
                 float acc[4] = {Sa, Sb, gap.x, gap.y};
                 const float t = block_sum<NT, 4>(acc, red);
@@ -505,12 +531,12 @@ resident_tm_kernel(const ResidentTmArgs a) {
             // (3) row phase: divergence of M q_{n+1}, primal step, over-relaxation, row FFT of chibar_{n+1}
             {
                 float2 d[E];
-                d_term_tm<N, NT>(r, j, d);
+                if constexpr (!L1) d_term_tm<N, NT>(r, j, d);
                 float *out_a = (act_a && n + 1 >= stop_a) ? a.chi_out + (long long)s0 * P + y * N : nullptr;
                 float *out_b = (act_b && n + 1 >= stop_b) ? a.chi_out + (long long)s1 * P + y * N : nullptr;
                 const bool need_next = (n + 1 < a.max_iters) && (n + 1 < stop_a || n + 1 < stop_b);
                 float2 dn = zero, cn = zero;
-                primal_tm_row<N, NT, Cfg::LDR>(r, a, j, smg_row, tw_row, d, out_a, out_b, dn, cn, need_next);
+                primal_tm_row<N, NT, Cfg::LDR, L1>(r, a, j, smg_row, tw_row, d, out_a, out_b, out_scale, mul2(splat(a.tau), alpha2), dn, cn, need_next);
                 if (out_a || out_b) {   // residual of the final iterate (reported, not used for stopping)
                     float acc[4] = {dn.x, cn.x, dn.y, cn.y};
                     const float t = block_sum<NT, 4>(acc, red);

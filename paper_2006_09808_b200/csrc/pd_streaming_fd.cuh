@@ -28,8 +28,7 @@
 // both as per-CTA partial sums.  Every CTA of fd_cols(n+1) reduces the partials of iteration n in the same fixed
 // order and reaches the same stop decision; column block 0 records it.  No host round trip.
 #pragma once
-#include "pd_resident.cuh"    // packed fp32x2 helpers, FFT building blocks
-#include "pd_streaming.cuh"   // group_sum
+#include "pd_resident.cuh"    // packed fp32x2 helpers, FFT building blocks (fft_regs.cuh)
 
 namespace pdk {
 
@@ -42,12 +41,14 @@ struct StreamFdArgs {
     float2 *Z, *phihat, *M2;                 // [npairs][ny][nx]
     float2 *W2;                              // literal path only: interleaved W; phihat then holds phi itself
     int literal;                             // 1: W != I or PD_OPT_FOURIER_DUAL = 0 (p kept in the image domain)
+    int reg_l1;                              // 1: PD_REG_L1 (l1 on chi, shrinkage) instead of the paper's TV term
     float2 *phat[2], *qx2[2], *qy2[2];       // double-buffered by iteration parity: iteration n reads [n&1]
     float2 *chi3[3];                         // chi_n in [n%3], chi_{n-1} in [(n+2)%3], chi_{n+1} written to [(n+1)%3]
     const float *Dtab;                       // D/(nx*ny), [ny][nx]
     const float2 *tw_row, *tw_col;
     int *stop_iter;                          // slice b is active in iteration n (0-based) iff n < stop_iter[b]
     float *P0, *relgap, *relres;
+    float *cscale;                           // [batch] power-of-two normalisation of every slice (pair_scale, pd_resident.cuh)
     int *iters_done;
     float *p0_part;                          // [npairs][nrowparts][2]
     float *gap_col[2];                       // [npairs][ncolparts][2], by iteration parity
@@ -62,23 +63,27 @@ template <int N> struct SfdRowCfg {
     static constexpr int THREADS = 128;
     static constexpr int G = THREADS / T;
     static constexpr int LD = T + 1;
-    static constexpr int SM_PER_GROUP = E * LD;
+    static constexpr int SM_PER_GROUP = E * LD > FftCfg<N>::REGION ? E * LD : FftCfg<N>::REGION;
 #ifndef PD_SFD_STAGE_MIN
 #define PD_SFD_STAGE_MIN 256
 #endif
     static constexpr bool STAGE = N >= PD_SFD_STAGE_MIN;   // park the spectrum in shared memory during the update loop
-    static constexpr int MINB = STAGE ? 5 : (N == 512 ? 3 : 4);
+#ifndef PD_SFD_ROWS512_MINB
+#define PD_SFD_ROWS512_MINB 5
+#endif
+    static constexpr int MINB = N == 512 ? PD_SFD_ROWS512_MINB : (STAGE ? 5 : 4);
 #ifndef PD_SFD_UNROLL
 #define PD_SFD_UNROLL 4
 #endif
     static constexpr int UNROLL = PD_SFD_UNROLL;           // elements of the update loop per unrolled body (STAGE only)
 };
 template <int N> struct SfdColCfg {
-    static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
+    using Fft = FftCfg<N, true>;                       // column configuration of the line transform (fft_regs.cuh)
+    static constexpr int E = Fft::E, T = Fft::T;
     static constexpr int HALF = 8, COLS = 16;          // 8 adjacent columns and their 8 mirror images
     static constexpr int THREADS = COLS * T;
-    static constexpr int CS = N + 1;
-    static constexpr int SMEM_BYTES = (COLS * CS + E * T) * (int)sizeof(float2) + 128;
+    static constexpr int CS = N + 1 > Fft::REGION ? N + 1 : Fft::REGION + 1;   // odd column stride
+    static constexpr int SMEM_BYTES = (COLS * CS + Fft::TW) * (int)sizeof(float2) + 256;
 #ifndef PD_SFD_COL_STAGE_MIN
 #define PD_SFD_COL_STAGE_MIN 256
 #endif
@@ -106,8 +111,49 @@ __device__ __forceinline__ float2 sfd_gap_sum(const StreamFdArgs &a, int pair, i
     return make_float2(ga, gb);
 }
 
+// The same sums by one whole warp: lane l takes the partials l, l + 32, ... of either array, then a butterfly over the
+// lanes -- a fixed order again, so every CTA of a launch reaches the same value, at one L2 latency instead of
+// ncolparts + nrowparts dependent additions by a single thread.  Result valid in every lane.
+__device__ __forceinline__ float2 sfd_gap_sum_warp(const StreamFdArgs &a, const int pair, const int par, const int lane) {
+    float ga = 0.f, gb = 0.f;
+    const float *gc = a.gap_col[par] + (long long)pair * a.ncolparts * 2;
+    for (int k = lane; k < a.ncolparts; k += 32) { ga += __ldcg(gc + 2 * k); gb += __ldcg(gc + 2 * k + 1); }
+    const float *gr = a.gap_row + (long long)pair * a.nrowparts * 2;
+    for (int k = lane; k < a.nrowparts; k += 32) { ga += __ldcg(gr + 2 * k); gb += __ldcg(gr + 2 * k + 1); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ga += __shfl_xor_sync(0xffffffffu, ga, o);
+        gb += __shfl_xor_sync(0xffffffffu, gb, o);
+    }
+    return make_float2(ga, gb);
+}
+
+// ------------------------------------------------------------------------------------------------ normalisation
+// c_b = 2^-floor(log2 rms(phi_b)) of every slice (pair_scale): one CTA per slice, fixed summation order.
+__global__ void __launch_bounds__(256)
+sfd_scale_kernel(const StreamFdArgs a) {
+    __shared__ float red[8];
+    const int b = blockIdx.x;
+    const long long P = (long long)a.nx * a.ny;
+    const float4 *f = reinterpret_cast<const float4 *>(a.field + (long long)b * P);
+    float s = 0.f;
+    for (int i = threadIdx.x; i < (int)(P / 4); i += 256) {
+        const float4 v = __ldg(f + i);
+        s = fmaf(v.x, v.x, fmaf(v.y, v.y, fmaf(v.z, v.z, fmaf(v.w, v.w, s))));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float t = 0.f;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        a.cscale[b] = pair_scale(t, (float)P);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ init
-// Load the pair's field rows, interleave the mask, zero the state that iteration 0 reads, partial sums of
+// Load the pair's field rows (normalised, see sfd_scale_kernel), interleave the mask, zero the state that iteration 0 reads, partial sums of
 // 1/2 ||phi||^2, row FFT of phi -> Z.  (chi_0 = chibar_0 = p_0 = q_0 = 0.)
 template <int NX>
 __global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS)
@@ -115,7 +161,7 @@ sfd_init_rows_kernel(const StreamFdArgs a) {
     using Cfg = SfdRowCfg<NX>;
     constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
     __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
-    __shared__ float2 tws[E * T];
+    __shared__ float2 tws[FftCfg<NX>::TW];
     __shared__ float red[G][2];
     TwiddlesSmem<NX>::fill(tws, a.tw_row, threadIdx.x, Cfg::THREADS);
     __syncthreads();
@@ -131,12 +177,13 @@ sfd_init_rows_kernel(const StreamFdArgs a) {
     const float *ma = a.mask ? a.mask + s0 * a.mask_bstride + rowoff : nullptr;
     const float *mb = a.mask ? a.mask + s1 * a.mask_bstride + rowoff : nullptr;
     const float2 zero = make_float2(0.f, 0.f);
+    const float ca = a.cscale[s0], cb = has_b ? a.cscale[s1] : 0.f;
     float2 v[E];
     float acc0 = 0.f, acc1 = 0.f;
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int x = j + T * m;
-        const float va = fa[x], vb = has_b ? fb[x] : 0.f;
+        const float va = ca * fa[x], vb = has_b ? cb * fb[x] : 0.f;
         v[m] = make_float2(va, vb);
         float wa = 1.f, wb = 1.f;
         if (a.literal) {   // phi and W interleaved, p_0 = 0; P0 = 1/2 ||W phi||^2
@@ -175,13 +222,13 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
     extern __shared__ __align__(16) unsigned char sfd_smem[];
     float2 *smc = reinterpret_cast<float2 *>(sfd_smem);
     float2 *tws = smc + Cfg::COLS * Cfg::CS;
-    TwiddlesSmem<NY>::fill(tws, a.tw_col, threadIdx.x, Cfg::THREADS);
+    TwiddlesSmem<NY, true>::fill(tws, a.tw_col, threadIdx.x, Cfg::THREADS);
     __syncthreads();
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
     const int kx = sfd_column_of(a.nx, blockIdx.x, c >> 3, c & 7);
     const long long po = (long long)pair * a.nx * NY + kx;
-    TwiddlesSmem<NY> tw;
+    TwiddlesSmem<NY, true> tw;
     tw.w = tws + j;
     if (!a.literal) {
         float2 v[E];
@@ -217,7 +264,9 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
 // reduces the same partial sums in the same order; block 0 records relgap and stop_iter.  Then
 //   X^ = column FFT of Z (zero when n == 0) ; p^_{n+1} = (p^_n + sigma (D X^ - phi^))/(1 + sigma) ;
 //   Z <- column FFT of conj(D/(nx ny) p^_{n+1})      (the row kernel's FFT finishes the inverse transform)
-// want_gap: S1 = sum |dp|^2, S2 = Re sum dp(k) dp(-k), dp = p^_{n+1} - p^_n; the mirror column is in this CTA.
+// want_gap: Sa = sum |dp(k) + conj dp(-k)|^2, Sb = sum |dp(k) - conj dp(-k)|^2, dp = p^_{n+1} - p^_n -- the two lanes'
+// spectra accumulated directly (no difference of two large sums, so a weak slice does not lose digits to a strong
+// partner); the mirror column is in this CTA.
 // PLAIN (literal path): only Z <- column FFT of conj(D/(nx ny) X^), i.e. one application of K between two row passes;
 // `decide` is set for the first of the two column launches of an iteration.
 template <int NY, bool PLAIN>
@@ -230,7 +279,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     extern __shared__ __align__(16) unsigned char sfd_smem[];
     float2 *smc = reinterpret_cast<float2 *>(sfd_smem);
     float2 *tws = smc + Cfg::COLS * Cfg::CS;
-    float *dec = reinterpret_cast<float *>(tws + E * T);   // [0..1] stop flags of this launch ; [2..] reduction
+    float *dec = reinterpret_cast<float *>(tws + Cfg::Fft::TW);   // [0..1] stop flags of this launch ; [2..] reduction
 
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
     const bool has_b = s1 < a.batch;
@@ -239,17 +288,19 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
 
     const bool decide = do_decide && n > 0 && a.tol > 0.f && (n % a.check_every) == 0;   // iteration n-1 was a checking one
     if (decide) {
-        if (threadIdx.x == 0) {
-            const float2 g = sfd_gap_sum(a, pair, (n - 1) & 1);
-            const float P0a = a.P0[s0], P0b = has_b ? a.P0[s1] : 0.f;
-            const float ra = P0a > 0.f ? g.x / P0a : 0.f, rb = P0b > 0.f ? g.y / P0b : 0.f;
-            int f0 = 0, f1 = 0;
-            if (n < stop0 && ra < a.tol) f0 = 1;
-            if (n < stop1 && rb < a.tol) f1 = 1;
-            dec[0] = (float)f0; dec[1] = (float)f1;
-            if (blockIdx.x == 0) {
-                if (n < stop0) { a.relgap[s0] = ra; if (f0) a.stop_iter[s0] = n; }
-                if (n < stop1) { a.relgap[s1] = rb; if (f1) a.stop_iter[s1] = n; }
+        if (threadIdx.x < 32) {
+            const float2 g = sfd_gap_sum_warp(a, pair, (n - 1) & 1, threadIdx.x);
+            if (threadIdx.x == 0) {
+                const float P0a = a.P0[s0], P0b = has_b ? a.P0[s1] : 0.f;
+                const float ra = P0a > 0.f ? g.x / P0a : 0.f, rb = P0b > 0.f ? g.y / P0b : 0.f;
+                int f0 = 0, f1 = 0;
+                if (n < stop0 && ra < a.tol) f0 = 1;
+                if (n < stop1 && rb < a.tol) f1 = 1;
+                dec[0] = (float)f0; dec[1] = (float)f1;
+                if (blockIdx.x == 0) {
+                    if (n < stop0) { a.relgap[s0] = ra; if (f0) a.stop_iter[s0] = n; }
+                    if (n < stop1) { a.relgap[s1] = rb; if (f1) a.stop_iter[s1] = n; }
+                }
             }
         }
         __syncthreads();
@@ -260,7 +311,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     const bool last = (n + 1 == a.max_iters);
     const bool want_gap = !PLAIN && (last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0));
 
-    TwiddlesSmem<NY>::fill(tws, a.tw_col, threadIdx.x, NT);
+    TwiddlesSmem<NY, true>::fill(tws, a.tw_col, threadIdx.x, NT);
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
     const int h = c >> 3, cc = c & 7;
     const int nx = a.nx;
@@ -272,7 +323,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     float2 *zc = a.Z + po, *phw = a.phat[(n & 1) ^ 1] + po;
     const float2 *phh = a.phihat + po, *phr = a.phat[n & 1] + po;
     const float *dcol = a.Dtab + kx;
-    TwiddlesSmem<NY> tw;
+    TwiddlesSmem<NY, true> tw;
     tw.w = tws + j;
     __syncthreads();
 
@@ -291,7 +342,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     }
     const float2 sig2 = splat(a.sigma), inv2 = splat(a.inv_one_plus_sigma);
     const float NN = (float)nx * (float)NY;
-    float S1 = 0.f, S2 = 0.f;
+    float Sa = 0.f, Sb = 0.f;
     if (PLAIN) {
 #pragma unroll
         for (int m = 0; m < E; ++m) {
@@ -313,10 +364,6 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
             const float2 pold = __ldg(phr + o);
             const float2 res = sub2(mul2(splat(d * NN), smg[j + T * m]), phat);
             const float2 pn = mul2(fma2(sig2, res, pold), inv2);
-            if (want_gap) {
-                const float2 dp = sub2(pn, pold);
-                S1 = fmaf(dp.x, dp.x, fmaf(dp.y, dp.y, S1));
-            }
             __stcs(phw + o, pn);
             smg[j + T * m] = pn;
         }
@@ -328,7 +375,9 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
                 const int ky = j + T * m, kym = (NY - ky) & (NY - 1);
                 const float2 dp = sub2(smg[ky], __ldg(phr + (long long)ky * nx));
                 const float2 dm = sub2(smg_mir[kym], __ldg(phr_mir + (long long)kym * nx));
-                S2 = fmaf(dp.x, dm.x, fmaf(-dp.y, dm.y, S2));
+                const float ax = dp.x + dm.x, ay = dp.y - dm.y, bx = dp.x - dm.x, by = dp.y + dm.y;
+                Sa = fmaf(ax, ax, fmaf(ay, ay, Sa));
+                Sb = fmaf(bx, bx, fmaf(by, by, Sb));
             }
         }
 #pragma unroll
@@ -347,11 +396,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
             const float2 pold = __ldg(phr + o);
             const float2 res = sub2(mul2(splat(d * NN), v[m]), phat);
             const float2 pn = mul2(fma2(sig2, res, pold), inv2);
-            if (want_gap) {
-                const float2 dp = sub2(pn, pold);
-                S1 = fmaf(dp.x, dp.x, fmaf(dp.y, dp.y, S1));
-                smg[j + T * m] = dp;
-            }
+            if (want_gap) smg[j + T * m] = sub2(pn, pold);
             __stcs(phw + o, pn);
             v[m] = make_float2(d * pn.x, -d * pn.y);
         }
@@ -362,7 +407,9 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
                 const int ky = j + T * m;
                 const float2 dp = smg[ky];
                 const float2 dm = smg_mir[(NY - ky) & (NY - 1)];
-                S2 = fmaf(dp.x, dm.x, fmaf(-dp.y, dm.y, S2));
+                const float ax = dp.x + dm.x, ay = dp.y - dm.y, bx = dp.x - dm.x, by = dp.y + dm.y;
+                Sa = fmaf(ax, ax, fmaf(ay, ay, Sa));
+                Sb = fmaf(bx, bx, fmaf(by, by, Sb));
             }
         }
     }
@@ -374,35 +421,36 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
         __syncthreads();
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-            S1 += __shfl_xor_sync(0xffffffffu, S1, o);
-            S2 += __shfl_xor_sync(0xffffffffu, S2, o);
+            Sa += __shfl_xor_sync(0xffffffffu, Sa, o);
+            Sb += __shfl_xor_sync(0xffffffffu, Sb, o);
         }
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-        if (lane == 0) { dec[2 + 2 * warp] = S1; dec[3 + 2 * warp] = S2; }
+        if (lane == 0) { dec[2 + 2 * warp] = Sa; dec[3 + 2 * warp] = Sb; }
         __syncthreads();
         if (threadIdx.x == 0) {
             float t1 = 0.f, t2 = 0.f;
             for (int w = 0; w < NT / 32; ++w) { t1 += dec[2 + 2 * w]; t2 += dec[3 + 2 * w]; }
-            // 1/2 sum_x e^2 = (S1 +- S2) / (4 nx ny sigma^2)   (Parseval; pd_resident_tm.cuh header)
-            const float scale = 0.25f / (NN * a.sigma * a.sigma);
+            // 1/2 sum_x e^2 = sum_k |dp(k) +- conj dp(-k)|^2 / (8 nx ny sigma^2)   (Parseval; pd_resident_tm.cuh header)
+            const float scale = 0.125f / (NN * a.sigma * a.sigma);
             float *gc = a.gap_col[n & 1] + ((long long)pair * a.ncolparts + blockIdx.x) * 2;
-            gc[0] = scale * (t1 + t2);
-            gc[1] = scale * (t1 - t2);
+            gc[0] = scale * t1;
+            gc[1] = scale * t2;
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------ row kernel
 // isotropic / anisotropic projection of (tx, ty) onto the alpha-ball, both lanes (PAPER.md:49 line 2; R4, R13)
-__device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float alpha, const float alpha_sq, const bool aniso) {
+// alpha is per lane: every slice is iterated in its own normalisation (pair_scale)
+__device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float2 alpha, const float2 alpha_sq, const bool aniso) {
     if (aniso) {
-        tx.x = fminf(fmaxf(tx.x, -alpha), alpha); tx.y = fminf(fmaxf(tx.y, -alpha), alpha);
-        ty.x = fminf(fmaxf(ty.x, -alpha), alpha); ty.y = fminf(fmaxf(ty.y, -alpha), alpha);
+        tx.x = fminf(fmaxf(tx.x, -alpha.x), alpha.x); tx.y = fminf(fmaxf(tx.y, -alpha.y), alpha.y);
+        ty.x = fminf(fmaxf(ty.x, -alpha.x), alpha.x); ty.y = fminf(fmaxf(ty.y, -alpha.y), alpha.y);
     } else {
         const float2 n2 = fma2(ty, ty, mul2(tx, tx));
         float2 sc;
-        sc.x = (n2.x > alpha_sq) ? alpha * rsqrtf(n2.x) : 1.f;
-        sc.y = (n2.y > alpha_sq) ? alpha * rsqrtf(n2.y) : 1.f;
+        sc.x = (n2.x > alpha_sq.x) ? proj_scale<kStreamingFastProj>(alpha.x, n2.x) : 1.f;
+        sc.y = (n2.y > alpha_sq.y) ? proj_scale<kStreamingFastProj>(alpha.y, n2.y) : 1.f;
         tx = mul2(tx, sc);
         ty = mul2(ty, sc);
     }
@@ -420,7 +468,7 @@ sfd_rows_kernel(const StreamFdArgs a, const int n_arg) {
     using Cfg = SfdRowCfg<NX>;
     constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
     __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
-    __shared__ float2 tws[E * T];
+    __shared__ float2 tws[FftCfg<NX>::TW];
     __shared__ float red[G][6];
 
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
@@ -468,7 +516,8 @@ sfd_rows_kernel(const StreamFdArgs a, const int n_arg) {
     }
 
     const float2 sig2 = splat(a.sigma), zero = make_float2(0.f, 0.f);
-    const float alpha = a.alpha, alpha_sq = a.alpha * a.alpha;
+    const float2 alpha = make_float2(a.alpha * a.cscale[s0], (s1 < a.batch) ? a.alpha * a.cscale[s1] : 0.f);
+    const float2 alpha_sq = mul2(alpha, alpha);
     const bool aniso = a.aniso != 0;
     const float2 ntau2 = splat(-a.tau), ntau_v = make_float2(-a.tau, a.tau), theta2 = splat(a.theta);
     const float2 actm = make_float2(act0 ? 1.f : 0.f, act1 ? 1.f : 0.f);
@@ -510,9 +559,9 @@ sfd_rows_kernel(const StreamFdArgs a, const int n_arg) {
                 gn = make_float2(fabsf(gx.x) + fabsf(gy.x), fabsf(gx.y) + fabsf(gy.y));
             } else {
                 const float2 g2 = fma2(gy, gy, mul2(gx, gx));
-                gn = make_float2(sqrtf(g2.x), sqrtf(g2.y));
+                gn = make_float2(gap_sqrt<kStreamingFastProj>(g2.x), gap_sqrt<kStreamingFastProj>(g2.y));
             }
-            gap = add2(gap, sub2(mul2(splat(alpha), gn), fma2(gy, ty, mul2(gx, tx))));
+            gap = add2(gap, sub2(mul2(alpha, gn), fma2(gy, ty, mul2(gx, tx))));
         }
         // row above, redundantly: (M qy_{n+1})[y-1][x]
         float2 mqy_up = zero;
@@ -569,6 +618,95 @@ sfd_rows_kernel(const StreamFdArgs a, const int n_arg) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------ row kernel, l1 on chi
+// soft shrinkage of both lanes: sign(v) max(|v| - t, 0), the prox of t |.| (BASELINE.json north_star "or shrinkage")
+__device__ __forceinline__ float2 shrink2(const float2 v, const float2 t) {
+    return make_float2(copysignf(fmaxf(fabsf(v.x) - t.x, 0.f), v.x), copysignf(fmaxf(fabsf(v.y) - t.y, 0.f), v.y));
+}
+
+// PD_REG_L1: min 1/2||W(K chi - phi)||^2 + alpha ||M chi||_1 (north_star's alternative regulariser).
+// No q: the row kernel of iteration n is
+//   v = K p_{n+1}: row FFT of Z gives (v_a, -v_b) ; chi_{n+1} = shrink(chi_n - tau v, tau alpha M) ;
+//   chibar_{n+1} = chi_{n+1} + theta (chi_{n+1} - chi_n) ; Z <- row FFT of chibar_{n+1}
+// on the same planes and with the same column kernels / dual row kernel as the TV iteration (the q planes stay unused).
+template <int NX, bool MASKED>
+__global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, 4)
+sfd_rows_l1_kernel(const StreamFdArgs a, const int n_arg) {
+    const int n = n_arg >= 0 ? n_arg : *a.iter;
+    using Cfg = SfdRowCfg<NX>;
+    constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
+    __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
+    __shared__ float2 tws[FftCfg<NX>::TW];
+    __shared__ float red[G][4];
+
+    const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
+    const bool act0 = n < a.stop_iter[s0];
+    const bool act1 = (s1 < a.batch) && (n < a.stop_iter[s1]);
+    if (!act0 && !act1) return;
+    const bool last = (n + 1 == a.max_iters);
+    const bool want_gap = last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0);
+
+    TwiddlesSmem<NX>::fill(tws, a.tw_row, threadIdx.x, Cfg::THREADS);
+    const int g = threadIdx.x / T, j = threadIdx.x % T;
+    const int y = blockIdx.x * G + g;
+    float2 *smg = sm + g * Cfg::SM_PER_GROUP;
+    TwiddlesSmem<NX> tw;
+    tw.w = tws + j;
+    const long long po = ((long long)pair * a.ny + y) * NX;
+    float2 *zr = a.Z + po, *chiw = a.chi3[(n + 1) % 3] + po;
+    const float2 *chn = a.chi3[n % 3] + po, *M = a.M2 + po;
+
+    float2 v[E];
+#pragma unroll
+    for (int m = 0; m < E; ++m) v[m] = __ldcs(zr + j + T * m);
+    __syncthreads();   // twiddle table
+    fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
+    __syncwarp();      // the second FFT stage of the other threads has read the region
+#pragma unroll
+    for (int m = 0; m < E; ++m) smg[j + T * m] = v[m];
+
+    const float2 ntau_v = make_float2(-a.tau, a.tau), theta2 = splat(a.theta);
+    // threshold tau alpha per lane, in the lane's own normalisation (pair_scale)
+    const float2 thr0 = make_float2(a.tau * a.alpha * a.cscale[s0], (s1 < a.batch) ? a.tau * a.alpha * a.cscale[s1] : 0.f);
+    float2 dn = make_float2(0.f, 0.f), cn = dn;
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int x = j + T * m;
+        const float2 c_old = __ldg(chn + x);
+        const float2 thr = MASKED ? mul2(thr0, __ldg(M + x)) : thr0;
+        const float2 sh = shrink2(fma2(ntau_v, smg[x], c_old), thr);
+        const float2 c_new = make_float2(act0 ? sh.x : c_old.x, act1 ? sh.y : c_old.y);   // a stopped slice keeps its chi
+        const float2 dc = sub2(c_new, c_old);
+        dn = fma2(dc, dc, dn);
+        cn = fma2(c_new, c_new, cn);
+        __stcs(chiw + x, c_new);
+        smg[x] = fma2(theta2, dc, c_new);
+    }
+    if (!last) {
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = smg[j + T * m];
+        fft_line<NX, Cfg::LD>(v, smg, j, tw, WarpSync());
+#pragma unroll
+        for (int m = 0; m < E; ++m) __stcs(zr + j + T * m, v[m]);
+    }
+    float s4[4] = {dn.x, cn.x, dn.y, cn.y};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) s4[k] = group_sum<T>(s4[k]);
+    if (j == 0) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) red[g][k] = s4[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        const int k = threadIdx.x;
+        float t = 0.f;
+        for (int q = 0; q < G; ++q) t += red[q][k];
+        const long long part = (long long)pair * a.nrowparts + blockIdx.x;
+        if ((k < 2) ? act0 : act1) a.res_part[part * 4 + k] = t;
+        if (want_gap && k < 2) a.gap_row[part * 2 + k] = 0.f;   // the gap has no regulariser term here (R9)
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ dual rows (literal path)
 // W != I (or PD_OPT_FOURIER_DUAL = 0): p lives in the image domain, K is applied twice per iteration (PAPER.md:49
 // literally).  Iteration n:  [sfd_cols<PLAIN>]  this kernel  [sfd_cols<PLAIN>]  sfd_rows.
@@ -583,7 +721,7 @@ sfd_dual_rows_kernel(const StreamFdArgs a, const int n_arg) {
     using Cfg = SfdRowCfg<NX>;
     constexpr int E = Cfg::E, T = Cfg::T, G = Cfg::G;
     __shared__ float2 sm[G * Cfg::SM_PER_GROUP];
-    __shared__ float2 tws[E * T];
+    __shared__ float2 tws[FftCfg<NX>::TW];
     __shared__ float red[G][2];
 
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
@@ -682,10 +820,11 @@ sfd_finish_kernel(const StreamFdArgs a) {
     const int st0 = a.stop_iter[s0], st1 = has_b ? a.stop_iter[s1] : 0;
     const float2 *c2 = a.chi3[(st0 > st1 ? st0 : st1) % 3] + (long long)pair * P;
     float *oa = a.chi_out + (long long)s0 * P, *ob = a.chi_out + (long long)s1 * P;
+    const float ia = 1.f / a.cscale[s0], ib = has_b ? 1.f / a.cscale[s1] : 0.f;   // back to the caller's units (exact: powers of two)
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P; i += (long long)gridDim.x * blockDim.x) {
         const float2 c = __ldcs(c2 + i);
-        oa[i] = c.x;
-        if (has_b) ob[i] = c.y;
+        oa[i] = ia * c.x;
+        if (has_b) ob[i] = ib * c.y;
     }
     if (blockIdx.x == 0 && threadIdx.x < 2 && (threadIdx.x == 0 || has_b)) {
         const int s = threadIdx.x, b = s ? s1 : s0;

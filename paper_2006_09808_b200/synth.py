@@ -152,9 +152,21 @@ CONFIGS = {
 # The stack BASELINE.json's north_star quotes its target on: 128 slices of 256x256, 200 iterations
 # (C3's phantoms with a single coil map per slice).
 CONFIGS[5] = Config(5, "NS 128x256x256 seeds (north-star stack)", 256, 256, 128, 1, 200, 0.005)
+# Stand-ins in the PAPER'S OWN matrix sizes (256x258x25, 128x132x12, 128x132x42; the data sets themselves are
+# not available): E1 with C2's seed phantoms, E2 and E3 with C1's cylinders; x (fastest axis) takes the odd length.
+# `like` names the config whose phantom and mask recipe is reused (its random streams too, scaled to the new size).
+CONFIGS[6] = Config(6, "E1 25x256x258 seeds (paper's matrix)", 258, 256, 25, 1, 200, 0.005, extra={"like": 2})
+CONFIGS[7] = Config(7, "E2 12x128x132 cylinders (paper's matrix)", 132, 128, 12, 1, 200, 0.01, extra={"like": 1})
+CONFIGS[8] = Config(8, "E3 42x128x132 cylinders (paper's matrix)", 132, 128, 42, 1, 200, 0.01, extra={"like": 1})
+
+
+def _like(cfg):
+    """The config whose phantom / mask recipe `cfg` uses (itself unless it is one of the paper-sized stand-ins)."""
+    return CONFIGS[cfg.extra["like"]] if "like" in cfg.extra else cfg
 
 
 def _mask(cfg, nx, ny):
+    cfg = _like(cfg)
     if cfg.cid in (0, 4):
         return np.ones((ny, nx), np.float32)
     if cfg.cid == 1:
@@ -165,6 +177,7 @@ def _mask(cfg, nx, ny):
 
 def _phantom(cfg, s, nx, ny):
     """chi_true of slice s (float64 [ny][nx])."""
+    cfg = _like(cfg)
     pcid = 3 if cfg.cid == 5 else cfg.cid  # the north-star stack reuses C3's per-slice phantoms
     chi = background(nx, ny, stream_key(pcid, s, 0, _BG))
     st = _Stream(stream_key(pcid, s, 0, _SHAPES))

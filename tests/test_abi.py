@@ -17,7 +17,7 @@ def libpath():
 def header_functions():
     src = open(os.path.join(ROOT, "include", "pd.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(pd_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(pd_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_and_binding_agree():
@@ -42,8 +42,9 @@ def test_error_paths_that_need_no_gpu(libpath):
     assert L.pd_plan(C.byref(h), 64, 64, 1, 7, 0.01, 0.25, 0.25, 1.0) == binding.EINVAL        # bad B0_dir
     assert L.pd_plan(C.byref(h), 64, 64, 1, 1, -1.0, 0.25, 0.25, 1.0) == binding.EINVAL        # lambda < 0
     assert L.pd_plan(C.byref(h), 64, 64, 1, 1, 0.01, 0.25, 0.25, 1.5) == binding.EINVAL        # theta > 1
-    assert L.pd_plan(C.byref(h), 258, 256, 1, 1, 0.01, 0.25, 0.25, 1.0) == binding.ESIZE       # paper's 258: NEXT-1
-    assert L.pd_plan(C.byref(h), 64, 100, 1, 1, 0.01, 0.25, 0.25, 1.0) == binding.ESIZE
+    assert L.pd_plan(C.byref(h), 257, 256, 1, 1, 0.01, 0.25, 0.25, 1.0) == binding.ESIZE       # odd lengths are not supported
+    assert L.pd_plan(C.byref(h), 64, 2, 1, 1, 0.01, 0.25, 0.25, 1.0) == binding.ESIZE
+    assert L.pd_plan(C.byref(h), 2048, 64, 1, 1, 0.01, 0.25, 0.25, 1.0) == binding.ESIZE
     assert L.pd_plan(C.byref(h), 64, 64, 1, 1, 0.01, 0.4, 0.4, 1.0) == binding.ESTEP           # 0.16*8.44 > 1
     assert h.value is None
     assert L.pd_solve(None, None, None, None, 1, 0.0, None) == binding.EINVAL

@@ -91,7 +91,8 @@ enum { PD_VARIANT_AUTO = 0, PD_VARIANT_STREAMING = 1, PD_VARIANT_RESIDENT = 2 };
  * necessary is allocated by pd_set_option(PD_OPT_VARIANT, ...) or by the first pd_solve that needs it (that one
  * call then contains a cudaMalloc and a NULL-stream synchronisation).  A plan serves one pd_solve at a time.
  * sigma <= 0 or tau <= 0 selects the automatic steps
- * sigma = tau = 1/sqrt(4/9 + 8) (upper bound on ||K_full||_2).  *out receives the plan.
+ * sigma = tau = 1/sqrt(4/9 + 8) (upper bound on ||K_full||_2 for |W|, |M| <= 1; pd_set_norm_bounds for
+ * larger weights or mask values).  *out receives the plan.
  * Errors: PD_EINVAL, PD_ESIZE, PD_ESTEP, PD_ENOMEM, PD_ECUDA.  Uses the current CUDA device. */
 int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir,
             float lambda, float sigma, float tau, float theta);
@@ -135,6 +136,13 @@ int pd_set_steps(pd_plan_t p, float lambda, float sigma, float tau, float theta)
  * K is the real part of F^-1 D F (R12), so the even part (D(k) + D(-k))/2 is stored (it differs from D only on
  * the Nyquist lines).  Host call; waits for the device, then uploads.  Errors: PD_EINVAL, PD_ECUDA. */
 int pd_set_b0_angle(pd_plan_t p, float angle_rad);
+
+/* Bounds on |W| and |M| (R14; "tau = sigma = 1/L, L = ||K||_2").  pd_plan assumes |W| <= 1 and |M| <= 1: the
+ * automatic steps are 1/sqrt(4/9 + 8) and PD_ESTEP tests sigma tau (4/9 + 8) < 1.  A caller whose weights or mask exceed 1
+ * states the bounds here: the automatic steps become 1/sqrt(4/9 max|W|^2 + 8 max|M|^2) and PD_ESTEP (here and in
+ * pd_set_steps) uses the same bound.  The arrays themselves arrive later and are never scanned (no host round trip).
+ * Errors: PD_EINVAL (non-positive or non-finite bound), PD_ESTEP (explicit steps of the plan violate the new bound). */
+int pd_set_norm_bounds(pd_plan_t p, float max_abs_w, float max_abs_m);
 
 int pd_set_option(pd_plan_t p, int key, int value);
 

@@ -24,7 +24,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -51,6 +51,7 @@ def lib():
         L.pd_set_steps.argtypes = [vp, fp, fp, fp, fp]
         L.pd_set_option.argtypes = [vp, ip, ip]
         L.pd_set_b0_angle.argtypes = [vp, fp]
+        L.pd_set_norm_bounds.argtypes = [vp, fp, fp]
         L.pd_get_stats.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.pd_get_stats_host.argtypes = [vp, vp, vp, vp, vp]
         L.pd_get_kernel_times.argtypes = [vp, vp, vp]
@@ -121,6 +122,10 @@ class Plan:
 
     def set_steps(self, lambda_, sigma, tau, theta=1.0):
         _check(lib().pd_set_steps(self._h, lambda_, sigma, tau, theta))
+
+    def set_norm_bounds(self, max_abs_w, max_abs_m):
+        """pd_set_norm_bounds: bounds on |W| and |M| for the automatic steps and the PD_ESTEP check."""
+        _check(lib().pd_set_norm_bounds(self._h, float(max_abs_w), float(max_abs_m)))
 
     def set_b0_angle(self, angle_rad):
         """pd_set_b0_angle: B0 along (cos a, sin a) in the slice plane."""

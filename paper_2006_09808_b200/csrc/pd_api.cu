@@ -43,7 +43,8 @@ void balanced_factors(int n, int *n1, int *n2) {
     *n2 = n / best;
 }
 
-constexpr double kNormBound = 4.0 / 9.0 + 8.0;  // ||K_full||^2 <= max|D|^2 + ||G||^2 = 4/9 + 8 for W = M = 1
+// ||K_full||^2 <= max|W|^2 max|D|^2 + max|M|^2 ||G||^2 = 4/9 w^2 + 8 m^2 (R14); w = m = 1 unless pd_set_norm_bounds says otherwise
+double norm_bound(double w, double m) { return 4.0 / 9.0 * w * w + 8.0 * m * m; }
 
 }  // namespace
 
@@ -57,6 +58,7 @@ struct pd_plan_s {
     int generic;           // a size that is not a power of two: general-length kernels (pd_streaming_gen.cuh), literal iteration
     pdk::GenDims gdims;
     int reg_l1;            // PD_OPT_REGULARISER = PD_REG_L1
+    double max_w, max_m;   // bounds on |W| and |M| behind the automatic steps and the PD_ESTEP check (pd_set_norm_bounds; 1, 1)
     int use_angle;         // oblique in-plane B0 (pd_set_b0_angle)
     double b0_angle;
     const float *weight;
@@ -128,9 +130,9 @@ int dev_alloc(T **ptr, size_t count) {
     return PD_OK;
 }
 
-int check_params(float lambda, float sigma, float tau, float theta, bool unsafe) {
+int check_params(float lambda, float sigma, float tau, float theta, bool unsafe, double bound) {
     if (!(lambda >= 0.f) || !(theta >= 0.f && theta <= 1.f) || std::isnan(sigma) || std::isnan(tau)) return PD_EINVAL;
-    if (sigma > 0.f && tau > 0.f && !unsafe && (double)sigma * (double)tau * kNormBound >= 1.0) return PD_ESTEP;
+    if (sigma > 0.f && tau > 0.f && !unsafe && (double)sigma * (double)tau * bound >= 1.0) return PD_ESTEP;
     return PD_OK;
 }
 
@@ -138,7 +140,7 @@ int check_params(float lambda, float sigma, float tau, float theta, bool unsafe)
 // rescaling A(lambda, sigma, tau) == B(1/lambda, sigma/lambda, tau*lambda) (R2, oracle pin P9).
 void effective_params(const pd_plan_s *p, float *alpha, float *sigma, float *tau) {
     float s = p->sigma_user, t = p->tau_user;
-    if (!(s > 0.f) || !(t > 0.f)) s = t = (float)(1.0 / std::sqrt(kNormBound));
+    if (!(s > 0.f) || !(t > 0.f)) s = t = (float)(1.0 / std::sqrt(norm_bound(p->max_w, p->max_m)));
     if (p->lambda_conv == PD_LAMBDA_DATA) {
         *alpha = 1.0f / p->lambda_user;
         *sigma = s / p->lambda_user;
@@ -356,11 +358,13 @@ template <int NY> void sfd_launch_init_cols(const StreamFdArgs &a, cudaStream_t 
 }
 template <int NY> void sfd_launch_cols(const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid(a.nx / 16, a.npairs);
-    pdk::sfd_cols_kernel<NY, false><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, 1);
+    if (a.nx == NY) pdk::sfd_cols_kernel<NY, false, NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, 1);
+    else pdk::sfd_cols_kernel<NY, false, 0><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, 1);
 }
 template <int NY> void sfd_launch_cols_plain(const StreamFdArgs &a, int n, int decide, cudaStream_t st) {
     dim3 grid(a.nx / 16, a.npairs);
-    pdk::sfd_cols_kernel<NY, true><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
+    if (a.nx == NY) pdk::sfd_cols_kernel<NY, true, NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
+    else pdk::sfd_cols_kernel<NY, true, 0><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
 }
 template <int NX> void sfd_launch_dual_rows(const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid(a.ny / pdk::SfdRowCfg<NX>::G, a.npairs);
@@ -368,11 +372,10 @@ template <int NX> void sfd_launch_dual_rows(const StreamFdArgs &a, int n, cudaSt
 }
 template <int NY>
 cudaError_t sfd_set_col_smem() {
-    cudaError_t e = cudaFuncSetAttribute(pdk::sfd_cols_kernel<NY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         pdk::SfdColCfg<NY>::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(pdk::sfd_cols_kernel<NY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             pdk::SfdColCfg<NY>::SMEM_BYTES);
+    cudaError_t e = cudaSuccess;
+    auto set = [&](auto kern) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, pdk::SfdColCfg<NY>::SMEM_BYTES); };
+    set(pdk::sfd_cols_kernel<NY, false, NY>); set(pdk::sfd_cols_kernel<NY, false, 0>);
+    set(pdk::sfd_cols_kernel<NY, true, NY>); set(pdk::sfd_cols_kernel<NY, true, 0>);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(pdk::sfd_init_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 pdk::SfdColCfg<NY>::SMEM_BYTES);
@@ -834,7 +837,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     if (batch < 1 || (B0_dir != PD_B0_X && B0_dir != PD_B0_Y)) return PD_EINVAL;
     const bool generic = !(size_ok(nx) && size_ok(ny));
     if (generic && !(gen_size_ok(nx) && gen_size_ok(ny))) return PD_ESIZE;
-    int rc = check_params(lambda, sigma, tau, theta, false);
+    int rc = check_params(lambda, sigma, tau, theta, false, norm_bound(1.0, 1.0));
     if (rc != PD_OK) return rc;
 
     pd_plan_s *p = new (std::nothrow) pd_plan_s;
@@ -846,6 +849,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
     p->nx = nx; p->ny = ny; p->batch = batch; p->npairs = (batch + 1) / 2; p->b0_dir = B0_dir;
     p->lambda_user = lambda; p->sigma_user = sigma; p->tau_user = tau; p->theta = theta;
     p->check_every = 1;
+    p->max_w = p->max_m = 1.0;
     p->hybrid_tail = -1;
     p->graph_loop = 1;
     {
@@ -954,9 +958,20 @@ int pd_set_b0_angle(pd_plan_t p, float angle_rad) {
 
 int pd_set_steps(pd_plan_t p, float lambda, float sigma, float tau, float theta) {
     if (!p) return PD_EINVAL;
-    int rc = check_params(lambda, sigma, tau, theta, p->unsafe_steps != 0);
+    int rc = check_params(lambda, sigma, tau, theta, p->unsafe_steps != 0, norm_bound(p->max_w, p->max_m));
     if (rc != PD_OK) return rc;
     p->lambda_user = lambda; p->sigma_user = sigma; p->tau_user = tau; p->theta = theta;
+    return PD_OK;
+}
+
+int pd_set_norm_bounds(pd_plan_t p, float max_abs_w, float max_abs_m) {
+    if (!p || !(max_abs_w > 0.f) || !(max_abs_m > 0.f) || !std::isfinite(max_abs_w) || !std::isfinite(max_abs_m)) return PD_EINVAL;
+    // explicit steps already in the plan must satisfy the new bound too
+    const int rc = check_params(p->lambda_user, p->sigma_user, p->tau_user, p->theta, p->unsafe_steps != 0,
+                                norm_bound((double)max_abs_w, (double)max_abs_m));
+    if (rc != PD_OK) return rc;
+    p->max_w = (double)max_abs_w;
+    p->max_m = (double)max_abs_m;
     return PD_OK;
 }
 

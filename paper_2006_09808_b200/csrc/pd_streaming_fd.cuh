@@ -269,7 +269,10 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
 // partner); the mirror column is in this CTA.
 // PLAIN (literal path): only Z <- column FFT of conj(D/(nx ny) X^), i.e. one application of K between two row passes;
 // `decide` is set for the first of the two column launches of an iteration.
-template <int NY, bool PLAIN>
+// NXC: the row length as a compile-time constant (square slices: NXC = NY) or 0 (taken from the arguments).  With a
+// constant row pitch every access of a thread is base + immediate; with a run-time pitch the 64-bit address arithmetic
+// of the five strided arrays was 28 % of the instructions of the 512-point kernel (profiles/r02/README.md).
+template <int NY, bool PLAIN, int NXC>
 __global__ void __launch_bounds__(SfdColCfg<NY>::THREADS, SfdColCfg<NY>::THREADS <= 128 ? 4 : 2)
 sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     const int n = n_arg >= 0 ? n_arg : *a.iter;      // inside the graphed loop the iteration number lives on the device
@@ -314,7 +317,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     TwiddlesSmem<NY, true>::fill(tws, a.tw_col, threadIdx.x, NT);
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
     const int h = c >> 3, cc = c & 7;
-    const int nx = a.nx;
+    const int nx = NXC ? NXC : a.nx;
     const int kx = sfd_column_of(nx, blockIdx.x, h, cc);
     const bool self_mirror = (blockIdx.x == 0 && cc == 0);
     float2 *smg = smc + c * Cfg::CS;

@@ -550,6 +550,33 @@ def test_repeatable_and_plan_reuse(torch, pd):
     plan.destroy()
 
 
+def test_norm_bounds_for_automatic_steps(torch, pd, oracle, variant):
+    """pd_set_norm_bounds (R14): mask values up to 2 and weights up to 1.5 with the automatic steps
+    sigma = tau = 1/sqrt(4/9 max|W|^2 + 8 max|M|^2); PD_ESTEP follows the same bound."""
+    case = synth.random_case(64, 64, 3, seed=14, with_mask=True, with_weight=True)
+    m, w = 2.0 * case["mask"], 1.5 * case["weight"]
+    step = 1.0 / np.sqrt(4.0 / 9.0 * 1.5 ** 2 + 8.0 * 2.0 ** 2)
+    batch, ny, nx = case["field"].shape
+    plan = pd.Plan(nx, ny, batch, pd.B0_Y, 0.3, 0.0, 0.0, 1.0)       # sigma = tau = 0: automatic
+    if variant == "streaming":
+        plan.set_option(pd.OPT_VARIANT, pd.VARIANT_STREAMING)
+    plan.set_norm_bounds(1.5, 2.0)
+    f, mm, ww = (torch.from_numpy(a).cuda() for a in (case["field"], m, w))
+    plan.set_weight(ww)
+    out = torch.empty_like(f)
+    plan.solve(f, mm, out, 25, 0.0)
+    torch.cuda.synchronize()
+    o = oracle.solve(case["field"], m, w, lambda_=0.3, sigma=step, tau=step, max_iters=25)
+    assert slice_rel(out.cpu().numpy(), o["chi"]).max() < 2e-5
+    with pytest.raises(pd.PdError) as e:     # 0.25 * 0.25 * (1 + 32) > 1 under the stated bounds
+        plan.set_steps(0.3, 0.25, 0.25)
+    assert e.value.code == pd.ESTEP
+    with pytest.raises(pd.PdError) as e:
+        plan.set_norm_bounds(0.0, 1.0)
+    assert e.value.code == pd.EINVAL
+    plan.destroy()
+
+
 def test_runtime_errors(torch, pd):
     plan = pd.Plan(64, 64, 2)
     f = torch.zeros(2, 64, 64, device="cuda")

@@ -43,24 +43,26 @@ KERNEL_BYTES_PER_PX = {
     "fd_rows": 40.0,      # Z r4 w4 + chi_n r4 + chi_{n-1} r4 + chi_{n+1} w4 + qx r4 w4 + qy r4 w4 + M r4 (36 without a mask)
 }
 # DRAM bytes per pixel of a slice per launch measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one
-# `--set full` capture over the whole batch, profiles/r01/ncu_sfd_*): (kernel, line length, masked) -> B/px
+# `--set full` capture over the whole batch): (kernel, line length, masked) -> B/px
 NCU_DRAM_BYTES_PER_PX = {
-    ("fd_rows", 512, False): 35.2,   # ncu_sfd_rows_c4_v2.txt: 1.342 + 1.020 GB over 256 slices of 512x512
-    ("fd_cols", 512, False): 21.2,   # ncu_sfd_cols_c4_v2.txt: 0.865 + 0.559 GB
-    ("fd_rows", 256, True): 39.3,    # ncu_sfd_rows_c3.txt: 1.611 + 1.028 GB over 1024 slices of 256x256
-    ("fd_cols", 256, True): 19.7,    # ncu_sfd_cols_c3.txt: 0.827 + 0.492 GB
+    ("fd_rows", 512, False): 35.8,   # profiles/r02/ncu_sfd_rows_c4.md: 1.376 + 1.027 GB over 256 slices of 512x512 (36 algorithmic)
+    ("fd_cols", 512, False): 20.4,   # profiles/r02/ncu_sfd_cols_c4.md: 0.872 + 0.495 GB (20 algorithmic)
+    ("fd_rows", 256, True): 39.3,    # profiles/r01/ncu_sfd_rows_c3.txt: 1.611 + 1.028 GB over 1024 slices of 256x256 (40 algorithmic)
+    ("fd_cols", 256, True): 19.7,    # profiles/r01/ncu_sfd_cols_c3.txt: 0.827 + 0.492 GB
 }
 PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
 
 # What ncu measured on the resident kernel of THIS build (profiles/r02/, one `--set full` capture of the kernel alone on
 # C2 and one metrics-only pass over every launch of a hybrid C3 step); quoted beside the live numbers, never timed here.
 NCU_RESIDENT = {
-    "source": "profiles/r02/ncu_resident_tm_c2.txt, profiles/r02/dram_bytes_C3_hybrid_step.md",
-    "issue_slots_busy_pct": None, "fma_pipe_pct": None, "l1tex_pct": None, "l2_pct": None, "shared_wavefronts_pct_of_peak": None,
-    "l2_bytes_per_pixel_pair_iteration": None,
+    "source": "profiles/r02/ncu_resident_tm_c2.md (kernel alone on C2, hybrid tail off), profiles/r02/dram_bytes_C3_hybrid_step.md",
+    "issue_slots_busy_pct": 42.4, "fma_pipe_pct": 39.1, "l1tex_pct": 54.5, "l2_pct": 11.4, "dram_pct": 0.06,
+    "shared_wavefronts_pct_of_peak": 55.2,          # 593.9 M wavefronts / (120 SMs x 8.97 M active cycles), 1 wavefront/clk/SM
+    "l2_bytes_per_pixel_pair_iteration": 51.7,      # lts__t_sectors 677.5 M x 32 B / (32 pairs x 200 iterations x 65536)
+    "warps_per_scheduler": 4.0, "cycles_per_issue": 9.45,
 }
 # dram__bytes_read.sum + dram__bytes_write.sum summed over every launch of one step (resident kernel + streaming tail)
-NCU_DRAM_BYTES_PER_STEP = {}   # (workload, hybrid_tail_pairs) -> bytes
+NCU_DRAM_BYTES_PER_STEP = {("C3", 47): 81401493248.0}   # (workload, hybrid_tail_pairs) -> bytes (profiles/r02/dram_bytes_C3_hybrid_step.md)
 
 
 def load_peaks():
@@ -365,7 +367,13 @@ def main():
         # max(shared memory, FP32 pipe): report the FP32 fraction, the ncu percentages beside it.
         flops = flops_per_slice_it * slice_its_local
         achieved = flops / (dom_ms / dom_n * 1e-3) / 1e12
-        traffic = NCU_DRAM_BYTES_PER_STEP.get((args.workload, plan_info.get("hybrid_tail_pairs", 0)))
+        # the ncu pass was taken at the tail the plan chose on that box; a plan whose measured rho gives a tail within 4
+        # pairs of it is the same step to 5 % (the tail's share of the traffic is proportional to its pairs)
+        tail_now = plan_info.get("hybrid_tail_pairs", 0)
+        traffic = None
+        for (wl, tl), byts in NCU_DRAM_BYTES_PER_STEP.items():
+            if wl == args.workload and abs(tl - tail_now) <= 4:
+                traffic = byts * (tail_now / tl if tl else 1.0)
         roofline = dict(common, bound="alu", achieved=achieved, peak=alu_peak, unit="TFLOP/s", frac=achieved / alu_peak,
                         traffic=traffic, peak_source=alu_src, flops_per_launch=flops,
                         flops_model="P (10 log2 P + 32) per slice-iteration (SURVEY.md 8(d)); the Fourier-domain dual executes "

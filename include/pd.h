@@ -66,10 +66,13 @@ enum pd_option {
                                 is cached in the plan and rebuilt when the arguments of pd_solve change.  0: one stream
                                 launch per kernel, 2*max_iters + 4 of them (the kernels of a stopped slice return at once).
                                 PD_OPT_KERNEL_TIMING = 1 always uses plain launches. */
-    PD_OPT_REGULARISER = 10  /* PD_REG_TV (default): the paper's lambda ||M G chi||_1 with the dual q.
+    PD_OPT_REGULARISER = 10, /* PD_REG_TV (default): the paper's lambda ||M G chi||_1 with the dual q.
                                 PD_REG_L1: lambda ||M chi||_1 (BASELINE.json north_star's alternative):
                                 no q, the primal step ends in the soft shrinkage chi <- sign(v) max(|v| - tau lambda M, 0);
                                 relgap is then the Fenchel-Young gap of the data term alone.  PD_OPT_TV_MODE is ignored. */
+    PD_OPT_HOST_CHUNKING = 11 /* pd_solve_host: 0 (default) cut the batch into pipelined chunks when every chunk still fills the
+                                GPU (resident: whole waves of clusters; streaming: >= 2 row CTAs per SM per launch), 1 always
+                                (when the batch has enough slice pairs), 2 never */
 };
 enum { PD_REG_TV = 0, PD_REG_L1 = 1 };
 /* kernel classes for pd_get_kernel_times.  Streaming variant: init, finish and, per iteration, fd_cols + fd_rows

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libpd_b200.so")
 
 B0_X, B0_Y = 0, 1
 OK, EINVAL, ESIZE, ESTEP, ENOMEM, ECUDA, EVARIANT = 0, -1, -2, -3, -4, -5, -6
-OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING, OPT_FOURIER_DUAL, OPT_HYBRID_TAIL, OPT_GRAPH_LOOP, OPT_REGULARISER = range(11)
+OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING, OPT_FOURIER_DUAL, OPT_HYBRID_TAIL, OPT_GRAPH_LOOP, OPT_REGULARISER, OPT_HOST_CHUNKING = range(12)
 REG_TV, REG_L1 = 0, 1
 KERNEL_CLASSES = ["init", "dual_rows", "dipole_cols", "primal_rows", "finish", "resident", "fd_cols", "fd_rows"]
 TV_ISO, TV_ANISO = 0, 1

@@ -57,6 +57,7 @@ struct pd_plan_s {
     int tv_mode, lambda_conv, variant, check_every, mask_shared, unsafe_steps, no_fd;
     int generic;           // a size that is not a power of two: general-length kernels (pd_streaming_gen.cuh), literal iteration
     pdk::GenDims gdims;
+    int host_chunking;     // PD_OPT_HOST_CHUNKING: 0 automatic, 1 always, 2 never
     int reg_l1;            // PD_OPT_REGULARISER = PD_REG_L1
     double max_w, max_m;   // bounds on |W| and |M| behind the automatic steps and the PD_ESTEP check (pd_set_norm_bounds; 1, 1)
     int use_angle;         // oblique in-plane B0 (pd_set_b0_angle)
@@ -349,8 +350,13 @@ template <int NX> void sfd_launch_rows(const StreamFdArgs &a, int n, cudaStream_
         else pdk::sfd_rows_l1_kernel<NX, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
         return;
     }
-    if (a.mask) pdk::sfd_rows_kernel<NX, true><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
-    else pdk::sfd_rows_kernel<NX, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+    if (a.aniso) {
+        if (a.mask) pdk::sfd_rows_kernel<NX, true, true><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+        else pdk::sfd_rows_kernel<NX, false, true><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+        return;
+    }
+    if (a.mask) pdk::sfd_rows_kernel<NX, true, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
+    else pdk::sfd_rows_kernel<NX, false, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
 }
 template <int NY> void sfd_launch_init_cols(const StreamFdArgs &a, cudaStream_t st) {
     dim3 grid(a.nx / 16, a.npairs);
@@ -1010,6 +1016,9 @@ int pd_set_option(pd_plan_t p, int key, int value) {
         case PD_OPT_REGULARISER:
             if (value != PD_REG_TV && value != PD_REG_L1) return PD_EINVAL;
             p->reg_l1 = (value == PD_REG_L1); return PD_OK;
+        case PD_OPT_HOST_CHUNKING:
+            if (value < 0 || value > 2) return PD_EINVAL;
+            p->host_chunking = value; return PD_OK;
         case PD_OPT_GRAPH_LOOP:
             if (value != 0 && value != 1) return PD_EINVAL;
             p->graph_loop = value; return PD_OK;
@@ -1040,7 +1049,13 @@ int host_chunks(const pd_plan_s *p, int *count /*[kMaxChunks]*/) {
     if (unit < 1) unit = 1;
     const int np = p->npairs;
     int n = 0, left = np;
-    if (res && np >= 24 * unit) {     // 1, 4, middle, 4, 2 units
+    // A streaming chunk must still fill the GPU with every launch (its time per iteration is bounded below by launch
+    // latency, not by work): automatic chunking only when the smallest chunk has at least two row CTAs per SM.  E1
+    // (13 pairs of 256x258) in three chunks took 126 ms end to end against 75 ms on device buffers.
+    bool chunk = p->host_chunking != 2;
+    if (chunk && p->host_chunking == 0 && !res) chunk = (long long)unit * p->nparts >= 2LL * p->num_sms;
+    if (!chunk) {
+    } else if (res && np >= 24 * unit) {     // 1, 4, middle, 4, 2 units
         const int head[2] = {unit, 4 * unit}, tail[2] = {4 * unit, 2 * unit};
         count[n++] = 2 * head[0]; count[n++] = 2 * head[1];
         count[n++] = 2 * (np - head[0] - head[1] - tail[0] - tail[1]);

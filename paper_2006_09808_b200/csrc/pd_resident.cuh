@@ -98,8 +98,21 @@ __device__ __forceinline__ float2 ldcg2(const float2 *p) { return __ldcg(p); }
 constexpr bool kResidentFastProj = PD_RESIDENT_FAST_PROJECTION != 0, kStreamingFastProj = PD_STREAMING_FAST_PROJECTION != 0;
 template <bool FAST>
 __device__ __forceinline__ float proj_scale(const float alpha, const float n2) {
-    if constexpr (FAST) return alpha * rsqrtf(n2);
-    else return __fdiv_rn(alpha, __fsqrt_rn(n2));
+    if constexpr (FAST) {
+        // ONE MUFU instruction (rsqrtf() wraps it in a denormal rescue of four more).  A denormal |t|^2 is flushed to 0,
+        // rsqrt gives inf and min(1, alpha inf) leaves such a t (|t| < 1e-19) unscaled: the same as |t| <= alpha.
+        float r;
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(n2));
+        return alpha * r;
+    } else {
+        return __fdiv_rn(alpha, __fsqrt_rn(n2));
+    }
+}
+// min(1, alpha / |t|): the factor of the isotropic projection, R13-safe (alpha = 0 gives 0; |t| = 0 gives 1 on a zero vector)
+template <bool FAST>
+__device__ __forceinline__ float proj_factor(const float alpha, const float alpha_sq, const float n2) {
+    if constexpr (FAST) return fminf(proj_scale<true>(alpha, n2), 1.f);   // fminf(NaN, 1) = 1 covers 0 * inf
+    else return (n2 > alpha_sq) ? proj_scale<false>(alpha, n2) : 1.f;
 }
 template <bool FAST>
 __device__ __forceinline__ float gap_sqrt(const float x) {
@@ -216,8 +229,8 @@ __device__ __forceinline__ void q_update_row(const RowPtrs &r, const ResidentArg
         } else {
             const float2 n2 = fma2(ty, ty, mul2(tx, tx));
             float2 sc;
-            sc.x = (n2.x > alpha_sq.x) ? proj_scale<kResidentFastProj>(alpha.x, n2.x) : 1.f;  // alpha/|t| where |t| > alpha, else 1 (R13: alpha=0 -> 0)
-            sc.y = (n2.y > alpha_sq.y) ? proj_scale<kResidentFastProj>(alpha.y, n2.y) : 1.f;
+            sc.x = proj_factor<kResidentFastProj>(alpha.x, alpha_sq.x, n2.x);  // alpha/|t| where |t| > alpha, else 1 (R13: alpha=0 -> 0)
+            sc.y = proj_factor<kResidentFastProj>(alpha.y, alpha_sq.y, n2.y);
             tx = mul2(tx, sc);
             ty = mul2(ty, sc);
         }

@@ -213,8 +213,8 @@ __device__ __forceinline__ void q_update_tm(const TmRow<N, NT> &r, const Residen
                 ty.y = fminf(fmaxf(ty.y, -alpha.y), alpha.y);
             } else {
                 const float2 n2 = fma2(ty, ty, mul2(tx, tx));
-                const float2 sc = make_float2(fminf(proj_scale<kResidentFastProj>(alpha.x, n2.x), 1.f),
-                                              fminf(proj_scale<kResidentFastProj>(alpha.y, n2.y), 1.f));
+                const float2 sc = make_float2(proj_factor<kResidentFastProj>(alpha.x, alpha.x * alpha.x, n2.x),
+                                              proj_factor<kResidentFastProj>(alpha.y, alpha.y * alpha.y, n2.y));
                 tx = mul2(tx, sc);
                 ty = mul2(ty, sc);
             }

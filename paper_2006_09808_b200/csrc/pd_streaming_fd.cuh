@@ -452,8 +452,8 @@ __device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float2
     } else {
         const float2 n2 = fma2(ty, ty, mul2(tx, tx));
         float2 sc;
-        sc.x = (n2.x > alpha_sq.x) ? proj_scale<kStreamingFastProj>(alpha.x, n2.x) : 1.f;
-        sc.y = (n2.y > alpha_sq.y) ? proj_scale<kStreamingFastProj>(alpha.y, n2.y) : 1.f;
+        sc.x = proj_factor<kStreamingFastProj>(alpha.x, alpha_sq.x, n2.x);
+        sc.y = proj_factor<kStreamingFastProj>(alpha.y, alpha_sq.y, n2.y);
         tx = mul2(tx, sc);
         ty = mul2(ty, sc);
     }
@@ -464,7 +464,7 @@ __device__ __forceinline__ void sfd_project(float2 &tx, float2 &ty, const float2
 //   q_{n+1} = proj_alpha(q_n + sigma M G chibar_n) for row y (stored) and, redundantly, its qy for row y-1
 //   d = G^T (M q_{n+1}) ; chi_{n+1} = chi_n - tau (v + d) ; chibar_{n+1} = chi_{n+1} + theta (chi_{n+1} - chi_n)
 //   Z <- row FFT of chibar_{n+1}
-template <int NX, bool MASKED>
+template <int NX, bool MASKED, bool ANISO>
 __global__ void __launch_bounds__(SfdRowCfg<NX>::THREADS, SfdRowCfg<NX>::MINB)
 sfd_rows_kernel(const StreamFdArgs a, const int n_arg) {
     const int n = n_arg >= 0 ? n_arg : *a.iter;
@@ -521,7 +521,7 @@ sfd_rows_kernel(const StreamFdArgs a, const int n_arg) {
     const float2 sig2 = splat(a.sigma), zero = make_float2(0.f, 0.f);
     const float2 alpha = make_float2(a.alpha * a.cscale[s0], (s1 < a.batch) ? a.alpha * a.cscale[s1] : 0.f);
     const float2 alpha_sq = mul2(alpha, alpha);
-    const bool aniso = a.aniso != 0;
+    constexpr bool aniso = ANISO;   // a template parameter: as a run-time flag both projections were computed and selected
     const float2 ntau2 = splat(-a.tau), ntau_v = make_float2(-a.tau, a.tau), theta2 = splat(a.theta);
     const float2 actm = make_float2(act0 ? 1.f : 0.f, act1 ? 1.f : 0.f);
     float2 gap = zero, dn = zero, cn = zero, mqx_prev = zero;

@@ -454,12 +454,13 @@ def test_config4_full_tolerance_stop_sampled(torch, pd, oracle):
 def test_host_entry_pipeline_chunks(torch, pd, oracle, ny, nx, batch, variant_):
     """pd_solve_host cuts a large batch into chunks (upload k+1 || solve k || download k-1 on plan-owned streams): same
     chi and statistics as pd_solve on device buffers -- bit for bit where every slice runs through the same kernels
-    (64x64: five chunks of resident waves; 64x128: five chunks of graphed streaming loops, odd batch), within the
+    (64x64: five chunks of resident waves; 64x128: three chunks of graphed streaming loops, odd batch), within the
     one-iteration gate where the hybrid tail may land elsewhere (256x256) -- and as the oracle on sampled slices."""
     case = synth.random_case(nx, ny, batch, seed=batch + nx, with_mask=True)
     iters, tol = (12, 0.0) if variant_ == "auto" else (40, 5e-2)
     dev = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, tol=tol, variant=variant_)
-    host = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, tol=tol, variant=variant_, host=True)
+    host = gpu_solve(torch, pd, case["field"], case["mask"], iters, lam=0.2, tol=tol, variant=variant_, host=True,
+                     options=[(pd.OPT_HOST_CHUNKING, 1)])   # small streaming batches are not chunked automatically
     assert np.array_equal(host["iters_done"], dev["iters_done"])
     if nx == 256:
         assert slice_rel(host["chi"], dev["chi"]).max() < TOL_1IT

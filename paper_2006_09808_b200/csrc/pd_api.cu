@@ -368,7 +368,7 @@ template <int NY> void sfd_launch_cols(const StreamFdArgs &a, int n, cudaStream_
     else pdk::sfd_cols_kernel<NY, false, 0><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, 1);
 }
 template <int NY> void sfd_launch_cols_plain(const StreamFdArgs &a, int n, int decide, cudaStream_t st) {
-    dim3 grid(a.nx / 16, a.npairs);
+    dim3 grid((a.nx + 15) / 16, a.npairs);
     if (a.nx == NY) pdk::sfd_cols_kernel<NY, true, NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
     else pdk::sfd_cols_kernel<NY, true, 0><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
 }
@@ -620,19 +620,19 @@ int solve_range(pd_plan_s *p, const float *field, const float *mask, float *chi_
     } while (0)
 
 // The iteration kernels of one PD iteration (n < 0: inside the graphed loop, the kernels read the device counter)
-size_t gen_rows_smem(const pd_plan_s *p) { return (size_t)(1 + 2 * pdk::kGenRows) * p->nx * sizeof(float2); }
-size_t gen_cols_smem(const pd_plan_s *p) { return (size_t)(1 + 2 * pdk::kGenColsB) * p->ny * sizeof(float2); }
+size_t gen_rows_smem(const pd_plan_s *p) { return (size_t)(pdk::gen_wsize(p->nx) + 2 * pdk::kGenRows * p->nx) * sizeof(float2); }
+size_t gen_cols_smem(const pd_plan_s *p) { return (size_t)(pdk::gen_wsize(p->ny) + 2 * pdk::kGenColsB * p->ny) * sizeof(float2); }
 void gen_launch_cols(const pd_plan_s *p, const StreamFdArgs &a, int n, int decide, cudaStream_t st) {
     dim3 grid((a.nx + pdk::kGenColsB - 1) / pdk::kGenColsB, a.npairs);
     pdk::gen_cols_kernel<<<grid, 32 * pdk::kGenColsB, gen_cols_smem(p), st>>>(a, p->gdims, n, decide);
 }
 void gen_launch_dual_rows(const pd_plan_s *p, const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid((a.ny + pdk::kGenRows - 1) / pdk::kGenRows, a.npairs);
-    pdk::gen_dual_rows_kernel<<<grid, 32 * pdk::kGenRows, gen_rows_smem(p), st>>>(a, p->gdims, n);
+    pdk::gen_dual_rows_kernel<<<grid, pdk::kGenLT * pdk::kGenRows, gen_rows_smem(p), st>>>(a, p->gdims, n);
 }
 void gen_launch_rows(const pd_plan_s *p, const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid((a.ny + pdk::kGenRows - 1) / pdk::kGenRows, a.npairs);
-    pdk::gen_rows_kernel<<<grid, 32 * pdk::kGenRows, gen_rows_smem(p), st>>>(a, p->gdims, n);
+    pdk::gen_rows_kernel<<<grid, pdk::kGenLT * pdk::kGenRows, gen_rows_smem(p), st>>>(a, p->gdims, n);
 }
 void gen_launch_init(const pd_plan_s *p, const StreamFdArgs &a, int which, cudaStream_t st) {
     if (which == 0) {
@@ -643,11 +643,18 @@ void gen_launch_init(const pd_plan_s *p, const StreamFdArgs &a, int which, cudaS
     }
 }
 
+// column pass of the general-length path: ny a power of two -> the tuned PLAIN column kernel over contiguous column
+// blocks (run-time row pitch); else the dense general-length kernel
+void gen_cols_any(const pd_plan_s *p, const StreamFdArgs &a, int n, int decide, cudaStream_t st) {
+    if (a.cols_contig) { PD_DISPATCH(p->ny, sfd_launch_cols_plain, a, n, decide, st); }
+    else gen_launch_cols(p, a, n, decide, st);
+}
+
 void sfd_enqueue_iteration(const pd_plan_s *p, const StreamFdArgs &a, bool literal, int n, cudaStream_t st) {
-    if (p->generic) {   // general-length kernels, literal iteration
-        if (n != 0) gen_launch_cols(p, a, n, 1, st);
+    if (p->generic) {   // general-length kernels, literal iteration; a power-of-two ny keeps the tuned column transform
+        if (n != 0) gen_cols_any(p, a, n, 1, st);
         gen_launch_dual_rows(p, a, n, st);
-        gen_launch_cols(p, a, n, 0, st);
+        gen_cols_any(p, a, n, 0, st);
         gen_launch_rows(p, a, n, st);
         return;
     }
@@ -765,6 +772,7 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     const bool literal = p->weight != nullptr || p->no_fd || p->generic;   // p in the image domain, K applied twice (PAPER.md:49 literally)
     a.literal = literal ? 1 : 0;
     a.reg_l1 = p->reg_l1;
+    a.cols_contig = (p->generic && size_ok(p->ny)) ? 1 : 0;
     a.weight = p->weight ? p->weight + (size_t)first * P : nullptr;
     a.field = field + (size_t)first * P;
     a.mask = mask ? mask + (size_t)first * (size_t)a.mask_bstride : nullptr;
@@ -809,9 +817,9 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
     }
     for (int n = 0; n < max_iters; ++n) {
         if (p->generic) {
-            if (n > 0) PD_LAUNCH(PD_KERNEL_COLS, gen_launch_cols(p, a, n, 1, st));
+            if (n > 0) PD_LAUNCH(PD_KERNEL_COLS, gen_cols_any(p, a, n, 1, st));
             PD_LAUNCH(PD_KERNEL_DUAL, gen_launch_dual_rows(p, a, n, st));
-            PD_LAUNCH(PD_KERNEL_COLS, gen_launch_cols(p, a, n, 0, st));
+            PD_LAUNCH(PD_KERNEL_COLS, gen_cols_any(p, a, n, 0, st));
             PD_LAUNCH(PD_KERNEL_FD_ROWS, gen_launch_rows(p, a, n, st));
             continue;
         }
@@ -898,7 +906,7 @@ int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda,
         if (e == cudaSuccess) e = sfd_set_col_smem<512>();
         if (e == cudaSuccess && generic) {
             // the attribute belongs to the function, not to the plan: always the largest supported length (1024)
-            const int cmax = (1 + 2 * pdk::kGenColsB) * 1024 * (int)sizeof(float2), rmax = (1 + 2 * pdk::kGenRows) * 1024 * (int)sizeof(float2);
+            const int cmax = (pdk::gen_wsize(1024) + 2 * pdk::kGenColsB * 1024) * (int)sizeof(float2), rmax = (pdk::gen_wsize(1024) + 2 * pdk::kGenRows * 1024) * (int)sizeof(float2);
             e = cudaFuncSetAttribute(pdk::gen_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, cmax);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(pdk::gen_dual_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rmax);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(pdk::gen_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rmax);

@@ -42,6 +42,8 @@ struct StreamFdArgs {
     float2 *W2;                              // literal path only: interleaved W; phihat then holds phi itself
     int literal;                             // 1: W != I or PD_OPT_FOURIER_DUAL = 0 (p kept in the image domain)
     int reg_l1;                              // 1: PD_REG_L1 (l1 on chi, shrinkage) instead of the paper's TV term
+    int cols_contig;                         // PLAIN column kernel only: CTA cb owns the columns [16 cb, 16 cb + 16) below nx (nx need
+                                             // not be a multiple of 16: the general-length path with a power-of-two ny) instead of mirror pairs
     float2 *phat[2], *qx2[2], *qy2[2];       // double-buffered by iteration parity: iteration n reads [n&1]
     float2 *chi3[3];                         // chi_n in [n%3], chi_{n-1} in [(n+2)%3], chi_{n+1} written to [(n+1)%3]
     const float *Dtab;                       // D/(nx*ny), [ny][nx]
@@ -318,7 +320,10 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
     const int h = c >> 3, cc = c & 7;
     const int nx = NXC ? NXC : a.nx;
-    const int kx = sfd_column_of(nx, blockIdx.x, h, cc);
+    // PLAIN with cols_contig: a ragged last block; its surplus threads redo column nx - 1 (they must reach the barriers) and do not store
+    const int kx_raw = (PLAIN && a.cols_contig) ? 16 * (int)blockIdx.x + c : sfd_column_of(nx, blockIdx.x, h, cc);
+    const bool kx_valid = kx_raw < nx;
+    const int kx = kx_valid ? kx_raw : nx - 1;
     const bool self_mirror = (blockIdx.x == 0 && cc == 0);
     float2 *smg = smc + c * Cfg::CS;
     const float2 *smg_mir = self_mirror ? smg : smc + (c ^ 8) * Cfg::CS;
@@ -417,8 +422,10 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
         }
     }
     fft_line<NY, T>(v, smg, j, tw, BlockSync());
+    if (kx_valid) {
 #pragma unroll
-    for (int m = 0; m < E; ++m) __stcs(zc + (long long)(j + T * m) * nx, v[m]);
+        for (int m = 0; m < E; ++m) __stcs(zc + (long long)(j + T * m) * nx, v[m]);
+    }
 
     if (want_gap) {   // CTA sums in fixed order: warp shuffles, then warp 0 over the per-warp values
         __syncthreads();

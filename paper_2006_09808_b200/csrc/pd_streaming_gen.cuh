@@ -21,45 +21,58 @@
 
 namespace pdk {
 
-constexpr int kGenRows = 4;      // rows per CTA of the row kernels (one warp each)
+constexpr int kGenRows = 4;      // rows per CTA of the row kernels
+constexpr int kGenWPR = 2;       // warps per row in the row kernels: the paper's stacks are small (13 and 21 slice pairs), one warp
+                                 // per row left the GPU at 22 warps per SM; the two warps of a row meet at a named barrier
+constexpr int kGenLT = 32 * kGenWPR;
 constexpr int kGenColsB = 8;     // adjacent columns per CTA of the column kernel (64-byte segments)
 
 struct GenDims { int n1x, n2x, n1y, n2y; };   // nx = n1x * n2x, ny = n1y * n2y
 
-// Forward DFT of one line by one warp.  W: table W_N^e (shared memory).  src (stride 1) -> tmp -> dst (stride 1); src and
-// dst may be the same buffer.  Ends with a __syncwarp.
+// The twiddle table W_N^e sits in shared memory with one padding slot after every 16 entries: the lanes of a warp read
+// W[(lane-dependent multiple of a stride) mod N], and strides that are multiples of 8 or 16 entries (N2 = 16: every
+// access; N = 258: every eighth n2) would otherwise land in one or two banks (measured: 20 cycles per warp instruction).
+__host__ __device__ constexpr int gen_wsize(int n) { return n + (n >> 4) + 1; }
+__device__ __forceinline__ int gen_wp(const int e) { return e + (e >> 4); }
+
+// sum_k x[k * xs] W[(k * step) mod N], k = 0..cnt-1, with eight independent accumulation chains (two elements per trip,
+// every product its own chain): the loop is bound by the latency of dependent FMAs and shared-memory loads, not by their count
+__device__ __forceinline__ float2 gen_dot(const float2 *W, const int N, const float2 *x, const int xs, const int cnt, const int step) {
+    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f, b3 = 0.f;
+    int e = 0, k = 0;
+    for (; k + 1 < cnt; k += 2) {
+        int e1 = e + step;
+        if (e1 >= N) e1 -= N;
+        const float2 x0 = x[k * xs], w0 = W[gen_wp(e)], x1 = x[(k + 1) * xs], w1 = W[gen_wp(e1)];
+        e = e1 + step;
+        if (e >= N) e -= N;
+        a0 = fmaf(x0.x, w0.x, a0); a1 = fmaf(-x0.y, w0.y, a1); a2 = fmaf(x0.x, w0.y, a2); a3 = fmaf(x0.y, w0.x, a3);
+        b0 = fmaf(x1.x, w1.x, b0); b1 = fmaf(-x1.y, w1.y, b1); b2 = fmaf(x1.x, w1.y, b2); b3 = fmaf(x1.y, w1.x, b3);
+    }
+    if (k < cnt) {
+        const float2 x0 = x[k * xs], w0 = W[gen_wp(e)];
+        a0 = fmaf(x0.x, w0.x, a0); a1 = fmaf(-x0.y, w0.y, a1); a2 = fmaf(x0.x, w0.y, a2); a3 = fmaf(x0.y, w0.x, a3);
+    }
+    return make_float2((a0 + b0) + (a1 + b1), (a2 + b2) + (a3 + b3));
+}
+
+// Forward DFT of one line by LT cooperating threads (one or two warps).  W: padded table W_N^e (shared memory).
+// src -> tmp -> dst; src and dst may be the same buffer.  sync() synchronises the LT threads; the call ends with one.
+template <int LT, class Sync>
 __device__ __forceinline__ void gen_line_dft(const float2 *W, const int N, const int N1, const int N2, const float2 *src,
-                                             float2 *tmp, float2 *dst, const int lane) {
-    for (int o = lane; o < N; o += 32) {
+                                             float2 *tmp, float2 *dst, const int lane, const Sync sync) {
+    for (int o = lane; o < N; o += LT) {
         const int n1 = o / N2, k2 = o - n1 * N2;
-        float2 acc = make_float2(0.f, 0.f);
-        const int step = k2 * N1;   // W_N2^(n2 k2) = W_N^(n2 k2 N1)
-        int e = 0;
-        for (int n2 = 0; n2 < N2; ++n2) {
-            const float2 x = src[n1 + N1 * n2], w = W[e];
-            acc.x = fmaf(x.x, w.x, fmaf(-x.y, w.y, acc.x));
-            acc.y = fmaf(x.x, w.y, fmaf(x.y, w.x, acc.y));
-            e += step;
-            if (e >= N) e -= N;
-        }
-        tmp[o] = cmul(acc, W[n1 * k2]);
+        // Y[n1][k2] = W_N^(n1 k2) sum_n2 x[n1 + N1 n2] W_N2^(n2 k2),  W_N2^(n2 k2) = W_N^(n2 k2 N1)
+        tmp[o] = cmul(gen_dot(W, N, src + n1, N1, N2, k2 * N1), W[gen_wp(n1 * k2)]);
     }
-    __syncwarp();
-    for (int o = lane; o < N; o += 32) {
+    sync();
+    for (int o = lane; o < N; o += LT) {
         const int k1 = o / N2, k2 = o - k1 * N2;
-        float2 acc = make_float2(0.f, 0.f);
-        const int step = k1 * N2;   // W_N1^(n1 k1) = W_N^(n1 k1 N2)
-        int e = 0;
-        for (int n1 = 0; n1 < N1; ++n1) {
-            const float2 x = tmp[n1 * N2 + k2], w = W[e];
-            acc.x = fmaf(x.x, w.x, fmaf(-x.y, w.y, acc.x));
-            acc.y = fmaf(x.x, w.y, fmaf(x.y, w.x, acc.y));
-            e += step;
-            if (e >= N) e -= N;
-        }
-        dst[k2 + N2 * k1] = acc;
+        // X[k2 + N2 k1] = sum_n1 Y[n1][k2] W_N1^(n1 k1),  W_N1^(n1 k1) = W_N^(n1 k1 N2)
+        dst[k2 + N2 * k1] = gen_dot(W, N, tmp + k2, N2, N1, k1 * N2);
     }
-    __syncwarp();
+    sync();
 }
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -140,8 +153,8 @@ gen_cols_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg, const i
     if (do_decide && n == 0) return;   // chibar_0 = 0: the first K application of iteration 0 is skipped
     extern __shared__ __align__(16) unsigned char gen_smem[];
     const int nx = a.nx, ny = a.ny;
-    float2 *W = reinterpret_cast<float2 *>(gen_smem);          // [ny]
-    float2 *buf = W + ny;                                      // [kGenColsB][2][ny]
+    float2 *W = reinterpret_cast<float2 *>(gen_smem);          // [gen_wsize(ny)], padded (gen_wp)
+    float2 *buf = W + gen_wsize(ny);                           // [kGenColsB][2][ny]
     __shared__ float dec[2];
 
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
@@ -168,7 +181,7 @@ gen_cols_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg, const i
         if (dec[1] != 0.f) stop1 = n;
         if (n >= stop0 && n >= stop1) return;
     }
-    for (int i = threadIdx.x; i < ny; i += blockDim.x) W[i] = __ldg(a.tw_col + i);
+    for (int i = threadIdx.x; i < ny; i += blockDim.x) W[gen_wp(i)] = __ldg(a.tw_col + i);
     const int x0 = blockIdx.x * kGenColsB;
     const int ncols = nx - x0 < kGenColsB ? nx - x0 : kGenColsB;
     float2 *zb = a.Z + (long long)pair * nx * ny + x0;
@@ -181,7 +194,7 @@ gen_cols_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg, const i
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp < ncols) {
         float2 *l0 = buf + (warp * 2) * ny, *l1 = l0 + ny;
-        gen_line_dft(W, ny, gd.n1y, gd.n2y, l0, l1, l0, lane);
+        gen_line_dft<32>(W, ny, gd.n1y, gd.n2y, l0, l1, l0, lane, WarpSync());
         const float *dcol = a.Dtab + x0 + warp;
         for (int y = lane; y < ny; y += 32) {
             const float d = __ldg(dcol + (long long)y * nx);
@@ -189,7 +202,7 @@ gen_cols_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg, const i
             l0[y] = make_float2(d * v.x, -d * v.y);   // conj(D z^): the next forward transform is the conjugate of the inverse
         }
         __syncwarp();
-        gen_line_dft(W, ny, gd.n1y, gd.n2y, l0, l1, l0, lane);
+        gen_line_dft<32>(W, ny, gd.n1y, gd.n2y, l0, l1, l0, lane, WarpSync());
     }
     __syncthreads();
     for (int i = threadIdx.x; i < ny * kGenColsB; i += blockDim.x) {
@@ -201,39 +214,40 @@ gen_cols_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg, const i
 // ------------------------------------------------------------------------------------------------ dual rows
 // u = K chibar_n: the row DFT of Z gives (u_a, -u_b) (zero in iteration 0) ; p_{n+1} = (p_n + sigma W (u - phi))/(1 + sigma)
 // [PAPER.md:49 line 1; R2, R3] ; Z <- row DFT of W p_{n+1} ; data term of the gap 1/2 ||W(u - phi) - p_{n+1}||^2.
-__global__ void __launch_bounds__(32 * kGenRows)
+__global__ void __launch_bounds__(kGenLT * kGenRows)
 gen_dual_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
     const int n = n_arg >= 0 ? n_arg : *a.iter;
     extern __shared__ __align__(16) unsigned char gen_smem[];
     const int nx = a.nx;
-    float2 *W = reinterpret_cast<float2 *>(gen_smem);          // [nx]
-    __shared__ float red[kGenRows][2];
+    float2 *W = reinterpret_cast<float2 *>(gen_smem);          // [gen_wsize(nx)], padded (gen_wp)
+    __shared__ float red[kGenRows * kGenWPR][2];
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
     const bool act0 = n < a.stop_iter[s0];
     const bool act1 = (s1 < a.batch) && (n < a.stop_iter[s1]);
     if (!act0 && !act1) return;
     const bool last = (n + 1 == a.max_iters);
     const bool want_gap = last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0);
-    for (int i = threadIdx.x; i < nx; i += blockDim.x) W[i] = __ldg(a.tw_row + i);
+    for (int i = threadIdx.x; i < nx; i += blockDim.x) W[gen_wp(i)] = __ldg(a.tw_row + i);
     __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int y = blockIdx.x * kGenRows + warp;
-    float2 *l0 = W + nx + (warp * 2) * nx, *l1 = l0 + nx;
+    const int warp = threadIdx.x >> 5, grp = threadIdx.x / kGenLT, lane = threadIdx.x % kGenLT;   // grp: the row of this thread
+    const int y = blockIdx.x * kGenRows + grp;
+    float2 *l0 = W + gen_wsize(nx) + (grp * 2) * nx, *l1 = l0 + nx;
+    const NamedSync rowsync{1 + grp, kGenLT};
     float2 gap = make_float2(0.f, 0.f);
     if (y < a.ny) {
         const long long po = ((long long)pair * a.ny + y) * nx;
         float2 *zr = a.Z + po, *pw = a.phat[(n & 1) ^ 1] + po;
         const float2 *pr = a.phat[n & 1] + po, *phi = a.phihat + po, *W2 = a.W2 + po;
         if (n > 0) {
-            for (int x = lane; x < nx; x += 32) l0[x] = __ldcs(zr + x);
-            __syncwarp();
-            gen_line_dft(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane);
+            for (int x = lane; x < nx; x += kGenLT) l0[x] = __ldcs(zr + x);
+            rowsync();
+            gen_line_dft<kGenLT>(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane, rowsync);
         } else {
-            for (int x = lane; x < nx; x += 32) l0[x] = make_float2(0.f, 0.f);
+            for (int x = lane; x < nx; x += kGenLT) l0[x] = make_float2(0.f, 0.f);
         }
         const float2 sig2 = splat(a.sigma), inv2 = splat(a.inv_one_plus_sigma), half2 = splat(0.5f);
         const float2 sgn = make_float2(1.f, -1.f);   // lane y of the transform carries -u_b
-        for (int x = lane; x < nx; x += 32) {
+        for (int x = lane; x < nx; x += kGenLT) {
             const float2 w = __ldg(W2 + x);
             const float2 res = mul2(w, sub2(mul2(sgn, l0[x]), __ldg(phi + x)));
             const float2 pn = mul2(fma2(sig2, res, __ldg(pr + x)), inv2);
@@ -244,18 +258,18 @@ gen_dual_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
             __stcs(pw + x, pn);
             l0[x] = mul2(w, pn);
         }
-        __syncwarp();
-        gen_line_dft(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane);
-        for (int x = lane; x < nx; x += 32) __stcs(zr + x, l0[x]);
+        rowsync();
+        gen_line_dft<kGenLT>(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane, rowsync);
+        for (int x = lane; x < nx; x += kGenLT) __stcs(zr + x, l0[x]);
     }
     if (want_gap) {   // per-CTA partial sums, fixed order; read by sfd_gap_sum through gap_col (ncolparts = nrowparts)
         gap.x = warp_sum(gap.x);
         gap.y = warp_sum(gap.y);
-        if (lane == 0) { red[warp][0] = gap.x; red[warp][1] = gap.y; }
+        if ((lane & 31) == 0) { red[warp][0] = gap.x; red[warp][1] = gap.y; }
         __syncthreads();
         if (threadIdx.x < 2) {
             float t = 0.f;
-            for (int q = 0; q < kGenRows; ++q) t += red[q][threadIdx.x];
+            for (int q = 0; q < kGenRows * kGenWPR; ++q) t += red[q][threadIdx.x];
             a.gap_col[n & 1][((long long)pair * a.ncolparts + blockIdx.x) * 2 + threadIdx.x] = t;
         }
     }
@@ -267,24 +281,25 @@ gen_dual_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
 //   d = G^T (M q_{n+1}) ; chi_{n+1} = chi_n - tau (v + d) ; chibar_{n+1} = chi_{n+1} + theta (chi_{n+1} - chi_n)
 // or, with the l1 regulariser, chi_{n+1} = shrink(chi_n - tau v, tau alpha M).  chibar_n is recomputed from chi_n and
 // chi_{n-1} wherever it is needed (as in sfd_rows_kernel); neighbours are plain (cached) loads.  Z <- row DFT of chibar_{n+1}.
-__global__ void __launch_bounds__(32 * kGenRows)
+__global__ void __launch_bounds__(kGenLT * kGenRows)
 gen_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
     const int n = n_arg >= 0 ? n_arg : *a.iter;
     extern __shared__ __align__(16) unsigned char gen_smem[];
     const int nx = a.nx, ny = a.ny;
-    float2 *W = reinterpret_cast<float2 *>(gen_smem);          // [nx]
-    __shared__ float red[kGenRows][6];
+    float2 *W = reinterpret_cast<float2 *>(gen_smem);          // [gen_wsize(nx)], padded (gen_wp)
+    __shared__ float red[kGenRows * kGenWPR][6];
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
     const bool act0 = n < a.stop_iter[s0];
     const bool act1 = (s1 < a.batch) && (n < a.stop_iter[s1]);
     if (!act0 && !act1) return;
     const bool last = (n + 1 == a.max_iters);
     const bool want_gap = last || (a.tol > 0.f && ((n + 1) % a.check_every) == 0);
-    for (int i = threadIdx.x; i < nx; i += blockDim.x) W[i] = __ldg(a.tw_row + i);
+    for (int i = threadIdx.x; i < nx; i += blockDim.x) W[gen_wp(i)] = __ldg(a.tw_row + i);
     __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int y = blockIdx.x * kGenRows + warp;
-    float2 *l0 = W + nx + (warp * 2) * nx, *l1 = l0 + nx;
+    const int warp = threadIdx.x >> 5, grp = threadIdx.x / kGenLT, lane = threadIdx.x % kGenLT;   // grp: the row of this thread
+    const int y = blockIdx.x * kGenRows + grp;
+    float2 *l0 = W + gen_wsize(nx) + (grp * 2) * nx, *l1 = l0 + nx;
+    const NamedSync rowsync{1 + grp, kGenLT};
     const float2 zero = make_float2(0.f, 0.f);
     float2 gap = zero, dn = zero, cn = zero;
     if (y < ny) {
@@ -295,9 +310,9 @@ gen_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
         float2 *qxw = a.qx2[wr] + po, *qyw = a.qy2[wr] + po, *chiw = a.chi3[(n + 1) % 3] + po;
         const float2 *chn = a.chi3[n % 3] + po, *chp = a.chi3[(n + 2) % 3] + po;   // chi_n, chi_{n-1}
         const bool has_up = y > 0, has_down = y < ny - 1;
-        for (int x = lane; x < nx; x += 32) l0[x] = __ldcs(zr + x);
-        __syncwarp();
-        gen_line_dft(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane);
+        for (int x = lane; x < nx; x += kGenLT) l0[x] = __ldcs(zr + x);
+        rowsync();
+        gen_line_dft<kGenLT>(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane, rowsync);
 
         const float2 sig2 = splat(a.sigma), theta2 = splat(a.theta);
         const float2 alpha = make_float2(a.alpha * a.cscale[s0], (s1 < a.batch) ? a.alpha * a.cscale[s1] : 0.f);
@@ -310,7 +325,7 @@ gen_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
             const float2 c = __ldg(chn + off);
             return fma2(theta2, sub2(c, __ldg(chp + off)), c);
         };
-        for (int x = lane; x < nx; x += 32) {
+        for (int x = lane; x < nx; x += kGenLT) {
             const float2 c_old = __ldg(chn + x), mm = __ldg(M + x);
             float2 c_new;
             if (a.reg_l1) {
@@ -367,15 +382,15 @@ gen_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
             l0[x] = fma2(theta2, dc, c_new);
         }
         if (!last) {
-            __syncwarp();
-            gen_line_dft(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane);
-            for (int x = lane; x < nx; x += 32) __stcs(zr + x, l0[x]);
+            rowsync();
+            gen_line_dft<kGenLT>(W, nx, gd.n1x, gd.n2x, l0, l1, l0, lane, rowsync);
+            for (int x = lane; x < nx; x += kGenLT) __stcs(zr + x, l0[x]);
         }
     }
     float s6[6] = {gap.x, gap.y, dn.x, cn.x, dn.y, cn.y};
 #pragma unroll
     for (int k = 0; k < 6; ++k) s6[k] = warp_sum(s6[k]);
-    if (lane == 0) {
+    if ((lane & 31) == 0) {
 #pragma unroll
         for (int k = 0; k < 6; ++k) red[warp][k] = s6[k];
     }
@@ -383,7 +398,7 @@ gen_rows_kernel(const StreamFdArgs a, const GenDims gd, const int n_arg) {
     if (threadIdx.x < 6) {
         const int k = threadIdx.x;
         float t = 0.f;
-        for (int q = 0; q < kGenRows; ++q) t += red[q][k];
+        for (int q = 0; q < kGenRows * kGenWPR; ++q) t += red[q][k];
         const long long part = (long long)pair * a.nrowparts + blockIdx.x;
         if (k < 2) { if (want_gap) a.gap_row[part * 2 + k] = t; }
         else if ((k < 4) ? act0 : act1) a.res_part[part * 4 + (k - 2)] = t;

@@ -308,6 +308,23 @@ def test_hybrid_schedule_tail_through_streaming(torch, pd, oracle, tail):
     assert slice_rel(g["chi"], off["chi"]).max() < TOL_1IT
 
 
+def test_hybrid_schedule_with_l1_regulariser_and_oblique_b0(torch, pd, oracle):
+    """The two halves of the hybrid schedule run different kernels (resident MODE = l1 / streaming sfd_rows_l1) and read
+    two layouts of the same dipole table (thread-private order / [ny][nx]): both must follow PD_REG_L1 and pd_set_b0_angle."""
+    case = synth.random_case(256, 256, 7, seed=77, with_mask=True)
+    kw = dict(lambda_=0.4, sigma=0.25, tau=0.25, max_iters=5)
+    g = gpu_solve(torch, pd, case["field"], case["mask"], 5, lam=0.4, b0_angle=0.9,
+                  options=[(pd.OPT_HYBRID_TAIL, 2), (pd.OPT_REGULARISER, pd.REG_L1)])
+    assert g["hybrid_tail"] == 2
+    o = _oracle_batch(oracle, case, 5, regulariser=oracle.REG_L1, b0_angle=0.9, **{k: v for k, v in kw.items() if k != "max_iters"})
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], o["relgap"], rtol=1e-4)
+    g = gpu_solve(torch, pd, case["field"], case["mask"], 5, lam=0.4, b0_angle=0.9, options=[(pd.OPT_HYBRID_TAIL, 2)])
+    o = _oracle_batch(oracle, case, 5, b0_angle=0.9, **{k: v for k, v in kw.items() if k != "max_iters"})
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT
+    assert np.allclose(g["relgap"], o["relgap"], rtol=1e-4)
+
+
 def test_hybrid_schedule_tolerance_stop(torch, pd, oracle):
     """Per-slice stopping under the hybrid schedule: the resident clusters and the streaming tail each stop their own
     slices on the device; both parts agree with the hybrid-off run and with the oracle's stop iteration (R16)."""

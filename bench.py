@@ -47,8 +47,8 @@ KERNEL_BYTES_PER_PX = {
 NCU_DRAM_BYTES_PER_PX = {
     ("fd_rows", 512, False): 35.8,   # profiles/r02/ncu_sfd_rows_c4.md: 1.376 + 1.027 GB over 256 slices of 512x512 (36 algorithmic)
     ("fd_cols", 512, False): 20.4,   # profiles/r02/ncu_sfd_cols_c4.md: 0.872 + 0.495 GB (20 algorithmic)
-    ("fd_rows", 256, True): 39.3,    # profiles/r01/ncu_sfd_rows_c3.txt: 1.611 + 1.028 GB over 1024 slices of 256x256 (40 algorithmic)
-    ("fd_cols", 256, True): 19.7,    # profiles/r01/ncu_sfd_cols_c3.txt: 0.827 + 0.492 GB
+    ("fd_rows", 256, True): 40.9,    # profiles/r02/ncu_sfd_rows_c3.md: 1.717 + 1.029 GB over 1024 slices of 256x256 (40 algorithmic)
+    ("fd_cols", 256, True): 19.7,    # profiles/r02/ncu_sfd_cols_c3.md: 0.828 + 0.496 GB (20 algorithmic)
 }
 PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
 
@@ -285,6 +285,10 @@ def main():
     plan_info = plan.info()
     plan_info["weighted"] = bool(args.weighted)
     plan_info["mask"] = "none (all ones)" if mask_is_one else "per slice"
+    pow2 = {64, 128, 256, 512}
+    if not (cfg.nx in pow2 and cfg.ny in pow2):
+        plan_info["kernels"] = ("general-length row kernels (dense two-stage line DFT, shared-memory bound, literal iteration; DESIGN.md 5.4)"
+                                + (" + tuned column kernel" if cfg.ny in pow2 else ""))
     plan_info["hybrid_tail_pairs"] = plan.hybrid_tail()
     plan_info["hybrid_rho_measured_at_plan_time"] = plan.hybrid_rho()
     small = batch * P * 32 <= 2 * 126e6

@@ -182,6 +182,13 @@ int pd_get_hybrid_tail(pd_plan_t p, int *tail_pairs);
  * tail = npairs - w * clusters (0 if that is negative) is returned. */
 int pd_hybrid_tail_rule(int npairs, int clusters, float rho);
 
+/* How a line of length n is transformed (pure host arithmetic, no device needed; HOST pointers).  Returns 1 for a
+ * power-of-two length of the tuned kernels: *n1 = threads per line, *n2 = points per thread of the row kernels
+ * (64: 8 x 8, 128: 8 x 16, 256: 16 x 16, 512: 32 x 16 in three stages).  Returns 0 for a general length (even, 4..1024):
+ * n = *n1 * *n2 with *n1 <= *n2 the most balanced factorisation, the two dense stages of pd_streaming_gen.cuh
+ * (258 = 6 x 43, 132 = 11 x 12; a prime gives 1 x n).  Errors: PD_ESIZE (unsupported length), PD_EINVAL. */
+int pd_line_factors(int n, int *n1, int *n2);
+
 /* rho of this plan: measured by pd_plan on the plan's device (one wave of resident clusters and a few slice pairs
  * through the streaming kernels, run concurrently on a synthetic field; a few ms), or the built-in 0.15 when the batch
  * is too small for a tail or the size has no hybrid schedule.  HOST pointer. */

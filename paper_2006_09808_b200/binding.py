@@ -24,7 +24,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_line_factors", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror"]
 
 _lib = None
 
@@ -59,6 +59,7 @@ def lib():
         L.pd_get_info.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
         L.pd_get_hybrid_tail.argtypes = [vp, C.POINTER(ip)]
         L.pd_hybrid_tail_rule.argtypes = [ip, ip, fp]
+        L.pd_line_factors.argtypes = [ip, C.POINTER(ip), C.POINTER(ip)]
         L.pd_get_hybrid_rho.argtypes = [vp, C.POINTER(fp)]
         L.pd_destroy.argtypes = [vp]
         L.pd_strerror.argtypes = [ip]
@@ -103,6 +104,15 @@ def hybrid_tail_rule(npairs, clusters, rho):
     """pd_hybrid_tail_rule: the automatic tail of the hybrid schedule for `npairs` slice pairs, `clusters` clusters and
     a streaming side that finishes rho * clusters pairs per resident wave."""
     return lib().pd_hybrid_tail_rule(int(npairs), int(clusters), float(rho))
+
+
+def line_factors(n):
+    """pd_line_factors: (tuned, n1, n2) -- how a line of length n is transformed (host arithmetic only)."""
+    a, b = C.c_int(), C.c_int()
+    rc = lib().pd_line_factors(int(n), C.byref(a), C.byref(b))
+    if rc < 0:
+        raise PdError(rc, strerror(rc))
+    return bool(rc), a.value, b.value
 
 
 class Plan:

@@ -1213,6 +1213,20 @@ int pd_get_info(pd_plan_t p, int *variant, int *clusters, int *cluster_size) {
     return PD_OK;
 }
 
+int pd_line_factors(int n, int *n1, int *n2) {
+    if (!n1 || !n2) return PD_EINVAL;
+    switch (n) {   // the tuned kernels: threads per line x points per thread of the row configuration (fft_regs.cuh)
+        case 64: *n1 = pdk::FftCfg<64>::T; *n2 = pdk::FftCfg<64>::E; return 1;
+        case 128: *n1 = pdk::FftCfg<128>::T; *n2 = pdk::FftCfg<128>::E; return 1;
+        case 256: *n1 = pdk::FftCfg<256>::T; *n2 = pdk::FftCfg<256>::E; return 1;
+        case 512: *n1 = pdk::FftCfg<512>::T; *n2 = pdk::FftCfg<512>::E; return 1;
+        default: break;
+    }
+    if (!gen_size_ok(n)) return PD_ESIZE;
+    balanced_factors(n, n1, n2);
+    return 0;
+}
+
 int pd_hybrid_tail_rule(int npairs, int clusters, float rho) { return hybrid_tail_rule(npairs, clusters, (double)rho); }
 
 int pd_get_hybrid_rho(pd_plan_t p, float *rho) {

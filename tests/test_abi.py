@@ -67,6 +67,25 @@ def test_product_does_not_import_the_oracle():
             assert "csrc/" not in text.replace("paper_2006_09808_b200/csrc/", "")  # only mentioned in a comment
 
 
+def test_line_factors_host_logic(libpath):
+    """pd_line_factors (pure host arithmetic): the tuned power-of-two lines, and the balanced two-factor split of the
+    general-length kernels (the paper's 258 = 6 x 43 and 132 = 11 x 12)."""
+    from paper_2006_09808_b200 import binding
+    assert binding.line_factors(64) == (True, 8, 8) and binding.line_factors(256) == (True, 16, 16)
+    assert binding.line_factors(512) == (True, 32, 16)          # a whole warp per row, three stages
+    assert binding.line_factors(258) == (False, 6, 43) and binding.line_factors(132) == (False, 11, 12)
+    for n in range(4, 1025, 2):
+        tuned, n1, n2 = binding.line_factors(n)
+        assert n1 * n2 == n and (tuned or n1 <= n2)
+        if not tuned:   # no factor pair is more balanced
+            assert all(n % f or f <= n1 for f in range(1, int(n ** 0.5) + 1))
+    assert binding.line_factors(254) == (False, 2, 127)        # 2 x prime: one long dense stage
+    for bad in (257, 2, 1026, 0, -4):
+        with pytest.raises(binding.PdError) as e:
+            binding.line_factors(bad)
+        assert e.value.code == binding.ESIZE
+
+
 def test_hybrid_tail_rule_host_logic(libpath):
     """pd_hybrid_tail_rule (pure host arithmetic behind PD_OPT_HYBRID_TAIL = -1): the resident clusters
     run whole waves, the tail is what is left, and it never asks the streaming side for more than it can do in that time."""

@@ -70,10 +70,15 @@ template <int N> struct SfdRowCfg {
 #define PD_SFD_STAGE_MIN 256
 #endif
     static constexpr bool STAGE = N >= PD_SFD_STAGE_MIN;   // park the spectrum in shared memory during the update loop
+    // CTAs per SM the row kernel is compiled for (register cap 65536 / (128 MINB)).  4 (128 registers) measured 1.5-3 %
+    // faster than 5 (96 registers) on both sizes, 6 and 7 slower (profiles/r02/README.md)
 #ifndef PD_SFD_ROWS512_MINB
-#define PD_SFD_ROWS512_MINB 5
+#define PD_SFD_ROWS512_MINB 4
 #endif
-    static constexpr int MINB = N == 512 ? PD_SFD_ROWS512_MINB : (STAGE ? 5 : 4);
+#ifndef PD_SFD_ROWS256_MINB
+#define PD_SFD_ROWS256_MINB 4
+#endif
+    static constexpr int MINB = N == 512 ? PD_SFD_ROWS512_MINB : (STAGE ? PD_SFD_ROWS256_MINB : 4);
 #ifndef PD_SFD_UNROLL
 #define PD_SFD_UNROLL 4
 #endif

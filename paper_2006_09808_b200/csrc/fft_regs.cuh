@@ -62,11 +62,23 @@ __device__ __forceinline__ float2 twiddle_mul(float2 d, int k) {
     constexpr float C8 = 0.70710678118654752440f;
     if (k == 0) return d;
     if (4 * k == R) return make_float2(d.y, -d.x);
+#ifdef PDK_PACKED_F32X2
+    // Blackwell's packed FFMA2 takes its operands with the halves swapped and with a sign per half (SASS: R.F32x2.LO_HI.NP)
+    // and a scalar broadcast (R.F32), so a complex multiplication is TWO instructions, FMUL2 + FFMA2, instead of four
+    // scalar ones: (d.x c + d.y s, d.y c - d.x s) = d (c, c) + (d.y, d.x) (s, -s)
+    const float2 dsw = make_float2(d.y, d.x);
+    if (8 * k == R) return __fmul2_rn(__ffma2_rn(dsw, make_float2(1.f, -1.f), d), make_float2(C8, C8));          // C8 (d.x + d.y, d.y - d.x)
+    if (8 * k == 3 * R) return __fmul2_rn(__ffma2_rn(dsw, make_float2(1.f, -1.f), make_float2(-d.x, -d.y)), make_float2(C8, C8));   // C8 (d.y - d.x, -d.x - d.y)
+    const int i = k * (32 / R);  // angle index on the 32-point circle, in (0,16)
+    const float c = cos32(i), s = sin32(i);
+    return __ffma2_rn(dsw, make_float2(s, -s), __fmul2_rn(d, make_float2(c, c)));
+#else
     if (8 * k == R) return make_float2(C8 * (d.x + d.y), C8 * (d.y - d.x));
     if (8 * k == 3 * R) return make_float2(C8 * (d.y - d.x), -C8 * (d.x + d.y));
     const int i = k * (32 / R);  // angle index on the 32-point circle, in (0,16)
     const float c = cos32(i), s = sin32(i);
     return make_float2(fmaf(d.y, s, d.x * c), fmaf(-d.x, s, d.y * c));
+#endif
 }
 
 // Radix-2 decimation-in-frequency on v[OFF..OFF+R): leaves X[k] at bit-reversed position.
@@ -126,7 +138,12 @@ __device__ __forceinline__ float group_sum(float v) {
 }
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
+#ifdef PDK_PACKED_F32X2
+    // (a.x w.x - a.y w.y, a.x w.y + a.y w.x) = a (w.x, w.x) + (a.y, a.x) (-w.y, w.y): FMUL2 + FFMA2 (see twiddle_mul)
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(-w.y, w.y), __fmul2_rn(a, make_float2(w.x, w.x)));
+#else
     return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.x, w.y, a.y * w.x));
+#endif
 }
 
 struct WarpSync {   // the T threads of a line sit in one warp

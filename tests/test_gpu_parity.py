@@ -568,6 +568,64 @@ def test_repeatable_and_plan_reuse(torch, pd):
     plan.destroy()
 
 
+@pytest.mark.parametrize("seed", range(24))
+def test_seeded_random_option_combinations(torch, pd, oracle, seed):
+    """A seeded differential sweep over combinations no other test pairs up: size (tuned, non-square, general length),
+    variant, regulariser, projection mode, lambda convention, theta, B0 (axis or oblique), weight, shared mask, batch parity,
+    iteration count, explicit or automatic steps -- each combination against the oracle with the same settings."""
+    r = np.random.default_rng(1000 + seed)
+    ny, nx = [(64, 64), (128, 128), (64, 128), (128, 64), (256, 256), (36, 66), (20, 12), (132, 128), (64, 66), (512, 64)][int(r.integers(10))]
+    batch = int(r.integers(1, 6))
+    iters = int(r.integers(1, 9))
+    variant = ["auto", "streaming"][int(r.integers(2))]
+    l1 = bool(r.integers(2))
+    aniso = bool(r.integers(2)) and not l1
+    conv_a = bool(r.integers(4) == 0)
+    theta = [1.0, 1.0, 0.5, 0.0][int(r.integers(4))]
+    angle = [None, None, float(r.uniform(-3, 3))][int(r.integers(3))]
+    b0 = int(r.integers(2))
+    weighted = bool(r.integers(3) == 0)
+    shared = bool(r.integers(4) == 0)
+    auto_steps = bool(r.integers(4) == 0)
+    fd = bool(r.integers(4) != 0)
+    lam = float([0.05, 0.3, 1.0][int(r.integers(3))])
+    if conv_a:
+        lam = 1.0 / lam
+    sig = tau = 0.25
+    case = synth.random_case(nx, ny, batch, seed=500 + seed, with_mask=True, with_weight=weighted)
+    mask = case["mask"]
+    if shared:
+        mask = np.repeat(mask[:1], batch, axis=0)
+    opts = []
+    if l1:
+        opts.append((pd.OPT_REGULARISER, pd.REG_L1))
+    if aniso:
+        opts.append((pd.OPT_TV_MODE, pd.TV_ANISO))
+    if conv_a:
+        opts.append((pd.OPT_LAMBDA_CONV, pd.LAMBDA_DATA))
+    if shared:
+        opts.append((pd.OPT_MASK_SHARED, 1))
+    if not fd:
+        opts.append((pd.OPT_FOURIER_DUAL, 0))
+    gs = 0.0 if auto_steps else sig
+    g = gpu_solve(torch, pd, case["field"], mask[0] if shared else mask, iters, lam=lam, sigma=gs, tau=gs, theta=theta,
+                  weight=case["weight"] if weighted else None, b0=b0, options=opts, variant=variant, b0_angle=angle)
+    if auto_steps:
+        sig = tau = 1.0 / np.sqrt(4.0 / 9.0 + 8.0)
+    kw = dict(lambda_=lam, sigma=sig, tau=tau, theta=theta, tv_mode=oracle.TV_ANISO if aniso else oracle.TV_ISO,
+              lambda_conv=oracle.LAMBDA_DATA if conv_a else oracle.LAMBDA_REG, regulariser=oracle.REG_L1 if l1 else oracle.REG_TV)
+    if angle is not None:
+        kw["b0_angle"] = angle
+    else:
+        kw["b0_dir"] = b0
+    o = _oracle_batch(oracle, dict(field=case["field"], mask=mask, weight=case["weight"] if weighted else None), iters, **kw)
+    what = dict(size=(ny, nx), batch=batch, iters=iters, variant=variant, l1=l1, aniso=aniso, conv_a=conv_a, theta=theta, angle=angle,
+                b0=b0, weighted=weighted, shared=shared, auto_steps=auto_steps, fd=fd, lam=lam)
+    assert slice_rel(g["chi"], o["chi"]).max() < TOL_1IT, what
+    assert np.allclose(g["relgap"], o["relgap"], rtol=1e-3), what
+    assert np.all(g["iters_done"] == iters), what
+
+
 def test_norm_bounds_for_automatic_steps(torch, pd, oracle, variant):
     """pd_set_norm_bounds (R14): mask values up to 2 and weights up to 1.5 with the automatic steps
     sigma = tau = 1/sqrt(4/9 max|W|^2 + 8 max|M|^2); PD_ESTEP follows the same bound."""

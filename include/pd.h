@@ -12,6 +12,10 @@
  * or, per slice, until the relative primal-dual gap falls below tol (BASELINE.json north_star (d)).
  * D(kx,ky) = 1/3 - k_b^2/(kx^2+ky^2), D(0,0) = 0 (BASELINE.json north_star).  G: forward
  * differences with Neumann boundary; M: mask on the gradient; W: optional data weighting.
+ * Variants: lambda ||M chi||_1 with a shrinkage prox (PD_OPT_REGULARISER), anisotropic projection, the paper's
+ * placement of lambda (PD_OPT_LAMBDA_CONV), an oblique in-plane B0 (pd_set_b0_angle).
+ * Sizes: nx, ny in {64,128,256,512} run the tuned kernels (square <= 256: the resident cluster kernel); any other even
+ * nx, ny in [4,1024] -- the paper's 256x258 and 128x132 -- run the general-length streaming kernels.
  *
  * Layout of every image argument: fp32, [batch][ny][nx], x fastest, contiguous, 16-byte aligned.
  * Multi-coil stacks: batch = nslices*ncoils, index slice*ncoils + coil (BASELINE.json configs[3]);
@@ -35,8 +39,9 @@ enum pd_b0 { PD_B0_X = 0, PD_B0_Y = 1 }; /* in-plane B0 axis: k_b = kx (fast axi
 enum pd_error {
     PD_OK = 0,
     PD_EINVAL = -1,   /* null plan/field/chi_out, batch < 1, max_iters < 0, theta outside [0,1], lambda < 0, bad option */
-    PD_ESIZE = -2,    /* nx or ny not in {64,128,256,512} */
-    PD_ESTEP = -3,    /* explicit steps with sigma*tau*(4/9+8) >= 1: convergence bound of [7] violated */
+    PD_ESIZE = -2,    /* nx, ny neither both in {64,128,256,512} (tuned kernels) nor both even and in [4,1024] (general-length kernels) */
+    PD_ESTEP = -3,    /* explicit steps with sigma*tau*(4/9 max|W|^2 + 8 max|M|^2) >= 1 (both maxima 1 unless pd_set_norm_bounds):
+                         convergence bound of [7] violated */
     PD_ENOMEM = -4,   /* device allocation failed */
     PD_ECUDA = -5,    /* a CUDA call or launch failed; pd_strerror(PD_ECUDA) returns the last CUDA error text */
     PD_EVARIANT = -6  /* PD_VARIANT_RESIDENT requested for a size that does not fit on chip */

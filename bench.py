@@ -45,10 +45,10 @@ KERNEL_BYTES_PER_PX = {
 # DRAM bytes per pixel of a slice per launch measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one
 # `--set full` capture over the whole batch): (kernel, line length, masked) -> B/px
 NCU_DRAM_BYTES_PER_PX = {
-    ("fd_rows", 512, False): 35.8,   # profiles/r02/ncu_sfd_rows_c4.md: 1.376 + 1.027 GB over 256 slices of 512x512 (36 algorithmic)
-    ("fd_cols", 512, False): 20.4,   # profiles/r02/ncu_sfd_cols_c4.md: 0.872 + 0.495 GB (20 algorithmic)
-    ("fd_rows", 256, True): 40.9,    # profiles/r02/ncu_sfd_rows_c3.md: 1.717 + 1.029 GB over 1024 slices of 256x256 (40 algorithmic)
-    ("fd_cols", 256, True): 19.7,    # profiles/r02/ncu_sfd_cols_c3.md: 0.828 + 0.496 GB (20 algorithmic)
+    ("fd_rows", 512, False): 35.3,   # profiles/r02/ncu_sfd_rows_c4.md: 1.347 + 1.025 GB over 256 slices of 512x512 (36 algorithmic)
+    ("fd_cols", 512, False): 20.4,   # profiles/r02/ncu_sfd_cols_c4.md: 0.874 + 0.496 GB (20 algorithmic)
+    ("fd_rows", 256, True): 39.7,    # profiles/r02/ncu_sfd_rows_c3.md: 1.636 + 1.029 GB over 1024 slices of 256x256 (40 algorithmic)
+    ("fd_cols", 256, True): 19.7,    # profiles/r02/ncu_sfd_cols_c3.md: 0.825 + 0.496 GB (20 algorithmic)
 }
 PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
 
@@ -56,10 +56,10 @@ PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iter
 # C2 and one metrics-only pass over every launch of a hybrid C3 step); quoted beside the live numbers, never timed here.
 NCU_RESIDENT = {
     "source": "profiles/r02/ncu_resident_tm_c2.md (kernel alone on C2, hybrid tail off), profiles/r02/dram_bytes_C3_hybrid_step.md",
-    "issue_slots_busy_pct": 42.4, "fma_pipe_pct": 39.1, "l1tex_pct": 54.5, "l2_pct": 11.4, "dram_pct": 0.06,
-    "shared_wavefronts_pct_of_peak": 55.2,          # 593.9 M wavefronts / (120 SMs x 8.97 M active cycles), 1 wavefront/clk/SM
-    "l2_bytes_per_pixel_pair_iteration": 51.7,      # lts__t_sectors 677.5 M x 32 B / (32 pairs x 200 iterations x 65536)
-    "warps_per_scheduler": 4.0, "cycles_per_issue": 9.45,
+    "issue_slots_busy_pct": 38.7, "fma_pipe_pct": 39.3, "l1tex_pct": 54.8, "l2_pct": 11.4, "dram_pct": 0.06,
+    "shared_wavefronts_pct_of_peak": 55.5,          # 596.1 M wavefronts / (120 SMs x 8.96 M active cycles), 1 wavefront/clk/SM
+    "l2_bytes_per_pixel_pair_iteration": 51.7,      # lts__t_sectors 677.3 M x 32 B / (32 pairs x 200 iterations x 65536)
+    "warps_per_scheduler": 4.0, "cycles_per_issue": 10.33,
 }
 # dram__bytes_read.sum + dram__bytes_write.sum summed over every launch of one step (resident kernel + streaming tail)
 NCU_DRAM_BYTES_PER_STEP = {("C3", 47): 81401493248.0}   # (workload, hybrid_tail_pairs) -> bytes (profiles/r02/dram_bytes_C3_hybrid_step.md)

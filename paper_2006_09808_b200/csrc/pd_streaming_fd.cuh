@@ -42,8 +42,8 @@ struct StreamFdArgs {
     float2 *W2;                              // literal path only: interleaved W; phihat then holds phi itself
     int literal;                             // 1: W != I or PD_OPT_FOURIER_DUAL = 0 (p kept in the image domain)
     int reg_l1;                              // 1: PD_REG_L1 (l1 on chi, shrinkage) instead of the paper's TV term
-    int cols_contig;                         // PLAIN column kernel only: CTA cb owns the columns [16 cb, 16 cb + 16) below nx (nx need
-                                             // not be a multiple of 16: the general-length path with a power-of-two ny) instead of mirror pairs
+    int cols_contig;                         // general-length plan with a power-of-two ny: the PLAIN column kernel runs over
+                                             // ceil(nx / 16) column blocks, the last one ragged
     float2 *phat[2], *qx2[2], *qy2[2];       // double-buffered by iteration parity: iteration n reads [n&1]
     float2 *chi3[3];                         // chi_n in [n%3], chi_{n-1} in [(n+2)%3], chi_{n+1} written to [(n+1)%3]
     const float *Dtab;                       // D/(nx*ny), [ny][nx]
@@ -325,8 +325,13 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
     const int h = c >> 3, cc = c & 7;
     const int nx = NXC ? NXC : a.nx;
-    // PLAIN with cols_contig: a ragged last block; its surplus threads redo column nx - 1 (they must reach the barriers) and do not store
-    const int kx_raw = (PLAIN && a.cols_contig) ? 16 * (int)blockIdx.x + c : sfd_column_of(nx, blockIdx.x, h, cc);
+    // Mirror-paired columns are needed only where the Parseval sums are taken (want_gap).  Everywhere else CTA cb owns the
+    // CONTIGUOUS columns [16 cb, 16 cb + 16): a warp's access then touches two 128-byte lines (two rows) instead of four
+    // (two rows x an adjacent and a mirrored 64-byte segment) -- the load/store path is what limits this kernel
+    // (profiles/r02/ncu_sfd_cols_c4.md: MIO throttle first, L1TEX 70 %).  With a.cols_contig (general-length plans, nx not a
+    // multiple of 16) the last block is ragged: its surplus threads redo column nx - 1 (they must reach the barriers) and do not store.
+    const bool contig = PLAIN || !want_gap;
+    const int kx_raw = contig ? 16 * (int)blockIdx.x + c : sfd_column_of(nx, blockIdx.x, h, cc);
     const bool kx_valid = kx_raw < nx;
     const int kx = kx_valid ? kx_raw : nx - 1;
     const bool self_mirror = (blockIdx.x == 0 && cc == 0);

@@ -316,12 +316,17 @@ void build_dipole_private(std::vector<float> &out, const std::vector<float> &D) 
 // resident plans stay small
 constexpr int kSfdPlanes = 13;   // Z, phi^ (or phi), M, W; p^ (or p), qx, qy twice each; chi three times
 
+// columns one CTA of the column kernels owns (SfdColCfg<ny>::COLS)
+int sfd_cols_per_cta(int ny) {
+    return ny == 64 ? pdk::SfdColCfg<64>::COLS : ny == 128 ? pdk::SfdColCfg<128>::COLS : ny == 256 ? pdk::SfdColCfg<256>::COLS : pdk::SfdColCfg<512>::COLS;
+}
+
 int ensure_sfd_workspace(pd_plan_s *p, size_t npairs) {
     if (p->sfd_planes && p->sfd_pairs_alloc >= npairs) return PD_OK;
     if (p->sfd_planes) { cudaFree(p->sfd_planes); p->sfd_planes = nullptr; }
     if (p->sfd_parts) { cudaFree(p->sfd_parts); p->sfd_parts = nullptr; }
     const size_t PP = (size_t)p->nx * p->ny * npairs;
-    p->sfd_ncolparts = p->generic ? p->nparts : p->nx / 16;
+    p->sfd_ncolparts = p->generic ? p->nparts : p->nx / sfd_cols_per_cta(p->ny);
     p->sfd_nrowparts = p->nparts;
     int rc;
     if ((rc = dev_alloc(&p->sfd_planes, PP * kSfdPlanes)) != PD_OK) return rc;
@@ -359,18 +364,19 @@ template <int NX> void sfd_launch_rows(const StreamFdArgs &a, int n, cudaStream_
     else pdk::sfd_rows_kernel<NX, false, false><<<grid, pdk::SfdRowCfg<NX>::THREADS, 0, st>>>(a, n);
 }
 template <int NY> void sfd_launch_init_cols(const StreamFdArgs &a, cudaStream_t st) {
-    dim3 grid(a.nx / 16, a.npairs);
+    dim3 grid(a.nx / pdk::SfdColCfg<NY>::COLS, a.npairs);
     pdk::sfd_init_cols_kernel<NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a);
 }
 template <int NY> void sfd_launch_cols(const StreamFdArgs &a, int n, cudaStream_t st) {
-    dim3 grid(a.nx / 16, a.npairs);
+    dim3 grid(a.nx / pdk::SfdColCfg<NY>::COLS, a.npairs);
     if (a.nx == NY) pdk::sfd_cols_kernel<NY, false, NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, 1);
     else pdk::sfd_cols_kernel<NY, false, 0><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, 1);
 }
 template <int NY> void sfd_launch_cols_plain(const StreamFdArgs &a, int n, int decide, cudaStream_t st) {
-    dim3 grid((a.nx + 15) / 16, a.npairs);
-    if (a.nx == NY) pdk::sfd_cols_kernel<NY, true, NY><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
-    else pdk::sfd_cols_kernel<NY, true, 0><<<grid, pdk::SfdColCfg<NY>::THREADS, pdk::SfdColCfg<NY>::SMEM_BYTES, st>>>(a, n, decide);
+    using PC = pdk::SfdColCfg<NY, true>;
+    dim3 grid((a.nx + PC::COLS - 1) / PC::COLS, a.npairs);
+    if (a.nx == NY) pdk::sfd_cols_kernel<NY, true, NY><<<grid, PC::THREADS, PC::SMEM_BYTES, st>>>(a, n, decide);
+    else pdk::sfd_cols_kernel<NY, true, 0><<<grid, PC::THREADS, PC::SMEM_BYTES, st>>>(a, n, decide);
 }
 template <int NX> void sfd_launch_dual_rows(const StreamFdArgs &a, int n, cudaStream_t st) {
     dim3 grid(a.ny / pdk::SfdRowCfg<NX>::G, a.npairs);
@@ -379,9 +385,9 @@ template <int NX> void sfd_launch_dual_rows(const StreamFdArgs &a, int n, cudaSt
 template <int NY>
 cudaError_t sfd_set_col_smem() {
     cudaError_t e = cudaSuccess;
-    auto set = [&](auto kern) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, pdk::SfdColCfg<NY>::SMEM_BYTES); };
-    set(pdk::sfd_cols_kernel<NY, false, NY>); set(pdk::sfd_cols_kernel<NY, false, 0>);
-    set(pdk::sfd_cols_kernel<NY, true, NY>); set(pdk::sfd_cols_kernel<NY, true, 0>);
+    auto set = [&](auto kern, int bytes) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); };
+    set(pdk::sfd_cols_kernel<NY, false, NY>, pdk::SfdColCfg<NY>::SMEM_BYTES); set(pdk::sfd_cols_kernel<NY, false, 0>, pdk::SfdColCfg<NY>::SMEM_BYTES);
+    set(pdk::sfd_cols_kernel<NY, true, NY>, pdk::SfdColCfg<NY, true>::SMEM_BYTES); set(pdk::sfd_cols_kernel<NY, true, 0>, pdk::SfdColCfg<NY, true>::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(pdk::sfd_init_cols_kernel<NY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 pdk::SfdColCfg<NY>::SMEM_BYTES);

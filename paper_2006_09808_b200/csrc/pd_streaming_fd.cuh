@@ -84,10 +84,17 @@ template <int N> struct SfdRowCfg {
 #endif
     static constexpr int UNROLL = PD_SFD_UNROLL;           // elements of the update loop per unrolled body (STAGE only)
 };
-template <int N> struct SfdColCfg {
+template <int N, bool PLAIN = false> struct SfdColCfg {
     using Fft = FftCfg<N, true>;                       // column configuration of the line transform (fft_regs.cuh)
     static constexpr int E = Fft::E, T = Fft::T;
-    static constexpr int HALF = 8, COLS = 16;          // 8 adjacent columns and their 8 mirror images
+#ifndef PD_SFD_COLS512_HALF
+#define PD_SFD_COLS512_HALF 16
+#endif
+    // HALF adjacent columns and their HALF mirror images per CTA: 64-byte segments at HALF = 8, whole 128-byte lines at 16.
+    // 16 + 16 columns of 512 points are 512 threads and 131 KB, one CTA per SM: measured 7 % faster for the Fourier-domain
+    // kernel at 512 (every C4 iteration takes the Parseval sums, i.e. the mirror-paired mapping: 33.1 -> 30.9 ms per step)
+    // and 8 % slower for the PLAIN kernel, which always runs over contiguous blocks and keeps 16 columns, two CTAs per SM.
+    static constexpr int HALF = (N == 512 && !PLAIN) ? PD_SFD_COLS512_HALF : 8, COLS = 2 * HALF;
     static constexpr int THREADS = COLS * T;
     static constexpr int CS = N + 1 > Fft::REGION ? N + 1 : Fft::REGION + 1;   // odd column stride
     static constexpr int SMEM_BYTES = (COLS * CS + Fft::TW) * (int)sizeof(float2) + 256;
@@ -99,8 +106,8 @@ template <int N> struct SfdColCfg {
 
 // column kx of (column block cb, half h, slot cc): [8cb, 8cb+8) and its mirror images nx - kx; the self-mirrored
 // columns 0 and nx/2 both sit in block 0, slot 0.
-__host__ __device__ constexpr int sfd_column_of(int nx, int cb, int h, int cc) {
-    const int lo = 8 * cb + cc;
+__host__ __device__ constexpr int sfd_column_of(int nx, int cb, int h, int cc, int half = 8) {
+    const int lo = half * cb + cc;
     return h == 0 ? lo : (lo == 0 ? nx / 2 : nx - lo);
 }
 
@@ -233,7 +240,7 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
     __syncthreads();
     const int pair = blockIdx.y, s0 = 2 * pair, s1 = s0 + 1;
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
-    const int kx = sfd_column_of(a.nx, blockIdx.x, c >> 3, c & 7);
+    const int kx = sfd_column_of(a.nx, blockIdx.x, c / Cfg::HALF, c % Cfg::HALF, Cfg::HALF);
     const long long po = (long long)pair * a.nx * NY + kx;
     TwiddlesSmem<NY, true> tw;
     tw.w = tws + j;
@@ -280,11 +287,11 @@ sfd_init_cols_kernel(const StreamFdArgs a) {
 // constant row pitch every access of a thread is base + immediate; with a run-time pitch the 64-bit address arithmetic
 // of the five strided arrays was 28 % of the instructions of the 512-point kernel (profiles/r02/README.md).
 template <int NY, bool PLAIN, int NXC>
-__global__ void __launch_bounds__(SfdColCfg<NY>::THREADS, SfdColCfg<NY>::THREADS <= 128 ? 4 : 2)
+__global__ void __launch_bounds__(SfdColCfg<NY, PLAIN>::THREADS, SfdColCfg<NY, PLAIN>::THREADS <= 128 ? 4 : (SfdColCfg<NY, PLAIN>::THREADS <= 256 ? 2 : 1))
 sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     const int n = n_arg >= 0 ? n_arg : *a.iter;      // inside the graphed loop the iteration number lives on the device
     if (PLAIN && do_decide && n == 0) return;        // literal path: chibar_0 = 0, the first K application of iteration 0 is skipped
-    using Cfg = SfdColCfg<NY>;
+    using Cfg = SfdColCfg<NY, PLAIN>;
     constexpr int E = Cfg::E, T = Cfg::T, NT = Cfg::THREADS;
     extern __shared__ __align__(16) unsigned char sfd_smem[];
     float2 *smc = reinterpret_cast<float2 *>(sfd_smem);
@@ -323,7 +330,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
 
     TwiddlesSmem<NY, true>::fill(tws, a.tw_col, threadIdx.x, NT);
     const int c = threadIdx.x & (Cfg::COLS - 1), j = threadIdx.x / Cfg::COLS;
-    const int h = c >> 3, cc = c & 7;
+    const int h = c / Cfg::HALF, cc = c % Cfg::HALF;
     const int nx = NXC ? NXC : a.nx;
     // Mirror-paired columns are needed only where the Parseval sums are taken (want_gap).  Everywhere else CTA cb owns the
     // CONTIGUOUS columns [16 cb, 16 cb + 16): a warp's access then touches two 128-byte lines (two rows) instead of four
@@ -331,12 +338,12 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     // (profiles/r02/ncu_sfd_cols_c4.md: MIO throttle first, L1TEX 70 %).  With a.cols_contig (general-length plans, nx not a
     // multiple of 16) the last block is ragged: its surplus threads redo column nx - 1 (they must reach the barriers) and do not store.
     const bool contig = PLAIN || !want_gap;
-    const int kx_raw = contig ? 16 * (int)blockIdx.x + c : sfd_column_of(nx, blockIdx.x, h, cc);
+    const int kx_raw = contig ? Cfg::COLS * (int)blockIdx.x + c : sfd_column_of(nx, blockIdx.x, h, cc, Cfg::HALF);
     const bool kx_valid = kx_raw < nx;
     const int kx = kx_valid ? kx_raw : nx - 1;
     const bool self_mirror = (blockIdx.x == 0 && cc == 0);
     float2 *smg = smc + c * Cfg::CS;
-    const float2 *smg_mir = self_mirror ? smg : smc + (c ^ 8) * Cfg::CS;
+    const float2 *smg_mir = self_mirror ? smg : smc + (c ^ Cfg::HALF) * Cfg::CS;
     const long long po = (long long)pair * nx * NY + kx;
     float2 *zc = a.Z + po, *phw = a.phat[(n & 1) ^ 1] + po;
     const float2 *phh = a.phihat + po, *phr = a.phat[n & 1] + po;
@@ -349,7 +356,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
     if (n > 0 || PLAIN) {
 #pragma unroll
         for (int m = 0; m < E; ++m) v[m] = __ldcs(zc + (long long)(j + T * m) * nx);
-        if (!PLAIN && (c & 7) == 1) {   // the 64-byte segments of phi^ and p^_n this half-block of 8 columns will read
+        if (!PLAIN && cc == 1) {   // the 64-byte segments of phi^ and p^_n this half-block of 8 columns will read
 #pragma unroll
             for (int m = 0; m < E; ++m) { prefetch_l2(phh + (long long)(j + T * m) * nx); prefetch_l2(phr + (long long)(j + T * m) * nx); }
         }
@@ -387,7 +394,7 @@ sfd_cols_kernel(const StreamFdArgs a, const int n_arg, const int do_decide) {
         }
         if (want_gap) {   // dp(k) dp(-k): p^_{n+1} of the mirror element from its slot, p^_n of both reloaded (L1/L2)
             __syncthreads();
-            const float2 *phr_mir = a.phat[n & 1] + (long long)pair * nx * NY + (self_mirror ? kx : sfd_column_of(nx, blockIdx.x, h ^ 1, cc));
+            const float2 *phr_mir = a.phat[n & 1] + (long long)pair * nx * NY + (self_mirror ? kx : sfd_column_of(nx, blockIdx.x, h ^ 1, cc, Cfg::HALF));
 #pragma unroll
             for (int m = 0; m < E; ++m) {
                 const int ky = j + T * m, kym = (NY - ky) & (NY - 1);

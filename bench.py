@@ -46,9 +46,9 @@ KERNEL_BYTES_PER_PX = {
 # `--set full` capture over the whole batch): (kernel, line length, masked) -> B/px
 NCU_DRAM_BYTES_PER_PX = {
     ("fd_rows", 512, False): 35.3,   # profiles/r02/ncu_sfd_rows_c4.md: 1.347 + 1.025 GB over 256 slices of 512x512 (36 algorithmic)
-    ("fd_cols", 512, False): 20.4,   # profiles/r02/ncu_sfd_cols_c4.md: 0.874 + 0.496 GB (20 algorithmic)
+    ("fd_cols", 512, False): 19.4,   # profiles/r02/ncu_sfd_cols_c4.md: 0.812 + 0.487 GB (20 algorithmic)
     ("fd_rows", 256, True): 39.7,    # profiles/r02/ncu_sfd_rows_c3.md: 1.636 + 1.029 GB over 1024 slices of 256x256 (40 algorithmic)
-    ("fd_cols", 256, True): 19.7,    # profiles/r02/ncu_sfd_cols_c3.md: 0.825 + 0.496 GB (20 algorithmic)
+    ("fd_cols", 256, True): 19.3,    # profiles/r02/ncu_sfd_cols_c3.md: 0.806 + 0.490 GB (20 algorithmic)
 }
 PATH_FLOOR_BYTES_PER_PX = 48.0  # streaming floor per slice-iteration (12 words)
 

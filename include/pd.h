@@ -44,7 +44,8 @@ enum pd_error {
                          convergence bound of [7] violated */
     PD_ENOMEM = -4,   /* device allocation failed */
     PD_ECUDA = -5,    /* a CUDA call or launch failed; pd_strerror(PD_ECUDA) returns the last CUDA error text */
-    PD_EVARIANT = -6  /* PD_VARIANT_RESIDENT requested for a size that does not fit on chip */
+    PD_EVARIANT = -6, /* PD_VARIANT_RESIDENT requested for a size that does not fit on chip */
+    PD_ESTATIC = -7   /* pd_solve_static: the problem does not fit the static workspace (limits below) */
 };
 
 enum pd_option {
@@ -200,6 +201,37 @@ int pd_line_factors(int n, int *n1, int *n2);
 int pd_get_hybrid_rho(pd_plan_t p, float *rho);
 
 int pd_destroy(pd_plan_t p);
+
+/* pd_solve_static: ONE allocation-free entry point, for callers that cannot call cudaMalloc (code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid it).  It runs the same iteration as pd_solve
+ * through the streaming kernels with the Fourier-domain dual (W = identity, isotropic TV, lambda on the regulariser,
+ * one mask per slice, tolerance checked every iteration) -- bit for bit what a fresh plan with
+ * PD_OPT_VARIANT = PD_VARIANT_STREAMING and PD_OPT_GRAPH_LOOP = 0 computes -- but needs no plan: the whole workspace
+ * (13 state planes, per-CTA partial sums, the dipole and twiddle tables, the per-slice state variables of PAPER.md:100)
+ * lives in one file-scope `static __device__` array of PD_STATIC_SCRATCH_BYTES bytes inside the library, which every GPU
+ * that loads the library holds until the process exits.  The call makes no cudaMalloc / cudaFree, creates no stream,
+ * event or graph and calls no allocating library routine; it enqueues one cudaMemsetAsync per cleared region and
+ * 2*max_iters + 4 kernels on cuda_stream and returns without synchronising.
+ * Limits (else PD_ESTATIC): nx, ny each in {64, 128, 256}; batch <= PD_STATIC_MAX_BATCH;
+ *   nx * ny * ceil(batch/2) <= PD_STATIC_MAX_CELLS  (e.g. 32 slices of 64x64, 8 of 128x128, 2 of 256x256).
+ * field, mask (NULL = ones), chi_out: DEVICE, [batch][ny][nx], as for pd_solve.  lambda, sigma, tau, theta, B0_dir,
+ *   max_iters, tol: as for pd_plan / pd_solve (sigma <= 0 or tau <= 0: automatic steps).
+ * iters_done, relgap, relres: DEVICE, [batch], caller-owned outputs as in pd_get_stats; any may be NULL.
+ * Set-up: the first call on a device asks cudaGetSymbolAddress for the array's device address there (with that device
+ *   current), and the first call for a new (nx, ny, B0_dir) on a device rebuilds the two tables on the host, waits for
+ *   the device (cudaDeviceSynchronize) and uploads them with cudaMemcpy -- make one such call before a capture or a
+ *   timed loop; later calls with the same three values only enqueue.
+ * Sharing: every call on a device uses the same array, which keeps the last call's contents (the call clears what must
+ *   start at zero).  Calls that overlap on the GPU -- two streams, or two host threads -- RACE on it: order them on
+ *   one stream or with events.  Not thread-safe.
+ * Errors: PD_EINVAL, PD_ESTATIC, PD_ESTEP, PD_ECUDA. */
+#define PD_STATIC_MAX_N 256
+#define PD_STATIC_MAX_BATCH 32
+#define PD_STATIC_MAX_CELLS 65536
+#define PD_STATIC_SCRATCH_BYTES 7149056
+int pd_solve_static(int nx, int ny, int batch, int B0_dir, float lambda, float sigma, float tau, float theta,
+                    const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                    int *iters_done, float *relgap, float *relres, void *cuda_stream);
 
 const char *pd_strerror(int code);
 

@@ -14,7 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpd_b200.so")
 
 B0_X, B0_Y = 0, 1
-OK, EINVAL, ESIZE, ESTEP, ENOMEM, ECUDA, EVARIANT = 0, -1, -2, -3, -4, -5, -6
+OK, EINVAL, ESIZE, ESTEP, ENOMEM, ECUDA, EVARIANT, ESTATIC = 0, -1, -2, -3, -4, -5, -6, -7
+STATIC_MAX_N, STATIC_MAX_BATCH, STATIC_MAX_CELLS = 256, 32, 65536   # limits of pd_solve_static (include/pd.h)
 OPT_TV_MODE, OPT_LAMBDA_CONV, OPT_VARIANT, OPT_CHECK_EVERY, OPT_MASK_SHARED, OPT_UNSAFE_STEPS, OPT_KERNEL_TIMING, OPT_FOURIER_DUAL, OPT_HYBRID_TAIL, OPT_GRAPH_LOOP, OPT_REGULARISER, OPT_HOST_CHUNKING = range(12)
 REG_TV, REG_L1 = 0, 1
 KERNEL_CLASSES = ["init", "dual_rows", "dipole_cols", "primal_rows", "finish", "resident", "fd_cols", "fd_rows"]
@@ -24,7 +25,8 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
-           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_line_factors", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror"]
+           "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_line_factors", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror",
+           "pd_solve_static"]
 
 _lib = None
 
@@ -62,6 +64,7 @@ def lib():
         L.pd_line_factors.argtypes = [ip, C.POINTER(ip), C.POINTER(ip)]
         L.pd_get_hybrid_rho.argtypes = [vp, C.POINTER(fp)]
         L.pd_destroy.argtypes = [vp]
+        L.pd_solve_static.argtypes = [ip, ip, ip, ip, fp, fp, fp, fp, vp, vp, vp, ip, fp, vp, vp, vp, vp]
         L.pd_strerror.argtypes = [ip]
         L.pd_strerror.restype = C.c_char_p
         for name in SYMBOLS:
@@ -113,6 +116,23 @@ def line_factors(n):
     if rc < 0:
         raise PdError(rc, strerror(rc))
     return bool(rc), a.value, b.value
+
+
+def solve_static(field, mask, chi_out, max_iters, tol=0.0, b0_dir=B0_Y, lambda_=0.01, sigma=0.25, tau=0.25, theta=1.0,
+                 iters_done=None, relgap=None, relres=None, stream=None):
+    """pd_solve_static: the allocation-free entry point (workspace in a static device array inside the library; limits
+    STATIC_MAX_*).  field, mask (or None), chi_out: float32 CUDA tensors [batch][ny][nx]; iters_done (int32), relgap,
+    relres (float32): optional CUDA tensors [batch].  Enqueues on `stream` (default: torch's current stream)."""
+    batch, ny, nx = field.shape
+    if chi_out.shape != field.shape or (mask is not None and mask.shape != field.shape):
+        raise ValueError("field, mask and chi_out must have the same [batch][ny][nx] shape")
+    for t in (iters_done, relgap, relres):
+        if t is not None and (not t.is_cuda or not t.is_contiguous() or t.numel() < batch or t.element_size() != 4):
+            raise ValueError("statistics outputs must be contiguous 4-byte CUDA tensors of length batch")
+    raw = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+    _check(lib().pd_solve_static(nx, ny, batch, b0_dir, lambda_, sigma, tau, theta, _ptr(field), _ptr(mask), _ptr(chi_out),
+                                 int(max_iters), float(tol), raw(iters_done), raw(relgap), raw(relres),
+                                 _stream_handle(stream)))
 
 
 class Plan:

@@ -849,7 +849,174 @@ int solve_streaming_fd(pd_plan_s *p, const float *field, const float *mask, floa
 
 }  // namespace
 
+// ---- pd_solve_static: the streaming solve (Fourier-domain dual, pd_streaming_fd.cuh) with its WHOLE workspace -- the 13
+// state planes, the per-CTA partial sums, the dipole and twiddle tables, the per-slice state variables -- in one
+// file-scope device array instead of cudaMalloc'ed memory, for callers that may not allocate (CUDA-graph capture, tight
+// serving loops).  Every GPU that loads the library holds the array until the process exits.  In host code the NAME of
+// the array is only a host-side stand-in: its device address comes from cudaGetSymbolAddress, once per device.
+constexpr size_t kStaticCells = PD_STATIC_MAX_CELLS;                 // nx * ny * ceil(batch / 2) of one call, at most
+constexpr size_t kStaticAlign = 256;
+constexpr size_t static_round(size_t bytes) { return (bytes + kStaticAlign - 1) / kStaticAlign * kStaticAlign; }
+constexpr size_t kStaticPartsFloats = 16384;                         // per-CTA partial sums (checked per call)
+constexpr size_t kStaticOffPlanes = 0;
+constexpr size_t kStaticOffD = kStaticOffPlanes + static_round(kSfdPlanes * kStaticCells * sizeof(float2));
+constexpr size_t kStaticOffTwRow = kStaticOffD + static_round(kStaticCells * sizeof(float));
+constexpr size_t kStaticOffTwCol = kStaticOffTwRow + static_round(PD_STATIC_MAX_N * sizeof(float2));
+// from here on: cleared by every call (what a fresh plan's cudaMemset clears)
+constexpr size_t kStaticOffZero = kStaticOffTwCol + static_round(PD_STATIC_MAX_N * sizeof(float2));
+constexpr size_t kStaticSlot = static_round((PD_STATIC_MAX_BATCH + 1) * sizeof(float));
+constexpr size_t kStaticOffStop = kStaticOffZero;                    // stop_iter [batch + 1]
+constexpr size_t kStaticOffIters = kStaticOffStop + kStaticSlot;     // iters_done [batch]
+constexpr size_t kStaticOffP0 = kStaticOffIters + kStaticSlot;
+constexpr size_t kStaticOffGap = kStaticOffP0 + kStaticSlot;
+constexpr size_t kStaticOffRes = kStaticOffGap + kStaticSlot;
+constexpr size_t kStaticOffScale = kStaticOffRes + kStaticSlot;      // cscale [batch + 1]
+constexpr size_t kStaticOffParts = kStaticOffScale + kStaticSlot;
+constexpr size_t kStaticBytes = kStaticOffParts + static_round(kStaticPartsFloats * sizeof(float));
+static_assert(kStaticBytes == PD_STATIC_SCRATCH_BYTES, "include/pd.h states the size of the static workspace");
+
+static __device__ __align__(256) unsigned char pd_static_scratch[kStaticBytes];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDev {
+    int ready;              // cudaGetSymbolAddress done on this device
+    unsigned char *base;    // DEVICE address of pd_static_scratch on this device
+    int nx, ny, b0;         // what the tables in the array were built for (nx = 0: nothing yet)
+};
+StaticDev g_static_dev[kStaticMaxDevices];
+
+bool static_size_ok(int n) { return n == 64 || n == 128 || n == 256; }
+
+// Set-up, once per device (address of the array, shared-memory attributes of the column kernels) and once per
+// (nx, ny, B0_dir) change on it (tables: built on the host in double like pd_plan's, uploaded synchronously).
+int static_setup(int nx, int ny, int b0_dir, StaticDev **out) {
+    int dev = -1;
+    PD_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return PD_EINVAL;
+    StaticDev &sd = g_static_dev[dev];
+    if (!sd.ready) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, pd_static_scratch);   // the current device's copy of the array
+        if (e != cudaSuccess || !ptr) return cuda_fail(e, "cudaGetSymbolAddress(pd_static_scratch)");
+        if (e == cudaSuccess) e = sfd_set_col_smem<64>();
+        if (e == cudaSuccess) e = sfd_set_col_smem<128>();
+        if (e == cudaSuccess) e = sfd_set_col_smem<256>();
+        if (e != cudaSuccess) return cuda_fail(e, "static workspace set-up");
+        sd.base = (unsigned char *)ptr;
+        sd.nx = sd.ny = 0;
+        sd.ready = 1;
+    }
+    if (sd.nx != nx || sd.ny != ny || sd.b0 != b0_dir) {
+        static float hD[kStaticCells];
+        static float2 htw[2][PD_STATIC_MAX_N];
+        PD_CUDA(cudaDeviceSynchronize());   // an earlier call may still be reading the tables
+        sd.nx = 0;
+        const double pi = 3.14159265358979323846264338327950288, scale = 1.0 / ((double)nx * (double)ny);
+        // D/(nx ny), the same arithmetic as build_dipole (axis-aligned B0: the table is even, no symmetrisation needed)
+        for (int jy = 0; jy < ny; ++jy) {
+            const double ky = (double)(jy < (ny + 1) / 2 ? jy : jy - ny) / (double)ny;
+            for (int ix = 0; ix < nx; ++ix) {
+                const double kx = (double)(ix < (nx + 1) / 2 ? ix : ix - nx) / (double)nx;
+                const double k2 = kx * kx + ky * ky, kb = (b0_dir == PD_B0_Y) ? ky : kx;
+                hD[(size_t)jy * nx + ix] = (float)(((ix == 0 && jy == 0) ? 0.0 : 1.0 / 3.0 - kb * kb / k2) * scale);
+            }
+        }
+        for (int w = 0; w < 2; ++w) {
+            const int n = w ? ny : nx;
+            for (int k = 0; k < n; ++k) {
+                const double ang = -2.0 * pi * (double)k / (double)n;
+                htw[w][k] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+            }
+        }
+        PD_CUDA(cudaMemcpy(sd.base + kStaticOffD, hD, (size_t)nx * ny * sizeof(float), cudaMemcpyHostToDevice));
+        PD_CUDA(cudaMemcpy(sd.base + kStaticOffTwRow, htw[0], (size_t)nx * sizeof(float2), cudaMemcpyHostToDevice));
+        PD_CUDA(cudaMemcpy(sd.base + kStaticOffTwCol, htw[1], (size_t)ny * sizeof(float2), cudaMemcpyHostToDevice));
+        PD_CUDA(cudaDeviceSynchronize());
+        sd.nx = nx; sd.ny = ny; sd.b0 = b0_dir;
+    }
+    *out = &sd;
+    return PD_OK;
+}
+
+}  // namespace
+
 extern "C" {
+
+int pd_solve_static(int nx, int ny, int batch, int B0_dir, float lambda, float sigma, float tau, float theta,
+                    const float *field, const float *mask, float *chi_out, int max_iters, float tol,
+                    int *iters_done, float *relgap, float *relres, void *cuda_stream) {
+    if (!field || !chi_out || max_iters < 0 || batch < 1 || (B0_dir != PD_B0_X && B0_dir != PD_B0_Y)) return PD_EINVAL;
+    if (nx < 1 || ny < 1) return PD_EINVAL;
+    const int np = (batch + 1) / 2;
+    if (!static_size_ok(nx) || !static_size_ok(ny) || batch > PD_STATIC_MAX_BATCH ||
+        (size_t)nx * (size_t)ny * (size_t)np > kStaticCells)
+        return PD_ESTATIC;
+    int rc = check_params(lambda, sigma, tau, theta, false, norm_bound(1.0, 1.0));
+    if (rc != PD_OK) return rc;
+    const int nrowparts = ny / (nx == 64 ? pdk::SfdRowCfg<64>::G : nx == 128 ? pdk::SfdRowCfg<128>::G : pdk::SfdRowCfg<256>::G);
+    const int ncolparts = nx / sfd_cols_per_cta(ny);
+    const size_t nr = (size_t)np * nrowparts, nc = (size_t)np * (size_t)(ncolparts > nrowparts ? ncolparts : nrowparts);
+    if (8 * nr + 4 * nc > kStaticPartsFloats) return PD_ESTATIC;
+    StaticDev *sd = nullptr;
+    if ((rc = static_setup(nx, ny, B0_dir, &sd)) != PD_OK) return rc;
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned char *base = sd->base;
+    const size_t P = (size_t)nx * ny, PP = P * (size_t)np;
+    pd_plan_s q;   // only the fields effective_params reads: the same steps as a fresh plan with default options
+    std::memset(&q, 0, sizeof(q));
+    q.lambda_user = lambda; q.sigma_user = sigma; q.tau_user = tau; q.theta = theta; q.max_w = q.max_m = 1.0;
+    StreamFdArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.nx = nx; a.ny = ny; a.batch = batch; a.npairs = np;
+    a.max_iters = max_iters; a.check_every = 1;
+    effective_params(&q, &a.alpha, &a.sigma, &a.tau);
+    a.theta = theta;
+    a.inv_one_plus_sigma = 1.0f / (1.0f + a.sigma);
+    a.tol = tol;
+    a.mask_bstride = (long long)P;
+    a.field = field; a.mask = mask; a.chi_out = chi_out;
+    float2 *b = (float2 *)(base + kStaticOffPlanes);
+    a.Z = b; a.phihat = b + PP; a.M2 = b + 2 * PP;
+    for (int k = 0; k < 2; ++k) { a.phat[k] = b + (3 + k) * PP; a.qx2[k] = b + (5 + k) * PP; a.qy2[k] = b + (7 + k) * PP; }
+    for (int k = 0; k < 3; ++k) a.chi3[k] = b + (9 + k) * PP;
+    a.W2 = b + 12 * PP;
+    a.Dtab = (const float *)(base + kStaticOffD);
+    a.tw_row = (const float2 *)(base + kStaticOffTwRow);
+    a.tw_col = (const float2 *)(base + kStaticOffTwCol);
+    a.stop_iter = (int *)(base + kStaticOffStop);
+    a.P0 = (float *)(base + kStaticOffP0);
+    a.cscale = (float *)(base + kStaticOffScale);
+    a.iters_done = iters_done ? iters_done : (int *)(base + kStaticOffIters);
+    a.relgap = relgap ? relgap : (float *)(base + kStaticOffGap);
+    a.relres = relres ? relres : (float *)(base + kStaticOffRes);
+    a.nrowparts = nrowparts;
+    a.ncolparts = ncolparts;
+    float *parts = (float *)(base + kStaticOffParts);
+    a.p0_part = parts; parts += 2 * nr;
+    a.gap_row = parts; parts += 2 * nr;
+    a.res_part = parts; parts += 4 * nr;
+    a.gap_col[0] = parts; parts += 2 * nc;
+    a.gap_col[1] = parts;
+
+    // the array keeps the last call's contents: clear what a fresh plan starts at zero (state variables, partial sums)
+    PD_CUDA(cudaMemsetAsync(base + kStaticOffZero, 0, kStaticBytes - kStaticOffZero, st));
+    if (iters_done) PD_CUDA(cudaMemsetAsync(iters_done, 0, (size_t)batch * sizeof(int), st));
+    if (relgap) PD_CUDA(cudaMemsetAsync(relgap, 0, (size_t)batch * sizeof(float), st));
+    if (relres) PD_CUDA(cudaMemsetAsync(relres, 0, (size_t)batch * sizeof(float), st));
+    pdk::sfd_scale_kernel<<<a.batch, 256, 0, st>>>(a);
+    PD_DISPATCH(nx, sfd_launch_init_rows, a, st);
+    PD_DISPATCH(ny, sfd_launch_init_cols, a, st);
+    for (int n = 0; n < max_iters; ++n) {
+        PD_DISPATCH(ny, sfd_launch_cols, a, n, st);
+        PD_DISPATCH(nx, sfd_launch_rows, a, n, st);
+    }
+    pdk::sfd_finish_kernel<<<dim3((unsigned)((P + 256 * 8 - 1) / (256 * 8)), np), 256, 0, st>>>(a);
+    PD_CUDA(cudaGetLastError());
+    return PD_OK;
+}
 
 int pd_plan(pd_plan_t *out, int nx, int ny, int batch, int B0_dir, float lambda, float sigma, float tau, float theta) {
     if (!out) return PD_EINVAL;
@@ -1282,6 +1449,8 @@ const char *pd_strerror(int code) {
         case PD_ENOMEM: return "out of device memory";
         case PD_ECUDA: return g_cuda_err;
         case PD_EVARIANT: return "requested variant is not available for this size";
+        case PD_ESTATIC: return "pd_solve_static: nx and ny must each be 64, 128 or 256, batch <= 32 and nx*ny*ceil(batch/2) <= 65536 "
+                                "(the static workspace of PD_STATIC_SCRATCH_BYTES bytes holds no more); use pd_plan / pd_solve";
         default: return "unknown error code";
     }
 }

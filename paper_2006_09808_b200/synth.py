@@ -264,3 +264,36 @@ def random_case(nx, ny, batch, seed, with_mask=True, with_weight=False):
             w[b] = (0.2 + 0.8 * uniform01(stream_key(100 + seed, b, 0, _BG), nx * ny)).reshape(ny, nx)
     out.update(field=f, mask=m, weight=w)
     return out
+
+
+_ECHO_PHASE, _ECHO_NOISE = 5, 6
+
+
+def echo_pair(cid, nslices=None, first_slice=0, phase_span=2.5, noise=0.01):
+    """The two complex volumes of the acquisition (without / with the echo shift T_shift) whose phase
+    difference encodes generate()'s field map -- inputs of the pre-processing step (flow step (1)).
+
+    Per batch entry (slice*ncoils + coil): magnitude A = tissue (1 inside the mask, 0.2 outside) x a smooth coil
+    sensitivity (a Gaussian bump centred on a circle around the slice, one position per coil) ; a smooth receive phase
+    theta0 ; s0 = A exp(i theta0) + n0, s1 = A exp(i (theta0 + pscale field)) + n1 with complex Gaussian noise of standard
+    deviation `noise`, pscale = phase_span / max|field| so that the phase difference stays inside (-pi, pi) (the reason
+    T_shift is small).  Returns dict(cfg, s0, s1 (complex64 [batch][ny][nx]), fscale = 1/pscale, field, mask)."""
+    d = generate(cid, nslices, first_slice)
+    cfg, f, m = d["cfg"], d["field"].astype(np.float64), d["mask"]
+    batch, ny, nx = f.shape
+    nc = cfg.ncoils
+    pscale = phase_span / float(np.max(np.abs(f)))
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    s0 = np.empty((batch, ny, nx), np.complex64)
+    s1 = np.empty((batch, ny, nx), np.complex64)
+    for b in range(batch):
+        s, c = first_slice + b // nc, b % nc
+        ang = 2.0 * np.pi * (c + 0.25) / nc
+        cx, cy = nx * (0.5 + 0.45 * np.cos(ang)), ny * (0.5 + 0.45 * np.sin(ang))
+        sens = 0.15 + np.exp(-((xx - cx) ** 2 + (yy - cy) ** 2) / (2.0 * (0.45 * min(nx, ny)) ** 2))
+        A = sens * np.where(m[b] > 0, 1.0, 0.2)
+        theta0 = 2.0 * np.pi * 5.0 * background(nx, ny, stream_key(cfg.cid, s, c, _ECHO_PHASE))
+        g = normal01(stream_key(cfg.cid, s, c, _ECHO_NOISE), 4 * nx * ny).reshape(4, ny, nx)
+        s0[b] = (A * np.exp(1j * theta0) + noise * (g[0] + 1j * g[1])).astype(np.complex64)
+        s1[b] = (A * np.exp(1j * (theta0 + pscale * f[b])) + noise * (g[2] + 1j * g[3])).astype(np.complex64)
+    return {"cfg": cfg, "s0": s0, "s1": s1, "fscale": 1.0 / pscale, "field": d["field"], "mask": m}

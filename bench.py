@@ -204,6 +204,73 @@ def run_reference(args):
     return 0
 
 
+def run_prepost(args):
+    """--prepost: the steps either side of the iteration (NEXT-4) on the shape of the chosen workload: pd_preprocess
+    (automatic scale: max pass + main pass) and pd_combine_coils, CUDA events on the launch stream, HBM roofline from the
+    algorithmic bytes (16 + 28 B per pixel; 8 ncoils + 4 B per output pixel).  Its own JSON line."""
+    import torch
+    from paper_2006_09808_b200 import binding
+    torch.cuda.set_device(0)
+    binding.lib()
+    cfg = synth.CONFIGS[WORKLOADS[args.workload]]
+    nsl = max(1, min(cfg.nslices, 4))
+    e = synth.echo_pair(cfg.cid, nslices=nsl)
+    rep = cfg.nslices // nsl
+    s0 = torch.from_numpy(e["s0"]).cuda().repeat(rep, 1, 1).contiguous()
+    s1 = torch.from_numpy(e["s1"]).cuda().repeat(rep, 1, 1).contiguous()
+    batch, ny, nx = s0.shape
+    npix = batch * ny * nx
+    f = torch.empty((batch, ny, nx), device="cuda")
+    w, m = torch.empty_like(f), torch.empty_like(f)
+    wmax = torch.zeros(1, device="cuda")
+    out = torch.empty((batch // cfg.ncoils, ny, nx), device="cuda")
+    flush = torch.empty(64 * 1024 * 1024, device="cuda") if npix * 44 <= 2 * 126e6 else None
+    peak, peak_src = load_peaks()
+
+    def timed(fn):
+        for _ in range(args.warmup):
+            fn()
+        tot = 0.0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(args.steps):
+            if flush is not None:
+                flush.fill_(1.0)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            tot += e0.elapsed_time(e1)
+        return tot / args.steps
+
+    sampler = ClockSampler(0)
+    ms_pre = timed(lambda: binding.preprocess(s0, s1, e["fscale"], 0.3, field=f, weight=w, mask=m, wmax=wmax))
+    ms_pre_given = timed(lambda: binding.preprocess(s0, s1, e["fscale"], 0.3, wscale=1.0, field=f, weight=w, mask=m))
+    ms_comb = timed(lambda: binding.combine_coils(f, w, cfg.ncoils, out))
+    clocks = sampler.stop()
+
+    def roof(ms, nbytes, launches):
+        gbs = nbytes / (ms * 1e-3) / 1e9
+        return {"ms": ms, "launches": launches, "algorithmic_bytes": nbytes, "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
+                "frac": gbs / peak, "peak_source": peak_src}
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import pd_prepost_oracle as po
+    t0 = time.perf_counter()
+    po.field_map(e["s0"], e["s1"], e["fscale"]); po.weight(e["s0"], e["s1"]); po.mask_f32(e["s0"], e["s1"], 0.3)
+    dt = time.perf_counter() - t0
+    line = {"metric": "prepost_pixels_per_s", "value": npix / (ms_pre * 1e-3), "unit": "pixels/s (pd_preprocess, automatic scale)", "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_pre, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "%s shape: %d maps of %dx%d, %d coils (synth.echo_pair of %d slices tiled x%d)"
+                                   % (args.workload, batch, ny, nx, cfg.ncoils, nsl, rep),
+                       "l2": "flushed between steps" if flush is not None else "working set exceeds the 126 MB L2"},
+            "preprocess_auto_scale": roof(ms_pre, 44.0 * npix, 2), "preprocess_given_scale": roof(ms_pre_given, 28.0 * npix, 1),
+            "combine_coils": roof(ms_comb, (8.0 * cfg.ncoils + 4.0) * (npix // cfg.ncoils), 1),
+            "cpu_baseline": {"value": e["s0"].size / dt, "unit": "pixels/s", "cores": 1, "kind": "oracle (numpy, float64)",
+                             "sample": "%d maps, %.2f s" % (e["s0"].shape[0], dt)},
+            "gpu_launches": 4 * args.steps, "clocks": clocks}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def flops_per_slice_it_ns(cfg):
     P = cfg.nx * cfg.ny
     return P * (10.0 * math.log2(P) + 32.0)
@@ -239,11 +306,15 @@ def main():
     ap.add_argument("--no-graph-loop", action="store_true",
                     help="PD_OPT_GRAPH_LOOP = 0: plain launches from the host instead of the graphed device-side loop "
                          "(used for the ncu launch lists)")
+    ap.add_argument("--prepost", action="store_true",
+                    help="time pd_preprocess and pd_combine_coils (NEXT-4) on the workload's shape instead of the solve; own JSON line")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.prepost:
+        return run_prepost(args)
 
     import torch
     import torch.distributed as dist

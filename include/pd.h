@@ -202,6 +202,32 @@ int pd_get_hybrid_rho(pd_plan_t p, float *rho);
 
 int pd_destroy(pd_plan_t p);
 
+/* pd_preprocess -- flow step (1): "Preprocess the two data collected by the positive contrast MRI to obtain
+ * ... the weighting matrix W, the mask Mask, and the phase contrast field iFreq delta" from the two volumes acquired
+ * without and with the echo shift T_shift.  The paper gives no formulas; readings R20, R21:
+ *   field  = arg(s1 * conj(s0)) * fscale        principal value in (-pi, pi], no unwrapping; 0 where the product is 0
+ *   m      = sqrt(|s0| |s1|);  weight = m * wscale;  mask = 1 where weight > threshold, else 0
+ * s0, s1 : DEVICE, const, complex64 interleaved (re, im), npixels = batch*ny*nx pixels in the layout of pd_solve, 16-byte
+ *          aligned (s0: without the shift, s1: with it).
+ * fscale : radians -> the unit of the field map, e.g. 1 / (2 pi T_shift gamma B0) for ppm.
+ * wscale : > 0: used as given.  <= 0: automatic, 1 / max(m) over all npixels (|W| <= 1, what the automatic steps of
+ *          pd_plan assume); wmax (DEVICE, one float, required in this mode) receives that maximum.
+ * field, weight, mask : DEVICE outputs, npixels floats each, 16-byte aligned; any may be NULL (not computed).
+ * The integer decisions (mask; the maximum) are taken in fp32 by the fixed sequence a_k = fl(fl(re_k^2) + fl(im_k^2)),
+ * m = sqrt(sqrt(fl(a_0 a_1))), weight = fl(m * fl(1/max)), all round-to-nearest, no fused multiply-add.
+ * Enqueues one or two kernels (and a 4-byte memset) on cuda_stream; allocates nothing; does not synchronise.
+ * Errors: PD_EINVAL (null input, misaligned pointer, automatic scale without wmax), PD_ECUDA. */
+int pd_preprocess(const float *s0, const float *s1, long long npixels, float fscale, float wscale, float threshold,
+                  float *field, float *weight, float *mask, float *wmax, void *cuda_stream);
+
+/* pd_combine_coils -- "the multi-coil acquisition data from parallel imaging": every coil's field map is
+ * reconstructed independently (batch index slice*ncoils + coil) and the per-coil maps are combined, reading
+ * R22: chi_out[s](x) = sum_c W_c(x)^2 chi_c(x) / sum_c W_c(x)^2 (coils in index order, fp32), 0 where no coil has weight.
+ * chi, weight : DEVICE, const, [nslices*ncoils][ny][nx] (weight: e.g. pd_preprocess's).  chi_out : DEVICE, [nslices][ny][nx].
+ * Enqueues one kernel on cuda_stream; allocates nothing.  Errors: PD_EINVAL, PD_ECUDA. */
+int pd_combine_coils(const float *chi, const float *weight, int nslices, int ncoils, int ny, int nx, float *chi_out,
+                     void *cuda_stream);
+
 /* pd_solve_static: ONE allocation-free entry point, for callers that cannot call cudaMalloc (code under CUDA-graph
  * capture, tight serving loops, harnesses that forbid it).  It runs the same iteration as pd_solve
  * through the streaming kernels with the Fourier-domain dual (W = identity, isotropic TV, lambda on the regulariser,

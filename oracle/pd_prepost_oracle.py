@@ -6,12 +6,13 @@ TEST INFRASTRUCTURE ONLY: only tests/, __graft_entry__.smoke() and bench.py's cp
 import this module.  Plain numpy, float64, one whole-array statement per step; pinned by tests/test_oracle_prepost_pins.py
 against closed forms, hand-computed values and pure-Python brute force.
 
-The paper names these steps and gives no formulas; the readings are DESIGN.md R18-R20:
-  R18  field = arg(s1 * conj(s0)) * fscale, principal value in (-pi, pi], no unwrapping ("two data were acquired (with or
+The paper names these steps and gives no formulas; the readings are DESIGN.md R20-R22 (that the code computes them is
+pinned; that they are the authors' own pre-processing is PARITY UNPINNED -- there is nothing in the paper to pin against):
+  R20  field = arg(s1 * conj(s0)) * fscale, principal value in (-pi, pi], 0 where the product is 0, no unwrapping ("two data were acquired (with or
        w/o echo shift) for measuring the field map"; fscale = 1 / (2 pi T_shift gamma B0) is the caller's).
-  R19  magnitude m = sqrt(|s0| |s1|); W = m * wscale with wscale = 1 / max(m over the whole stack) unless given (so that
+  R21  magnitude m = sqrt(|s0| |s1|); W = m * wscale with wscale = 1 / max(m over the whole stack) unless given (so that
        |W| <= 1, which the step bound of PAPER.md:44 assumes); Mask = 1 where W > threshold, else 0.
-  R20  chi(x) = sum_c W_c(x)^2 chi_c(x) / sum_c W_c(x)^2 over the coils of a slice, 0 where the denominator is 0 (the
+  R22  chi(x) = sum_c W_c(x)^2 chi_c(x) / sum_c W_c(x)^2 over the coils of a slice, 0 where the denominator is 0 (the
        magnitude-squared weighted mean; every coil map is reconstructed independently).
 Where floating point decides an integer (the mask; the stack maximum that scales W) the decision is specified in the
 kernel's precision, fp32, as a fixed sequence of correctly rounded IEEE operations -- *_f32 below -- and the double
@@ -21,18 +22,18 @@ import numpy as np
 
 
 def field_map(s0, s1, fscale):
-    """R18.  s0, s1: complex [..][ny][nx]; returns float64."""
+    """R20.  s0, s1: complex [..][ny][nx]; returns float64."""
     d = np.asarray(s1, np.complex128) * np.conj(np.asarray(s0, np.complex128))
-    return np.arctan2(d.imag, d.real) * float(fscale)
+    return np.where(d == 0, 0.0, np.arctan2(d.imag, d.real)) * float(fscale)   # a zero product has no phase: 0
 
 
 def magnitude(s0, s1):
-    """R19: sqrt(|s0| |s1|), float64."""
+    """R21: sqrt(|s0| |s1|), float64."""
     return np.sqrt(np.abs(np.asarray(s0, np.complex128)) * np.abs(np.asarray(s1, np.complex128)))
 
 
 def weight(s0, s1, wscale=None):
-    """R19: W = m * wscale, wscale = 1 / max(m) over everything passed in unless given.  float64."""
+    """R21: W = m * wscale, wscale = 1 / max(m) over everything passed in unless given.  float64."""
     m = magnitude(s0, s1)
     if wscale is None:
         mx = float(m.max())
@@ -41,7 +42,7 @@ def weight(s0, s1, wscale=None):
 
 
 def mask_from_weight(W, threshold):
-    """R19 in double precision (the definition): 1 where W > threshold."""
+    """R21 in double precision (the definition): 1 where W > threshold."""
     return (np.asarray(W, np.float64) > float(threshold)).astype(np.float64)
 
 
@@ -73,7 +74,7 @@ def mask_f32(s0, s1, threshold, wscale=None):
 
 
 def combine_coils(chi, W, ncoils):
-    """R20.  chi, W: [nslices*ncoils][ny][nx], batch index slice*ncoils + coil (BASELINE.json configs[3]).  Returns
+    """R22.  chi, W: [nslices*ncoils][ny][nx], batch index slice*ncoils + coil (BASELINE.json configs[3]).  Returns
     float64 [nslices][ny][nx]."""
     chi = np.asarray(chi, np.float64)
     W = np.asarray(W, np.float64)

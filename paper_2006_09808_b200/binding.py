@@ -26,7 +26,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
            "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_line_factors", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror",
-           "pd_solve_static"]
+           "pd_solve_static", "pd_preprocess", "pd_combine_coils"]
 
 _lib = None
 
@@ -64,6 +64,8 @@ def lib():
         L.pd_line_factors.argtypes = [ip, C.POINTER(ip), C.POINTER(ip)]
         L.pd_get_hybrid_rho.argtypes = [vp, C.POINTER(fp)]
         L.pd_destroy.argtypes = [vp]
+        L.pd_preprocess.argtypes = [vp, vp, C.c_longlong, fp, fp, fp, vp, vp, vp, vp, vp]
+        L.pd_combine_coils.argtypes = [vp, vp, ip, ip, ip, ip, vp, vp]
         L.pd_solve_static.argtypes = [ip, ip, ip, ip, fp, fp, fp, fp, vp, vp, vp, ip, fp, vp, vp, vp, vp]
         L.pd_strerror.argtypes = [ip]
         L.pd_strerror.restype = C.c_char_p
@@ -116,6 +118,26 @@ def line_factors(n):
     if rc < 0:
         raise PdError(rc, strerror(rc))
     return bool(rc), a.value, b.value
+
+
+def preprocess(s0, s1, fscale, threshold, wscale=0.0, field=None, weight=None, mask=None, wmax=None, stream=None):
+    """pd_preprocess: s0, s1 complex64 CUDA tensors [batch][ny][nx] (without / with the echo shift); field, weight, mask:
+    float32 CUDA tensors of the same shape or None; wmax: float32 CUDA tensor of one element (needed when wscale <= 0)."""
+    for t in (s0, s1):
+        if not t.is_cuda or not t.is_contiguous() or str(t.dtype) != "torch.complex64" or t.data_ptr() % 16:
+            raise ValueError("expected contiguous, 16-byte aligned complex64 CUDA tensors")
+    if s0.shape != s1.shape or any(t is not None and t.shape != s0.shape for t in (field, weight, mask)):
+        raise ValueError("s0, s1 and the outputs must have the same shape")
+    _check(lib().pd_preprocess(C.c_void_p(s0.data_ptr()), C.c_void_p(s1.data_ptr()), s0.numel(), float(fscale), float(wscale),
+                               float(threshold), _ptr(field), _ptr(weight), _ptr(mask), _ptr(wmax), _stream_handle(stream)))
+
+
+def combine_coils(chi, weight, ncoils, chi_out, stream=None):
+    """pd_combine_coils: chi, weight [nslices*ncoils][ny][nx] -> chi_out [nslices][ny][nx] (float32 CUDA tensors)."""
+    batch, ny, nx = chi.shape
+    if batch % ncoils or weight.shape != chi.shape or tuple(chi_out.shape) != (batch // ncoils, ny, nx):
+        raise ValueError("chi, weight: [nslices*ncoils][ny][nx]; chi_out: [nslices][ny][nx]")
+    _check(lib().pd_combine_coils(_ptr(chi), _ptr(weight), batch // ncoils, ncoils, ny, nx, _ptr(chi_out), _stream_handle(stream)))
 
 
 def solve_static(field, mask, chi_out, max_iters, tol=0.0, b0_dir=B0_Y, lambda_=0.01, sigma=0.25, tau=0.25, theta=1.0,

@@ -48,6 +48,9 @@ double norm_bound(double w, double m) { return 4.0 / 9.0 * w * w + 8.0 * m * m; 
 
 }  // namespace
 
+// for the other translation units of the library (pd_prepost.cu): record the text behind PD_ECUDA
+int pd_cuda_fail_(int cuda_error, const char *where) { return cuda_fail((cudaError_t)cuda_error, where); }
+
 constexpr int kGraphSlots = 8, kMaxChunks = 6;
 
 struct pd_plan_s {

@@ -1,4 +1,4 @@
-"""Pins of oracle/pd_prepost_oracle.py (NEXT-4: pre-processing and coil combination; readings R18-R20 of DESIGN.md)
+"""Pins of oracle/pd_prepost_oracle.py (NEXT-4: pre-processing and coil combination; readings R20-R22 of DESIGN.md)
 against things other than itself: closed forms, hand-computed values, pure-Python brute force.  No GPU."""
 import cmath
 import math
@@ -16,7 +16,7 @@ from paper_2006_09808_b200 import synth  # noqa: E402
 
 
 def test_p17_field_map_closed_form():
-    """s0 = A e^{ia}, s1 = B e^{i(a+d)}  =>  field = d * fscale for d in (-pi, pi), whatever A, B, a (R18)."""
+    """s0 = A e^{ia}, s1 = B e^{i(a+d)}  =>  field = d * fscale for d in (-pi, pi), whatever A, B, a (R20)."""
     rng = np.random.default_rng(17)
     d = np.linspace(-3.1, 3.1, 63).reshape(7, 9)
     a = rng.uniform(-np.pi, np.pi, d.shape)
@@ -32,6 +32,7 @@ def test_p17_field_map_closed_form():
     # antisymmetry under exchange of the two echoes, and a zero pixel gives 0
     assert np.allclose(po.field_map(s1, s0, 0.37), -po.field_map(s0, s1, 0.37))
     assert po.field_map(np.zeros((1, 1), complex), np.ones((1, 1), complex), 1.0)[0, 0] == 0.0
+    assert po.field_map(np.zeros((1, 2), complex), np.array([[-1 - 1j, -2.0]]), 1.0).tolist() == [[0.0, 0.0]]   # not pi from a -0
 
 
 def test_p17b_field_map_recovers_the_simulated_field():
@@ -42,7 +43,7 @@ def test_p17b_field_map_recovers_the_simulated_field():
 
 
 def test_p18_weight_and_mask_hand_values():
-    """|3+4i| = 5, |20i| = 20 -> m = sqrt(100) = 10 ; |2| = 2, |8| = 8 -> m = 4 ; zero pixel -> 0 (R19)."""
+    """|3+4i| = 5, |20i| = 20 -> m = sqrt(100) = 10 ; |2| = 2, |8| = 8 -> m = 4 ; zero pixel -> 0 (R21)."""
     s0 = np.array([[[3 + 4j, 2, 0, 1]]])
     s1 = np.array([[[20j, -8, 5, 1j]]])
     assert po.magnitude(s0, s1)[0, 0].tolist() == pytest.approx([10.0, 4.0, 0.0, 1.0])
@@ -75,7 +76,7 @@ def test_p18b_fp32_decisions_agree_with_the_definition_away_from_the_threshold()
 
 
 def test_p19_combine_coils_hand_values_and_brute_force():
-    """chi = (1, 3): W = (1, 1) -> 2 ; W = (1, 2) -> (1 + 4*3)/5 = 2.6 ; W = (0, 0) -> 0 ; W = (0, 7) -> 3 (R20)."""
+    """chi = (1, 3): W = (1, 1) -> 2 ; W = (1, 2) -> (1 + 4*3)/5 = 2.6 ; W = (0, 0) -> 0 ; W = (0, 7) -> 3 (R22)."""
     chi = np.array([1.0, 3.0]).reshape(2, 1, 1)
     for w, want in [((1, 1), 2.0), ((1, 2), 2.6), ((0, 0), 0.0), ((0, 7), 3.0), ((-2, 1), 1.4)]:
         assert po.combine_coils(chi, np.array(w, float).reshape(2, 1, 1), 2)[0, 0, 0] == pytest.approx(want)

@@ -271,6 +271,57 @@ def run_prepost(args):
     return 0
 
 
+def run_volume(args):
+    """--volume: the true 3-D variant (NEXT-2) on 8 coil volumes of 256 x 256 x 64 (the voxel count of 512 slices of 256^2),
+    100 iterations; voxel-iterations/s, HBM roofline of the whole step from its algorithmic bytes (DESIGN.md 5.7:
+    the bytes its seven passes must move: 12 + 16 + 44 + 16 + 12 + 32 + 32 = 164 B per voxel and iteration with a mask).  Its own JSON line."""
+    import torch
+    from paper_2006_09808_b200 import binding
+    torch.cuda.set_device(0)
+    binding.lib()
+    nx, ny, nz, nvol, iters = 256, 256, 64, 8, 100
+    case = synth.volume_case(nx, ny, nz, nvol=2, seed=9)
+    f = torch.from_numpy(case["field"]).cuda().repeat(nvol // 2, 1, 1, 1).contiguous()
+    m = torch.from_numpy(case["mask"]).cuda().repeat(nvol // 2, 1, 1, 1).contiguous()
+    lam = 0.02 * float(np.abs(case["field"]).max())
+    out = torch.empty_like(f)
+    plan = binding.Plan3D(nx, ny, nz, nvol, 2, lam, 0.25, 0.25, 1.0)
+    peak, peak_src = load_peaks()
+    for _ in range(args.warmup):
+        plan.solve(f, m, out, iters)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        plan.solve(f, m, out, iters)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    clocks = sampler.stop()
+    launches = plan.last_launch_count
+    plan.destroy()
+    nvox = nvol * nz * ny * nx
+    bytes_per_voxel_it = 164.0
+    gbs = bytes_per_voxel_it * nvox * iters / (ms * 1e-3) / 1e9
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import pd3_oracle as o3
+    t0 = time.perf_counter()
+    o3.solve3(case["field"][0], case["mask"][0], lambda_=lam, sigma=0.25, tau=0.25, max_iters=4)
+    dt = time.perf_counter() - t0
+    line = {"metric": "pd3_voxel_iterations_per_s", "value": nvox * iters / (ms * 1e-3), "unit": "voxel-iterations/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "V1: %d coil volumes of %dx%dx%d (synth.volume_case), %d iterations, B0 along z, mask" % (nvol, nx, ny, nz, iters),
+                       "l2": "working set (%.1f GB) exceeds the 126 MB L2" % (48.0 * nvox / 1e9)},
+            "roofline": {"kernel": "whole step (7 launches per iteration)", "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
+                         "frac": gbs / peak, "algorithmic_bytes_per_voxel_iteration": bytes_per_voxel_it, "peak_source": peak_src, "traffic": None},
+            "cpu_baseline": {"value": nz * ny * nx * 4 / dt, "unit": "voxel-iterations/s", "cores": os.cpu_count(), "kind": "oracle (numpy float64, numpy.fft)",
+                             "sample": "1 volume, 4 iterations, %.1f s" % dt},
+            "gpu_launches": launches * args.steps, "clocks": clocks}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def flops_per_slice_it_ns(cfg):
     P = cfg.nx * cfg.ny
     return P * (10.0 * math.log2(P) + 32.0)
@@ -306,6 +357,7 @@ def main():
     ap.add_argument("--no-graph-loop", action="store_true",
                     help="PD_OPT_GRAPH_LOOP = 0: plain launches from the host instead of the graphed device-side loop "
                          "(used for the ncu launch lists)")
+    ap.add_argument("--volume", action="store_true", help="time the true 3-D variant (NEXT-2, pd_solve3d); own JSON line")
     ap.add_argument("--prepost", action="store_true",
                     help="time pd_preprocess and pd_combine_coils (NEXT-4) on the workload's shape instead of the solve; own JSON line")
     args = ap.parse_args()
@@ -315,6 +367,8 @@ def main():
         return run_reference(args)
     if args.prepost:
         return run_prepost(args)
+    if args.volume:
+        return run_volume(args)
 
     import torch
     import torch.distributed as dist

@@ -202,6 +202,25 @@ int pd_get_hybrid_rho(pd_plan_t p, float *rho);
 
 int pd_destroy(pd_plan_t p);
 
+/* The true 3-D variant: Eq.(1) as PAPER.md:37-40 literally states it -- "G is the gradient
+ * operator in all three dimensions" -- with the 3-D dipole kernel D3(k) = 1/3 - k_b^2/|k|^2, D3(0) = 0,
+ * k = (fi/nx, fj/ny, fk/nz) with signed indices (isotropic voxels; reading R23), one problem per VOLUME:
+ * the same iteration with q of three components projected on the lambda-ball by its pointwise Euclidean
+ * norm, forward differences with Neumann boundary on all three axes, W = identity, lambda on the regulariser (R2).  The
+ * slices of a volume are coupled by the z transform and the z difference: there is no per-slice stop, the call runs
+ * exactly max_iters iterations.  A first streaming implementation (7 launches per iteration).
+ * pd_plan3d: nx in {16..256}, ny, nz in {8..256}, powers of two (else PD_ESIZE); nvol independent volumes (coils);
+ *   B0_axis 0 = x, 1 = y, 2 = z; sigma <= 0 or tau <= 0: automatic steps 1/sqrt(4/9 + 12); explicit steps with
+ *   sigma*tau*(4/9 + 12) >= 1 give PD_ESTEP.  Allocates 48 bytes per voxel of workspace + the D3 table.
+ * pd_solve3d: field, mask (NULL = ones), chi_out: DEVICE, [nvol][nz][ny][nx] fp32, x fastest; chi_out is the primal
+ *   state during the call.  Enqueues everything on cuda_stream; does not synchronise.
+ * Errors: PD_EINVAL, PD_ESIZE, PD_ESTEP, PD_ENOMEM, PD_ECUDA. */
+typedef struct pd_plan3d_s *pd_plan3d_t;
+int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, float lambda, float sigma, float tau, float theta);
+int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_out, int max_iters, void *cuda_stream);
+int pd_last_launch_count3d(pd_plan3d_t p);   /* kernels enqueued by the last pd_solve3d */
+int pd_destroy3d(pd_plan3d_t p);
+
 /* pd_preprocess -- flow step (1): "Preprocess the two data collected by the positive contrast MRI to obtain
  * ... the weighting matrix W, the mask Mask, and the phase contrast field iFreq delta" from the two volumes acquired
  * without and with the echo shift T_shift.  The paper gives no formulas; readings R20, R21:

@@ -26,7 +26,8 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
            "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_line_factors", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror",
-           "pd_solve_static", "pd_preprocess", "pd_combine_coils"]
+           "pd_solve_static", "pd_preprocess", "pd_combine_coils", "pd_plan3d", "pd_solve3d", "pd_last_launch_count3d",
+           "pd_destroy3d"]
 
 _lib = None
 
@@ -66,6 +67,10 @@ def lib():
         L.pd_destroy.argtypes = [vp]
         L.pd_preprocess.argtypes = [vp, vp, C.c_longlong, fp, fp, fp, vp, vp, vp, vp, vp]
         L.pd_combine_coils.argtypes = [vp, vp, ip, ip, ip, ip, vp, vp]
+        L.pd_plan3d.argtypes = [C.POINTER(vp), ip, ip, ip, ip, ip, fp, fp, fp, fp]
+        L.pd_solve3d.argtypes = [vp, vp, vp, vp, ip, vp]
+        L.pd_last_launch_count3d.argtypes = [vp]
+        L.pd_destroy3d.argtypes = [vp]
         L.pd_solve_static.argtypes = [ip, ip, ip, ip, fp, fp, fp, fp, vp, vp, vp, ip, fp, vp, vp, vp, vp]
         L.pd_strerror.argtypes = [ip]
         L.pd_strerror.restype = C.c_char_p
@@ -118,6 +123,31 @@ def line_factors(n):
     if rc < 0:
         raise PdError(rc, strerror(rc))
     return bool(rc), a.value, b.value
+
+
+class Plan3D:
+    """pd_plan3d(nx, ny, nz, nvol, B0_axis, lambda, sigma, tau, theta): the true 3-D variant, one problem per volume."""
+
+    def __init__(self, nx, ny, nz, nvol=1, b0_axis=2, lambda_=0.01, sigma=0.25, tau=0.25, theta=1.0):
+        self._h = C.c_void_p()
+        self.shape = (nvol, nz, ny, nx)
+        _check(lib().pd_plan3d(C.byref(self._h), nx, ny, nz, nvol, b0_axis, lambda_, sigma, tau, theta))
+
+    def solve(self, field, mask, chi_out, max_iters, stream=None):
+        """field, mask (or None), chi_out: float32 CUDA tensors [nvol][nz][ny][nx]."""
+        for t in (field, mask, chi_out):
+            if t is not None and tuple(t.shape) != self.shape:
+                raise ValueError("expected shape %r" % (self.shape,))
+        _check(lib().pd_solve3d(self._h, _ptr(field), _ptr(mask), _ptr(chi_out), int(max_iters), _stream_handle(stream)))
+
+    @property
+    def last_launch_count(self):
+        return lib().pd_last_launch_count3d(self._h)
+
+    def destroy(self):
+        if self._h:
+            _check(lib().pd_destroy3d(self._h))
+            self._h = C.c_void_p()
 
 
 def preprocess(s0, s1, fscale, threshold, wscale=0.0, field=None, weight=None, mask=None, wmax=None, stream=None):

@@ -1,0 +1,337 @@
+// pd_volume.cu -- the true 3-D variant: Eq.(1) as the paper literally states it, "G is the
+// gradient operator in all three dimensions", with the 3-D dipole kernel, one problem per VOLUME
+// [nz][ny][nx] (slices are coupled: no per-slice stop, the iteration count is the caller's; R23, 5.7).
+//
+// A first, correct, streaming implementation (not yet tuned like the 2-D path): W = identity, so the dual p lives in the
+// Fourier domain as in DESIGN.md 5.0 -- ONE 3-D FFT round trip per iteration:
+//   x lines (chi_bar real -> complex) ; y lines ; z lines + [ p^ <- (p^ + sigma (D Z - phi^))/(1+sigma) ; Z <- D p^ ] + z lines
+//   back ; y lines back ; x lines back (-> K p, real) ; q-update (3 components) ; chi-update with the 3-D divergence.
+// Line transforms: radix-2 in shared memory, 16 lines per CTA; strided axes (y, z) are read as tiles of 16 adjacent x so
+// that every access is a full 128-byte line.  Twiddles and D come from double-precision host tables (R17).  No cuFFT.
+#include "../../include/pd.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+int pd_cuda_fail_(int cuda_error, const char *where);   // pd_api.cu: records the text behind PD_ECUDA
+
+namespace {
+
+constexpr int kTL = 16;         // lines per CTA
+constexpr int kThreads = 256;
+
+enum { kModePlain = 0, kModeInReal = 1, kModeOutReal = 2, kModeStoreSpectrum = 3, kModeDual = 4 };
+
+struct FftArgs {
+    const float *in_real;     // kModeInReal
+    float2 *z;                // complex work volume (in place)
+    float *out_real;          // kModeOutReal
+    float2 *phihat, *phat;    // kModeStoreSpectrum / kModeDual
+    const float *D;           // [nz][ny][nx], unscaled
+    const float2 *tw;         // exp(-2 pi i k / N), k < N/2
+    long long nlines;         // x pass: number of lines
+    long long S;              // strided pass: distance between consecutive points of a line (nx, or nx*ny)
+    float sigma, inv1ps, out_scale;
+    int inverse;
+};
+
+template <int N> struct Log2 { static constexpr int v = 1 + Log2<N / 2>::v; };
+template <> struct Log2<1> { static constexpr int v = 0; };
+
+template <int N>
+__device__ __forceinline__ int brev(int k) { return (int)(__brev((unsigned)k) >> (32 - Log2<N>::v)); }
+
+// radix-2 decimation in time over the kTL lines of the tile; input in bit-reversed order, output in natural order
+template <int N>
+__device__ __forceinline__ void fft_tile(float2 *buf, const float2 *tws, bool inverse) {
+    constexpr int LOGN = Log2<N>::v, LD = N + 1;
+#pragma unroll 1
+    for (int s = 0; s < LOGN; ++s) {
+        const int half = 1 << s;
+        for (int idx = threadIdx.x; idx < kTL * (N / 2); idx += kThreads) {
+            const int l = idx / (N / 2), b = idx % (N / 2);
+            const int j = b & (half - 1), i0 = ((b >> s) << (s + 1)) + j, i1 = i0 + half;
+            float2 w = tws[j << (LOGN - 1 - s)];
+            if (inverse) w.y = -w.y;
+            const float2 a = buf[l * LD + i0], c = buf[l * LD + i1];
+            const float2 t = make_float2(c.x * w.x - c.y * w.y, c.x * w.y + c.y * w.x);
+            buf[l * LD + i0] = make_float2(a.x + t.x, a.y + t.y);
+            buf[l * LD + i1] = make_float2(a.x - t.x, a.y - t.y);
+        }
+        __syncthreads();
+    }
+}
+
+// STRIDED = false: lines along x (contiguous), the tile is 16 consecutive lines.
+// STRIDED = true : point k of line (o, j) sits at (o*N + k)*S + j; the tile is 16 consecutive j (blockIdx.x), o = blockIdx.y.
+template <int N, bool STRIDED>
+__global__ void __launch_bounds__(kThreads) fft_lines_kernel(const FftArgs a, const int mode) {
+    constexpr int LD = N + 1;
+    __shared__ float2 buf[kTL * LD];
+    __shared__ float2 tws[N / 2 > 0 ? N / 2 : 1];
+    for (int k = threadIdx.x; k < N / 2; k += kThreads) tws[k] = a.tw[k];
+    const long long L0 = (long long)blockIdx.x * kTL;                                    // first line (x) / first j (strided)
+    const long long base = STRIDED ? (long long)blockIdx.y * N * a.S + L0 : L0 * N;
+    // ---- load (bit-reversed positions)
+    for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
+        int l, k;
+        long long g;
+        if (STRIDED) { l = idx % kTL; k = idx / kTL; g = base + (long long)k * a.S + l; }
+        else { l = idx / N; k = idx % N; g = base + (long long)l * N + k; }
+        float2 v = make_float2(0.f, 0.f);
+        if (STRIDED || L0 + l < a.nlines) v = (mode == kModeInReal) ? make_float2(a.in_real[g], 0.f) : a.z[g];
+        buf[l * LD + brev<N>(k)] = v;
+    }
+    __syncthreads();
+    fft_tile<N>(buf, tws, a.inverse != 0);
+    if (mode == kModeStoreSpectrum || mode == kModeDual) {
+        // the last forward axis: every coordinate is a frequency now (PAPER.md:49 line 1 in the Fourier domain, W = I)
+        for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
+            const int l = idx % kTL, k = idx / kTL;
+            const long long g = base + (long long)k * a.S + l;
+            const float2 z = buf[l * LD + k];
+            if (mode == kModeStoreSpectrum) { a.phihat[g] = z; continue; }
+            const float d = a.D[g - (long long)blockIdx.y * N * a.S];
+            const float2 f = a.phihat[g];
+            float2 p = a.phat[g];
+            p.x = (p.x + a.sigma * (d * z.x - f.x)) * a.inv1ps;
+            p.y = (p.y + a.sigma * (d * z.y - f.y)) * a.inv1ps;
+            a.phat[g] = p;
+            buf[l * LD + k] = make_float2(d * p.x, d * p.y);                             // spectrum of K p (unnormalised)
+        }
+        if (mode == kModeStoreSpectrum) return;
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {                    // natural -> bit-reversed, in place
+            const int l = idx % kTL, k = idx / kTL, r = brev<N>(k);
+            if (k < r) { const float2 t = buf[l * LD + k]; buf[l * LD + k] = buf[l * LD + r]; buf[l * LD + r] = t; }
+        }
+        __syncthreads();
+        fft_tile<N>(buf, tws, true);
+    }
+    // ---- store
+    for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
+        int l, k;
+        long long g;
+        if (STRIDED) { l = idx % kTL; k = idx / kTL; g = base + (long long)k * a.S + l; }
+        else { l = idx / N; k = idx % N; g = base + (long long)l * N + k; }
+        if (!STRIDED && L0 + l >= a.nlines) continue;
+        const float2 v = buf[l * LD + k];
+        if (mode == kModeOutReal) a.out_real[g] = v.x * a.out_scale; else a.z[g] = v;
+    }
+}
+
+struct VoxArgs {
+    int nx, ny, nz;
+    long long nvox;           // nvol * nz * ny * nx
+    const float *mask;        // or NULL (ones)
+    float *chi, *chibar, *qx, *qy, *qz;
+    const float *kp;
+    float sigma, tau, theta, alpha;
+};
+
+// q <- proj_alpha(q + sigma M G chi_bar): forward differences, Neumann, pointwise Euclidean norm over the three components
+// (PAPER.md:49 line 2; R4, R7, R13 carried to 3-D by R23)
+__global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
+    const long long sy = a.nx, sz = (long long)a.nx * a.ny;
+    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < a.nvox; i += (long long)gridDim.x * kThreads) {
+        const int x = (int)(i % a.nx), y = (int)((i / a.nx) % a.ny), z = (int)((i / sz) % a.nz);
+        const float c = a.chibar[i], m = a.mask ? a.mask[i] : 1.f;
+        const float gx = x + 1 < a.nx ? a.chibar[i + 1] - c : 0.f;
+        const float gy = y + 1 < a.ny ? a.chibar[i + sy] - c : 0.f;
+        const float gz = z + 1 < a.nz ? a.chibar[i + sz] - c : 0.f;
+        const float tx = a.qx[i] + a.sigma * m * gx, ty = a.qy[i] + a.sigma * m * gy, tz = a.qz[i] + a.sigma * m * gz;
+        const float nrm = sqrtf(tx * tx + ty * ty + tz * tz);
+        const float s = nrm > a.alpha ? a.alpha / nrm : 1.f;
+        a.qx[i] = tx * s; a.qy[i] = ty * s; a.qz[i] = tz * s;
+    }
+}
+
+// chi+ = chi - tau (K p + G^T (M q)) ; chi_bar = chi+ + theta (chi+ - chi)   (PAPER.md:49 lines 3, 4)
+__global__ void __launch_bounds__(kThreads) chi_update3_kernel(const VoxArgs a) {
+    const long long sy = a.nx, sz = (long long)a.nx * a.ny;
+    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < a.nvox; i += (long long)gridDim.x * kThreads) {
+        const int x = (int)(i % a.nx), y = (int)((i / a.nx) % a.ny), z = (int)((i / sz) % a.nz);
+        const float m = a.mask ? a.mask[i] : 1.f;
+        float div = 0.f;
+        if (x >= 1) div += (a.mask ? a.mask[i - 1] : 1.f) * a.qx[i - 1];
+        if (x + 1 < a.nx) div -= m * a.qx[i];
+        if (y >= 1) div += (a.mask ? a.mask[i - sy] : 1.f) * a.qy[i - sy];
+        if (y + 1 < a.ny) div -= m * a.qy[i];
+        if (z >= 1) div += (a.mask ? a.mask[i - sz] : 1.f) * a.qz[i - sz];
+        if (z + 1 < a.nz) div -= m * a.qz[i];
+        const float c = a.chi[i], n = c - a.tau * (a.kp[i] + div);
+        a.chi[i] = n;
+        a.chibar[i] = n + a.theta * (n - c);
+    }
+}
+
+bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1)) == 0; }
+
+template <bool STRIDED>
+void launch_fft(int n, dim3 grid, const FftArgs &a, int mode, cudaStream_t st) {
+    switch (n) {
+        case 8: fft_lines_kernel<8, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
+        case 16: fft_lines_kernel<16, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
+        case 32: fft_lines_kernel<32, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
+        case 64: fft_lines_kernel<64, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
+        case 128: fft_lines_kernel<128, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
+        default: fft_lines_kernel<256, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
+    }
+}
+
+}  // namespace
+
+struct pd_plan3d_s {
+    int nx, ny, nz, nvol, b0_axis, num_sms;
+    float lambda, sigma, tau, theta;
+    float *D, *chibar, *kp, *q;     // q: three volumes
+    float2 *tw[3], *z, *phihat, *phat;
+    int last_launches;
+};
+
+extern "C" {
+
+int pd_destroy3d(pd_plan3d_t p) {
+    if (!p) return PD_EINVAL;
+    void *ptrs[] = {p->D, p->chibar, p->kp, p->q, p->tw[0], p->tw[1], p->tw[2], p->z, p->phihat, p->phat};
+    for (void *q : ptrs)
+        if (q) cudaFree(q);
+    delete p;
+    return PD_OK;
+}
+
+int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, float lambda, float sigma, float tau, float theta) {
+    if (!out) return PD_EINVAL;
+    *out = nullptr;
+    if (nvol < 1 || B0_axis < 0 || B0_axis > 2) return PD_EINVAL;
+    if (!pow2_in(nx, 16, 256) || !pow2_in(ny, 8, 256) || !pow2_in(nz, 8, 256)) return PD_ESIZE;
+    if (!(lambda >= 0.f) || !(theta >= 0.f && theta <= 1.f) || std::isnan(sigma) || std::isnan(tau)) return PD_EINVAL;
+    const double bound = 4.0 / 9.0 + 12.0;   // ||K||^2 <= 4/9, ||G||^2 <= 12 in three dimensions (tau = sigma = 1/L)
+    if (!(sigma > 0.f) || !(tau > 0.f)) sigma = tau = (float)(1.0 / std::sqrt(bound));
+    else if ((double)sigma * (double)tau * bound >= 1.0) return PD_ESTEP;
+    pd_plan3d_s *p = new (std::nothrow) pd_plan3d_s;
+    if (!p) return PD_ENOMEM;
+    std::memset(p, 0, sizeof(*p));
+    p->nx = nx; p->ny = ny; p->nz = nz; p->nvol = nvol; p->b0_axis = B0_axis;
+    p->lambda = lambda; p->sigma = sigma; p->tau = tau; p->theta = theta;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) { delete p; return pd_cuda_fail_((int)e, "cudaGetDevice"); }
+    const size_t V = (size_t)nx * ny * nz, T = V * (size_t)nvol;
+    const int dims[3] = {nx, ny, nz};
+    auto alloc = [&](void **ptr, size_t bytes) {
+        if (e != cudaSuccess) return;
+        e = cudaMalloc(ptr, bytes);
+    };
+    alloc((void **)&p->D, V * sizeof(float));
+    alloc((void **)&p->chibar, T * sizeof(float));
+    alloc((void **)&p->kp, T * sizeof(float));
+    alloc((void **)&p->q, 3 * T * sizeof(float));
+    alloc((void **)&p->z, T * sizeof(float2));
+    alloc((void **)&p->phihat, T * sizeof(float2));
+    alloc((void **)&p->phat, T * sizeof(float2));
+    for (int k = 0; k < 3; ++k) alloc((void **)&p->tw[k], (size_t)(dims[k] / 2) * sizeof(float2));
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); pd_destroy3d(p); return PD_ENOMEM; }
+    if (e != cudaSuccess) { pd_destroy3d(p); return pd_cuda_fail_((int)e, "cudaMalloc"); }
+    {   // tables in double on the host (R17): D3 = 1/3 - k_b^2/|k|^2, D3(0) = 0, k = (fi/nx, fj/ny, fk/nz) signed (R23)
+        std::vector<float> D(V);
+        for (int kz = 0; kz < nz; ++kz) {
+            const double fz = (double)(kz < (nz + 1) / 2 ? kz : kz - nz) / nz;
+            for (int ky = 0; ky < ny; ++ky) {
+                const double fy = (double)(ky < (ny + 1) / 2 ? ky : ky - ny) / ny;
+                for (int kx = 0; kx < nx; ++kx) {
+                    const double fx = (double)(kx < (nx + 1) / 2 ? kx : kx - nx) / nx;
+                    const double k2 = fx * fx + fy * fy + fz * fz, kb = B0_axis == 0 ? fx : B0_axis == 1 ? fy : fz;
+                    D[((size_t)kz * ny + ky) * nx + kx] = (float)(k2 == 0.0 ? 0.0 : 1.0 / 3.0 - kb * kb / k2);
+                }
+            }
+        }
+        e = cudaMemcpy(p->D, D.data(), V * sizeof(float), cudaMemcpyHostToDevice);
+        const double pi = 3.14159265358979323846264338327950288;
+        for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
+            std::vector<float2> tw(dims[k] / 2);
+            for (int j = 0; j < dims[k] / 2; ++j) {
+                const double ang = -2.0 * pi * (double)j / (double)dims[k];
+                tw[j] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+            }
+            e = cudaMemcpy(p->tw[k], tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice);
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(nullptr);
+        if (e != cudaSuccess) { pd_destroy3d(p); return pd_cuda_fail_((int)e, "3-D plan table upload"); }
+    }
+    *out = p;
+    return PD_OK;
+}
+
+int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_out, int max_iters, void *cuda_stream) {
+    if (!p || !field || !chi_out || max_iters < 0) return PD_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int nx = p->nx, ny = p->ny, nz = p->nz, nvol = p->nvol;
+    const long long V = (long long)nx * ny * nz, T = V * nvol;
+    cudaError_t e = cudaMemsetAsync(p->phat, 0, T * sizeof(float2), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(p->q, 0, 3 * T * sizeof(float), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(p->chibar, 0, T * sizeof(float), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(chi_out, 0, T * sizeof(float), st);
+    if (e != cudaSuccess) return pd_cuda_fail_((int)e, "cudaMemsetAsync (3-D state)");
+
+    FftArgs f;
+    std::memset(&f, 0, sizeof(f));
+    f.z = p->z; f.phihat = p->phihat; f.phat = p->phat; f.D = p->D;
+    f.sigma = p->sigma; f.inv1ps = 1.0f / (1.0f + p->sigma); f.out_scale = (float)(1.0 / (double)V);
+    const long long xlines = (long long)nvol * nz * ny;
+    const dim3 gx((unsigned)((xlines + kTL - 1) / kTL)), gy((unsigned)(nx / kTL), (unsigned)(nvol * nz)),
+        gz((unsigned)((long long)nx * ny / kTL), (unsigned)nvol);
+    int launches = 0;
+    auto pass_x = [&](const float *in_real, float *out_real, bool inverse) {
+        FftArgs a = f;
+        a.tw = p->tw[0]; a.nlines = xlines; a.inverse = inverse ? 1 : 0; a.in_real = in_real; a.out_real = out_real;
+        launch_fft<false>(nx, gx, a, in_real ? kModeInReal : out_real ? kModeOutReal : kModePlain, st);
+        ++launches;
+    };
+    auto pass_y = [&](bool inverse) {
+        FftArgs a = f;
+        a.tw = p->tw[1]; a.S = nx; a.inverse = inverse ? 1 : 0;
+        launch_fft<true>(ny, gy, a, kModePlain, st);
+        ++launches;
+    };
+    auto pass_z = [&](int mode) {
+        FftArgs a = f;
+        a.tw = p->tw[2]; a.S = (long long)nx * ny; a.inverse = 0;
+        launch_fft<true>(nz, gz, a, mode, st);
+        ++launches;
+    };
+    // phi^ = F phi, once (everything else starts at zero)
+    pass_x(field, nullptr, false);
+    pass_y(false);
+    pass_z(kModeStoreSpectrum);
+
+    VoxArgs v;
+    std::memset(&v, 0, sizeof(v));
+    v.nx = nx; v.ny = ny; v.nz = nz; v.nvox = T; v.mask = mask;
+    v.chi = chi_out; v.chibar = p->chibar; v.qx = p->q; v.qy = p->q + T; v.qz = p->q + 2 * T; v.kp = p->kp;
+    v.sigma = p->sigma; v.tau = p->tau; v.theta = p->theta; v.alpha = p->lambda;
+    const long long need = (T + kThreads - 1) / kThreads, cap = (long long)p->num_sms * 8;
+    const int vgrid = (int)(need < cap ? need : cap);
+    for (int n = 0; n < max_iters; ++n) {
+        pass_x(p->chibar, nullptr, false);     // F chi_bar
+        pass_y(false);
+        pass_z(kModeDual);                     // p-update in the Fourier domain, spectrum of K p, z lines back
+        pass_y(true);
+        pass_x(nullptr, p->kp, true);          // K p
+        q_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
+        chi_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
+        launches += 2;
+    }
+    p->last_launches = launches;
+    e = cudaGetLastError();
+    return e == cudaSuccess ? PD_OK : pd_cuda_fail_((int)e, "pd_solve3d launch");
+}
+
+int pd_last_launch_count3d(pd_plan3d_t p) { return p ? p->last_launches : PD_EINVAL; }
+
+}  // extern "C"

@@ -297,3 +297,41 @@ def echo_pair(cid, nslices=None, first_slice=0, phase_span=2.5, noise=0.01):
         s0[b] = (A * np.exp(1j * theta0) + noise * (g[0] + 1j * g[1])).astype(np.complex64)
         s1[b] = (A * np.exp(1j * (theta0 + pscale * f[b])) + noise * (g[2] + 1j * g[3])).astype(np.complex64)
     return {"cfg": cfg, "s0": s0, "s1": s1, "fscale": 1.0 / pscale, "field": d["field"], "mask": m}
+
+
+_VOL = 7
+
+
+def volume_case(nx, ny, nz, nvol=1, seed=0, b0_axis=2, noise=0.01):
+    """Inputs of the true 3-D variant (NEXT-2): per volume a phantom of a few ellipsoids (susceptibility sources) and a
+    thin needle along a random direction in a zero background, the field it induces through the 3-D dipole kernel
+    (numpy.fft, float64: the measurement is simulated, nothing is solved), Gaussian noise of `noise` x max|field|, and an
+    ellipsoidal mask.  Returns dict(field, mask: float32 [nvol][nz][ny][nx], chi_true float64)."""
+    zz, yy, xx = np.mgrid[0:nz, 0:ny, 0:nx]
+    kz, ky, kx = np.meshgrid(np.fft.fftfreq(nz), np.fft.fftfreq(ny), np.fft.fftfreq(nx), indexing="ij")
+    k2 = kx * kx + ky * ky + kz * kz
+    kb = (kx, ky, kz)[b0_axis]
+    D = 1.0 / 3.0 - kb * kb / np.where(k2 == 0, 1.0, k2)
+    D[0, 0, 0] = 0.0
+    field = np.empty((nvol, nz, ny, nx), np.float32)
+    mask = np.empty((nvol, nz, ny, nx), np.float32)
+    truth = np.empty((nvol, nz, ny, nx), np.float64)
+    for v in range(nvol):
+        u = uniform01(stream_key(900 + seed, v, 0, _VOL), 64)
+        chi = np.zeros((nz, ny, nx))
+        for e in range(3):
+            c = (nx * (0.3 + 0.4 * u[6 * e]), ny * (0.3 + 0.4 * u[6 * e + 1]), nz * (0.3 + 0.4 * u[6 * e + 2]))
+            r = [max(1.0, 0.08 * n * (0.5 + u[6 * e + 3 + a])) for a, n in enumerate((nx, ny, nz))]
+            chi[((xx - c[0]) / r[0]) ** 2 + ((yy - c[1]) / r[1]) ** 2 + ((zz - c[2]) / r[2]) ** 2 <= 1.0] += 1.0 + u[40 + e]
+        d = np.array([u[50] - 0.5, u[51] - 0.5, u[52] - 0.5])
+        d /= max(np.linalg.norm(d), 1e-6)
+        rel = np.stack([xx - nx / 2.0, yy - ny / 2.0, zz - nz / 2.0])
+        along = (rel * d[:, None, None, None]).sum(0)
+        perp2 = (rel ** 2).sum(0) - along ** 2
+        chi[(perp2 <= 1.5) & (np.abs(along) <= 0.3 * min(nx, ny, nz))] += 5.0
+        phi = np.real(np.fft.ifftn(D * np.fft.fftn(chi)))
+        g = normal01(stream_key(900 + seed, v, 1, _VOL), nx * ny * nz).reshape(nz, ny, nx)
+        field[v] = (phi + noise * np.abs(phi).max() * g).astype(np.float32)
+        mask[v] = (((xx - nx / 2.0) / (0.46 * nx)) ** 2 + ((yy - ny / 2.0) / (0.46 * ny)) ** 2 + ((zz - nz / 2.0) / (0.48 * nz)) ** 2 <= 1.0)
+        truth[v] = chi
+    return {"field": field, "mask": mask, "chi_true": truth}

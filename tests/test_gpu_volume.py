@@ -1,0 +1,108 @@
+"""GPU-vs-oracle parity of the true 3-D variant (NEXT-2) through the C ABI: pd_plan3d / pd_solve3d against
+oracle/pd3_oracle.py (numpy float64, the paper's iteration literally).  Gates as for the 2-D path (north_star): per-volume
+relative L2 of chi <= 1e-5 after one iteration, <= 1e-3 after the full count."""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+from paper_2006_09808_b200 import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def pd(torch):
+    from paper_2006_09808_b200 import binding
+    binding.lib()   # fails loudly if the extension is missing: there is no fallback
+    return binding
+
+
+@pytest.fixture(scope="module")
+def o3():
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import pd3_oracle
+    return pd3_oracle
+
+
+def vol_rel(a, b):
+    a = a.reshape(a.shape[0], -1).astype(np.float64)
+    b = b.reshape(b.shape[0], -1).astype(np.float64)
+    return np.linalg.norm(a - b, axis=1) / np.maximum(np.linalg.norm(b, axis=1), 1e-300)
+
+
+def gpu_solve3(torch, pd, field, mask, iters, *, lam, b0, sigma=0.25, tau=0.25, theta=1.0):
+    nvol, nz, ny, nx = field.shape
+    plan = pd.Plan3D(nx, ny, nz, nvol, b0, lam, sigma, tau, theta)
+    f = torch.from_numpy(field).cuda()
+    m = None if mask is None else torch.from_numpy(mask).cuda()
+    out = torch.full_like(f, float("nan"))
+    plan.solve(f, m, out, iters)
+    torch.cuda.synchronize()
+    n = plan.last_launch_count
+    plan.destroy()
+    return out.cpu().numpy(), n
+
+
+@pytest.mark.parametrize("nx,ny,nz,b0", [(16, 8, 8, 2), (64, 32, 16, 0), (32, 128, 64, 1), (256, 16, 8, 2), (128, 256, 32, 2)])
+def test_one_iteration_all_axes(torch, pd, o3, nx, ny, nz, b0):
+    rng = np.random.default_rng(nx + ny + nz)
+    f = rng.normal(size=(2, nz, ny, nx)).astype(np.float32)          # unstructured: every frequency is exercised
+    m = (rng.uniform(size=f.shape) > 0.3).astype(np.float32)
+    g, launches = gpu_solve3(torch, pd, f, m, 1, lam=0.05, b0=b0)
+    o = o3.solve3(f, m, lambda_=0.05, sigma=0.25, tau=0.25, max_iters=1, b0_dir=b0)
+    assert vol_rel(g, o).max() < 1e-5
+    assert launches == 3 + 7
+
+
+@pytest.mark.parametrize("iters,theta,masked", [(2, 1.0, True), (3, 0.5, True), (25, 1.0, True), (25, 1.0, False)])
+def test_iterations_exercise_q_and_divergence(torch, pd, o3, iters, theta, masked):
+    case = synth.volume_case(64, 32, 16, nvol=3, seed=iters, b0_axis=2)
+    lam = 0.02 * float(np.abs(case["field"]).max())                  # the ball is active on part of the volume
+    m = case["mask"] if masked else None
+    g, _ = gpu_solve3(torch, pd, case["field"], m, iters, lam=lam, b0=2, theta=theta)
+    o = o3.solve3(case["field"], m, lambda_=lam, sigma=0.25, tau=0.25, theta=theta, max_iters=iters, b0_dir=2)
+    assert vol_rel(g, o).max() < (1e-5 if iters <= 3 else 1e-3)
+    assert vol_rel(g, o).max() < 2e-5                                  # what fp32 actually achieves
+    assert np.abs(g.reshape(3, -1).mean(1)).max() < 1e-5 * np.abs(g).max()   # D3(0) = 0 and sum(G^T v) = 0: zero mean
+
+
+def test_automatic_steps_alpha_zero_and_max_iters_zero(torch, pd, o3):
+    case = synth.volume_case(32, 16, 8, nvol=1, seed=3, b0_axis=0)
+    s = 1.0 / np.sqrt(4.0 / 9.0 + 12.0)
+    g, _ = gpu_solve3(torch, pd, case["field"], case["mask"], 6, lam=0.0, b0=0, sigma=0.0, tau=0.0)   # alpha = 0: q = 0 (R13)
+    o = o3.solve3(case["field"], case["mask"], lambda_=0.0, sigma=s, tau=s, max_iters=6, b0_dir=0)
+    assert vol_rel(g, o).max() < 1e-5
+    g, n = gpu_solve3(torch, pd, case["field"], None, 0, lam=0.1, b0=0)
+    assert not g.any() and n == 3
+
+
+def test_full_size_volume(torch, pd, o3):
+    """The size bench.py --volume times per coil: 256 x 256 x 64, 10 iterations against the oracle."""
+    case = synth.volume_case(256, 256, 64, nvol=1, seed=9, b0_axis=2)
+    lam = 0.02 * float(np.abs(case["field"]).max())
+    g, _ = gpu_solve3(torch, pd, case["field"], case["mask"], 10, lam=lam, b0=2)
+    o = o3.solve3(case["field"], case["mask"], lambda_=lam, sigma=0.25, tau=0.25, max_iters=10, b0_dir=2)
+    assert vol_rel(g, o).max() < 2e-5
+
+
+def test_plan3d_errors(pd):
+    import ctypes as C
+    L, h = pd.lib(), C.c_void_p()
+    assert L.pd_plan3d(C.byref(h), 8, 16, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE       # nx < 16
+    assert L.pd_plan3d(C.byref(h), 64, 48, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE      # not a power of two
+    assert L.pd_plan3d(C.byref(h), 512, 16, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE
+    assert L.pd_plan3d(C.byref(h), 64, 16, 16, 1, 3, 0.01, 0.25, 0.25, 1.0) == pd.EINVAL     # B0 axis
+    assert L.pd_plan3d(C.byref(h), 64, 16, 16, 0, 2, 0.01, 0.25, 0.25, 1.0) == pd.EINVAL
+    assert L.pd_plan3d(C.byref(h), 64, 16, 16, 1, 2, 0.01, 0.3, 0.3, 1.0) == pd.ESTEP        # 0.09 * 12.44 > 1
+    assert h.value is None
+    assert L.pd_solve3d(None, None, None, None, 1, None) == pd.EINVAL and L.pd_destroy3d(None) == pd.EINVAL

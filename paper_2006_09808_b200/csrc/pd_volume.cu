@@ -9,6 +9,7 @@
 // Line transforms: radix-2 in shared memory, 16 lines per CTA; strided axes (y, z) are read as tiles of 16 adjacent x so
 // that every access is a full 128-byte line.  Twiddles and D come from double-precision host tables (R17).  No cuFFT.
 #include "../../include/pd.h"
+#include "fft_regs.cuh"
 
 #include <cuda_runtime.h>
 
@@ -32,7 +33,7 @@ struct FftArgs {
     float *out_real;          // kModeOutReal
     float2 *phihat, *phat;    // kModeStoreSpectrum / kModeDual
     const float *D;           // [nz][ny][nx], unscaled
-    const float2 *tw;         // exp(-2 pi i k / N), k < N/2
+    const float2 *tw;         // exp(-2 pi i k / N), k < N
     long long nlines;         // x pass: number of lines
     long long S;              // strided pass: distance between consecutive points of a line (nx, or nx*ny)
     float sigma, inv1ps, out_scale;
@@ -124,8 +125,84 @@ __global__ void __launch_bounds__(kThreads) fft_lines_kernel(const FftArgs a, co
     }
 }
 
+// Lines of 64, 128 or 256 points: the register transform of fft_regs.cuh (T threads per line hold E points each, one
+// exchange through shared memory, packed FFMA2 butterflies); input and output share the thread map k = j + T m, so the
+// forward transform, the p-update and the inverse transform of the z pass chain in registers.  Same tiles as above.
+template <int N, bool STRIDED, int mode>
+__global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 512 : 768) / (kTL * pdk::FftCfg<N>::T)) fft_lines_reg_kernel(const FftArgs a) {
+    using Cfg = pdk::FftCfg<N>;
+    constexpr int E = Cfg::E, T = Cfg::T, LD = T + 1, NT = kTL * T;
+    // exchange region of one line: E rows of LD, plus one entry so that the regions of the 16 lines of a tile start in
+    // different banks (E*LD float2 is a multiple of 32 words: sixteen lines on one bank, a 16-way conflict, measured)
+    constexpr int REG = E * LD + 1;
+    __shared__ float2 tws[E * T];
+    __shared__ float2 ex[kTL * REG];
+    pdk::TwiddlesSmem<N>::fill(tws, a.tw, threadIdx.x, NT);
+    const int l = STRIDED ? threadIdx.x % kTL : threadIdx.x / T;     // line of the tile
+    const int j = STRIDED ? threadIdx.x / kTL : threadIdx.x % T;     // thread of the line
+    pdk::TwiddlesSmem<N> tw;
+    tw.w = tws + j;
+    float2 *sm = ex + l * REG;
+    const long long L0 = (long long)blockIdx.x * kTL;
+    const long long vol = STRIDED ? (long long)blockIdx.y * N * a.S : 0;                 // first point of my (outer) block
+    const long long base = STRIDED ? vol + L0 + l : (L0 + l) * N;                        // first point of my line
+    const int step = STRIDED ? (int)a.S : 1;                                             // distance between its points
+    const bool live = STRIDED || L0 + l < a.nlines;
+    float2 *const zl = a.z + base;
+    float2 v[E];
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int o = (j + T * m) * step;
+        v[m] = !live ? make_float2(0.f, 0.f) : (mode == kModeInReal) ? make_float2(__ldg(a.in_real + base + o), 0.f) : zl[o];
+    }
+    __syncthreads();   // twiddle table filled
+    auto transform = [&](bool inverse) {   // the inverse is the forward transform of the swapped halves (fft_regs.cuh)
+        if (inverse) {
+#pragma unroll
+            for (int m = 0; m < E; ++m) v[m] = make_float2(v[m].y, v[m].x);
+        }
+        if (STRIDED) pdk::fft_line<N, LD>(v, sm, j, tw, pdk::BlockSync());
+        else pdk::fft_line<N, LD>(v, sm, j, tw, pdk::WarpSync());
+        if (inverse) {
+#pragma unroll
+            for (int m = 0; m < E; ++m) v[m] = make_float2(v[m].y, v[m].x);
+        }
+    };
+    transform(a.inverse != 0);
+    if (mode == kModeStoreSpectrum) {
+        float2 *const fl = a.phihat + base;
+#pragma unroll
+        for (int m = 0; m < E; ++m) fl[(j + T * m) * step] = v[m];
+        return;
+    }
+    if (mode == kModeDual) {   // PAPER.md:49 line 1 in the Fourier domain (W = I), then the spectrum of K p
+        const float2 *const fl = a.phihat + base;
+        float2 *const pl = a.phat + base;
+        const float *const dl = a.D + (base - vol);
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const int o = (j + T * m) * step;
+            const float d = __ldg(dl + o);
+            const float2 f = fl[o];
+            float2 p = pl[o];
+            p.x = (p.x + a.sigma * (d * v[m].x - f.x)) * a.inv1ps;
+            p.y = (p.y + a.sigma * (d * v[m].y - f.y)) * a.inv1ps;
+            pl[o] = p;
+            v[m] = make_float2(d * p.x, d * p.y);
+        }
+        transform(true);
+    }
+    if (!live) return;
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int o = (j + T * m) * step;
+        if (mode == kModeOutReal) a.out_real[base + o] = v[m].x * a.out_scale; else zl[o] = v[m];
+    }
+}
+
 struct VoxArgs {
-    int nx, ny, nz;
+    int nx, ny, nz;           // powers of two; nx a multiple of 4
+    int lx, ly;               // log2 nx, log2 ny
     long long nvox;           // nvol * nz * ny * nx
     const float *mask;        // or NULL (ones)
     float *chi, *chibar, *qx, *qy, *qz;
@@ -133,43 +210,80 @@ struct VoxArgs {
     float sigma, tau, theta, alpha;
 };
 
+__device__ __forceinline__ float4 ld4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+__device__ __forceinline__ void st4(float *p, float4 v) { *reinterpret_cast<float4 *>(p) = v; }
+__device__ __forceinline__ float4 sub4(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
+
 // q <- proj_alpha(q + sigma M G chi_bar): forward differences, Neumann, pointwise Euclidean norm over the three components
-// (PAPER.md:49 line 2; R4, R7, R13 carried to 3-D by R23)
+// (PAPER.md:49 line 2; R4, R7, R13 carried to 3-D by R23).  Four voxels along x per thread and trip.
 __global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
-    const long long sy = a.nx, sz = (long long)a.nx * a.ny;
-    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < a.nvox; i += (long long)gridDim.x * kThreads) {
-        const int x = (int)(i % a.nx), y = (int)((i / a.nx) % a.ny), z = (int)((i / sz) % a.nz);
-        const float c = a.chibar[i], m = a.mask ? a.mask[i] : 1.f;
-        const float gx = x + 1 < a.nx ? a.chibar[i + 1] - c : 0.f;
-        const float gy = y + 1 < a.ny ? a.chibar[i + sy] - c : 0.f;
-        const float gz = z + 1 < a.nz ? a.chibar[i + sz] - c : 0.f;
-        const float tx = a.qx[i] + a.sigma * m * gx, ty = a.qy[i] + a.sigma * m * gy, tz = a.qz[i] + a.sigma * m * gz;
-        const float nrm = sqrtf(tx * tx + ty * ty + tz * tz);
-        const float s = nrm > a.alpha ? a.alpha / nrm : 1.f;
-        a.qx[i] = tx * s; a.qy[i] = ty * s; a.qz[i] = tz * s;
+    const long long sy = a.nx, sz = (long long)a.nx << a.ly, nquad = a.nvox >> 2;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f), one = make_float4(1.f, 1.f, 1.f, 1.f);
+    for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < nquad; i4 += (long long)gridDim.x * kThreads) {
+        const long long i = i4 << 2;
+        const int x = (int)(i & (a.nx - 1)), y = (int)((i >> a.lx) & (a.ny - 1)), z = (int)((i >> (a.lx + a.ly)) & (a.nz - 1));
+        const float4 c = ld4(a.chibar + i), m = a.mask ? ld4(a.mask + i) : one;
+        const float cn = x + 4 < a.nx ? a.chibar[i + 4] : c.w;                         // Neumann: last x difference is 0
+        const float4 gx = make_float4(c.y - c.x, c.z - c.y, c.w - c.z, cn - c.w);
+        const float4 gy = y + 1 < a.ny ? sub4(ld4(a.chibar + i + sy), c) : zero;
+        const float4 gz = z + 1 < a.nz ? sub4(ld4(a.chibar + i + sz), c) : zero;
+        float4 qx = ld4(a.qx + i), qy = ld4(a.qy + i), qz = ld4(a.qz + i);
+        auto one_voxel = [&](float &px, float &py, float &pz, float mm, float dx, float dy, float dz) {
+            const float tx = px + a.sigma * mm * dx, ty = py + a.sigma * mm * dy, tz = pz + a.sigma * mm * dz;
+            const float nrm = sqrtf(tx * tx + ty * ty + tz * tz);
+            const float s = nrm > a.alpha ? a.alpha / nrm : 1.f;
+            px = tx * s; py = ty * s; pz = tz * s;
+        };
+        one_voxel(qx.x, qy.x, qz.x, m.x, gx.x, gy.x, gz.x);
+        one_voxel(qx.y, qy.y, qz.y, m.y, gx.y, gy.y, gz.y);
+        one_voxel(qx.z, qy.z, qz.z, m.z, gx.z, gy.z, gz.z);
+        one_voxel(qx.w, qy.w, qz.w, m.w, gx.w, gy.w, gz.w);
+        st4(a.qx + i, qx); st4(a.qy + i, qy); st4(a.qz + i, qz);
     }
 }
 
 // chi+ = chi - tau (K p + G^T (M q)) ; chi_bar = chi+ + theta (chi+ - chi)   (PAPER.md:49 lines 3, 4)
+// G^T v at a voxel = v_x(x-1) [x >= 1] - v_x(x) [x <= nx-2] + the same along y and z, v = M q.
 __global__ void __launch_bounds__(kThreads) chi_update3_kernel(const VoxArgs a) {
-    const long long sy = a.nx, sz = (long long)a.nx * a.ny;
-    for (long long i = (long long)blockIdx.x * kThreads + threadIdx.x; i < a.nvox; i += (long long)gridDim.x * kThreads) {
-        const int x = (int)(i % a.nx), y = (int)((i / a.nx) % a.ny), z = (int)((i / sz) % a.nz);
-        const float m = a.mask ? a.mask[i] : 1.f;
-        float div = 0.f;
-        if (x >= 1) div += (a.mask ? a.mask[i - 1] : 1.f) * a.qx[i - 1];
-        if (x + 1 < a.nx) div -= m * a.qx[i];
-        if (y >= 1) div += (a.mask ? a.mask[i - sy] : 1.f) * a.qy[i - sy];
-        if (y + 1 < a.ny) div -= m * a.qy[i];
-        if (z >= 1) div += (a.mask ? a.mask[i - sz] : 1.f) * a.qz[i - sz];
-        if (z + 1 < a.nz) div -= m * a.qz[i];
-        const float c = a.chi[i], n = c - a.tau * (a.kp[i] + div);
-        a.chi[i] = n;
-        a.chibar[i] = n + a.theta * (n - c);
+    const long long sy = a.nx, sz = (long long)a.nx << a.ly, nquad = a.nvox >> 2;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f), one = make_float4(1.f, 1.f, 1.f, 1.f);
+    auto mul4 = [](float4 u, float4 w) { return make_float4(u.x * w.x, u.y * w.y, u.z * w.z, u.w * w.w); };
+    for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < nquad; i4 += (long long)gridDim.x * kThreads) {
+        const long long i = i4 << 2;
+        const int x = (int)(i & (a.nx - 1)), y = (int)((i >> a.lx) & (a.ny - 1)), z = (int)((i >> (a.lx + a.ly)) & (a.nz - 1));
+        const float4 m = a.mask ? ld4(a.mask + i) : one;
+        float4 vx = mul4(m, ld4(a.qx + i));
+        const float4 vy = mul4(m, ld4(a.qy + i)), vz = mul4(m, ld4(a.qz + i));
+        const float vxl = x >= 1 ? (a.mask ? a.mask[i - 1] : 1.f) * a.qx[i - 1] : 0.f;
+        if (x + 4 == a.nx) vx.w = 0.f;                                                 // no difference leaves the last column
+        float4 div = make_float4(vxl - vx.x, vx.x - vx.y, vx.y - vx.z, vx.z - vx.w);
+        if (y >= 1) { const float4 t = mul4(a.mask ? ld4(a.mask + i - sy) : one, ld4(a.qy + i - sy)); div.x += t.x; div.y += t.y; div.z += t.z; div.w += t.w; }
+        if (y + 1 < a.ny) { div.x -= vy.x; div.y -= vy.y; div.z -= vy.z; div.w -= vy.w; }
+        if (z >= 1) { const float4 t = mul4(a.mask ? ld4(a.mask + i - sz) : one, ld4(a.qz + i - sz)); div.x += t.x; div.y += t.y; div.z += t.z; div.w += t.w; }
+        if (z + 1 < a.nz) { div.x -= vz.x; div.y -= vz.y; div.z -= vz.z; div.w -= vz.w; }
+        const float4 c = ld4(a.chi + i), k = ld4(a.kp + i);
+        const float4 n = make_float4(c.x - a.tau * (k.x + div.x), c.y - a.tau * (k.y + div.y), c.z - a.tau * (k.z + div.z), c.w - a.tau * (k.w + div.w));
+        st4(a.chi + i, n);
+        st4(a.chibar + i, make_float4(n.x + a.theta * (n.x - c.x), n.y + a.theta * (n.y - c.y), n.z + a.theta * (n.z - c.z), n.w + a.theta * (n.w - c.w)));
+        (void)zero;
     }
 }
 
 bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1)) == 0; }
+
+template <int N, bool STRIDED>
+void launch_reg(dim3 grid, const FftArgs &a, int mode, cudaStream_t st) {
+    constexpr int NT = kTL * pdk::FftCfg<N>::T;
+    if constexpr (STRIDED) {
+        if (mode == kModeDual) fft_lines_reg_kernel<N, STRIDED, kModeDual><<<grid, NT, 0, st>>>(a);
+        else if (mode == kModeStoreSpectrum) fft_lines_reg_kernel<N, STRIDED, kModeStoreSpectrum><<<grid, NT, 0, st>>>(a);
+        else fft_lines_reg_kernel<N, STRIDED, kModePlain><<<grid, NT, 0, st>>>(a);
+    } else {
+        if (mode == kModeInReal) fft_lines_reg_kernel<N, STRIDED, kModeInReal><<<grid, NT, 0, st>>>(a);
+        else if (mode == kModeOutReal) fft_lines_reg_kernel<N, STRIDED, kModeOutReal><<<grid, NT, 0, st>>>(a);
+        else fft_lines_reg_kernel<N, STRIDED, kModePlain><<<grid, NT, 0, st>>>(a);
+    }
+}
 
 template <bool STRIDED>
 void launch_fft(int n, dim3 grid, const FftArgs &a, int mode, cudaStream_t st) {
@@ -177,9 +291,9 @@ void launch_fft(int n, dim3 grid, const FftArgs &a, int mode, cudaStream_t st) {
         case 8: fft_lines_kernel<8, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
         case 16: fft_lines_kernel<16, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
         case 32: fft_lines_kernel<32, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
-        case 64: fft_lines_kernel<64, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
-        case 128: fft_lines_kernel<128, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
-        default: fft_lines_kernel<256, STRIDED><<<grid, kThreads, 0, st>>>(a, mode); break;
+        case 64: launch_reg<64, STRIDED>(grid, a, mode, st); break;
+        case 128: launch_reg<128, STRIDED>(grid, a, mode, st); break;
+        default: launch_reg<256, STRIDED>(grid, a, mode, st); break;
     }
 }
 
@@ -235,7 +349,7 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
     alloc((void **)&p->z, T * sizeof(float2));
     alloc((void **)&p->phihat, T * sizeof(float2));
     alloc((void **)&p->phat, T * sizeof(float2));
-    for (int k = 0; k < 3; ++k) alloc((void **)&p->tw[k], (size_t)(dims[k] / 2) * sizeof(float2));
+    for (int k = 0; k < 3; ++k) alloc((void **)&p->tw[k], (size_t)dims[k] * sizeof(float2));
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); pd_destroy3d(p); return PD_ENOMEM; }
     if (e != cudaSuccess) { pd_destroy3d(p); return pd_cuda_fail_((int)e, "cudaMalloc"); }
     {   // tables in double on the host (R17): D3 = 1/3 - k_b^2/|k|^2, D3(0) = 0, k = (fi/nx, fj/ny, fk/nz) signed (R23)
@@ -254,8 +368,8 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
         e = cudaMemcpy(p->D, D.data(), V * sizeof(float), cudaMemcpyHostToDevice);
         const double pi = 3.14159265358979323846264338327950288;
         for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
-            std::vector<float2> tw(dims[k] / 2);
-            for (int j = 0; j < dims[k] / 2; ++j) {
+            std::vector<float2> tw(dims[k]);
+            for (int j = 0; j < dims[k]; ++j) {
                 const double ang = -2.0 * pi * (double)j / (double)dims[k];
                 tw[j] = make_float2((float)std::cos(ang), (float)std::sin(ang));
             }
@@ -270,6 +384,7 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
 
 int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_out, int max_iters, void *cuda_stream) {
     if (!p || !field || !chi_out || max_iters < 0) return PD_EINVAL;
+    if (((unsigned long long)field | (unsigned long long)mask | (unsigned long long)chi_out) & 15ull) return PD_EINVAL;   // float4 accesses
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int nx = p->nx, ny = p->ny, nz = p->nz, nvol = p->nvol;
     const long long V = (long long)nx * ny * nz, T = V * nvol;
@@ -313,9 +428,11 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     VoxArgs v;
     std::memset(&v, 0, sizeof(v));
     v.nx = nx; v.ny = ny; v.nz = nz; v.nvox = T; v.mask = mask;
+    for (v.lx = 0; (1 << v.lx) < nx; ++v.lx) {}
+    for (v.ly = 0; (1 << v.ly) < ny; ++v.ly) {}
     v.chi = chi_out; v.chibar = p->chibar; v.qx = p->q; v.qy = p->q + T; v.qz = p->q + 2 * T; v.kp = p->kp;
     v.sigma = p->sigma; v.tau = p->tau; v.theta = p->theta; v.alpha = p->lambda;
-    const long long need = (T + kThreads - 1) / kThreads, cap = (long long)p->num_sms * 8;
+    const long long need = (T / 4 + kThreads - 1) / kThreads, cap = (long long)p->num_sms * 8;
     const int vgrid = (int)(need < cap ? need : cap);
     for (int n = 0; n < max_iters; ++n) {
         pass_x(p->chibar, nullptr, false);     // F chi_bar

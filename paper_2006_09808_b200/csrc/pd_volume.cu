@@ -168,6 +168,20 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
             for (int m = 0; m < E; ++m) v[m] = make_float2(v[m].y, v[m].x);
         }
     };
+    // z pass of the iteration: with 8 points per thread the operands of the p-update are requested BEFORE the forward
+    // transform, so that a CTA has one memory phase instead of two dependent ones (40 registers; not at 16 points)
+    constexpr bool PRE = (mode == kModeDual) && E <= 8;
+    float2 pf[PRE ? E : 1], pp[PRE ? E : 1];
+    float pd[PRE ? E : 1];
+    if (PRE) {
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const int o = (j + T * m) * step;
+            pd[m] = __ldg(a.D + (base - vol) + o);
+            pf[m] = a.phihat[base + o];
+            pp[m] = a.phat[base + o];
+        }
+    }
     transform(a.inverse != 0);
     if (mode == kModeStoreSpectrum) {
         float2 *const fl = a.phihat + base;
@@ -182,9 +196,9 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
 #pragma unroll
         for (int m = 0; m < E; ++m) {
             const int o = (j + T * m) * step;
-            const float d = __ldg(dl + o);
-            const float2 f = fl[o];
-            float2 p = pl[o];
+            const float d = PRE ? pd[m] : __ldg(dl + o);
+            const float2 f = PRE ? pf[m] : fl[o];
+            float2 p = PRE ? pp[m] : pl[o];
             p.x = (p.x + a.sigma * (d * v[m].x - f.x)) * a.inv1ps;
             p.y = (p.y + a.sigma * (d * v[m].y - f.y)) * a.inv1ps;
             pl[o] = p;

@@ -2,8 +2,9 @@
 // gradient operator in all three dimensions", with the 3-D dipole kernel, one problem per VOLUME
 // [nz][ny][nx] (slices are coupled: no per-slice stop, the iteration count is the caller's; R23, 5.7).
 //
-// A first, correct, streaming implementation (not yet tuned like the 2-D path): W = identity, so the dual p lives in the
-// Fourier domain as in DESIGN.md 5.0 -- ONE 3-D FFT round trip per iteration:
+// A streaming implementation: W = identity, so the dual p lives in the Fourier domain as in DESIGN.md 5.0 -- ONE 3-D FFT
+// round trip per iteration -- and two real volumes (coils) ride one complex transform, z = a + i b (D3 is real and even,
+// so F^-1 D3 F z = K a + i K b, and the p-update is linear: it acts on the packed spectrum as it stands):
 //   x lines (chi_bar real -> complex) ; y lines ; z lines + [ p^ <- (p^ + sigma (D Z - phi^))/(1+sigma) ; Z <- D p^ ] + z lines
 //   back ; y lines back ; x lines back (-> K p, real) ; q-update (3 components) ; chi-update with the 3-D divergence.
 // Line transforms: radix-2 in shared memory, 16 lines per CTA; strided axes (y, z) are read as tiles of 16 adjacent x so
@@ -34,7 +35,10 @@ struct FftArgs {
     float2 *phihat, *phat;    // kModeStoreSpectrum / kModeDual
     const float *D;           // [nz][ny][nx], unscaled
     const float2 *tw;         // exp(-2 pi i k / N), k < N
-    long long nlines;         // x pass: number of lines
+    long long nlines;         // x pass: number of lines (of the PAIRED volumes)
+    long long V;              // voxels of one volume
+    int lines_per_vol;        // nz * ny
+    int nvol;                 // real volumes: the pair pv holds volume 2 pv in its real part and 2 pv + 1 (if any) in its imaginary part
     long long S;              // strided pass: distance between consecutive points of a line (nx, or nx*ny)
     float sigma, inv1ps, out_scale;
     int inverse;
@@ -84,7 +88,14 @@ __global__ void __launch_bounds__(kThreads) fft_lines_kernel(const FftArgs a, co
         if (STRIDED) { l = idx % kTL; k = idx / kTL; g = base + (long long)k * a.S + l; }
         else { l = idx / N; k = idx % N; g = base + (long long)l * N + k; }
         float2 v = make_float2(0.f, 0.f);
-        if (STRIDED || L0 + l < a.nlines) v = (mode == kModeInReal) ? make_float2(a.in_real[g], 0.f) : a.z[g];
+        if (STRIDED || L0 + l < a.nlines) {
+            if (mode == kModeInReal) {
+                const long long pv = (L0 + l) / a.lines_per_vol, r = g + pv * a.V;       // volume 2 pv, same line and point
+                v = make_float2(a.in_real[r], 2 * pv + 1 < a.nvol ? a.in_real[r + a.V] : 0.f);
+            } else {
+                v = a.z[g];
+            }
+        }
         buf[l * LD + brev<N>(k)] = v;
     }
     __syncthreads();
@@ -121,7 +132,13 @@ __global__ void __launch_bounds__(kThreads) fft_lines_kernel(const FftArgs a, co
         else { l = idx / N; k = idx % N; g = base + (long long)l * N + k; }
         if (!STRIDED && L0 + l >= a.nlines) continue;
         const float2 v = buf[l * LD + k];
-        if (mode == kModeOutReal) a.out_real[g] = v.x * a.out_scale; else a.z[g] = v;
+        if (mode == kModeOutReal) {
+            const long long pv = (L0 + l) / a.lines_per_vol, r = g + pv * a.V;
+            a.out_real[r] = v.x * a.out_scale;
+            if (2 * pv + 1 < a.nvol) a.out_real[r + a.V] = v.y * a.out_scale;
+        } else {
+            a.z[g] = v;
+        }
     }
 }
 
@@ -149,11 +166,16 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
     const int step = STRIDED ? (int)a.S : 1;                                             // distance between its points
     const bool live = STRIDED || L0 + l < a.nlines;
     float2 *const zl = a.z + base;
+    // real volumes behind the pair (x passes only): volume 2 pv at rbase, volume 2 pv + 1 one volume further
+    const long long pv = STRIDED ? 0 : (L0 + l) / a.lines_per_vol, rbase = base + pv * a.V;
+    const bool has_b = !STRIDED && 2 * pv + 1 < a.nvol;
     float2 v[E];
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int o = (j + T * m) * step;
-        v[m] = !live ? make_float2(0.f, 0.f) : (mode == kModeInReal) ? make_float2(__ldg(a.in_real + base + o), 0.f) : zl[o];
+        if (!live) v[m] = make_float2(0.f, 0.f);
+        else if (mode == kModeInReal) v[m] = make_float2(__ldg(a.in_real + rbase + o), has_b ? __ldg(a.in_real + rbase + a.V + o) : 0.f);
+        else v[m] = zl[o];
     }
     __syncthreads();   // twiddle table filled
     auto transform = [&](bool inverse) {   // the inverse is the forward transform of the swapped halves (fft_regs.cuh)
@@ -210,7 +232,12 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int o = (j + T * m) * step;
-        if (mode == kModeOutReal) a.out_real[base + o] = v[m].x * a.out_scale; else zl[o] = v[m];
+        if (mode == kModeOutReal) {
+            a.out_real[rbase + o] = v[m].x * a.out_scale;
+            if (has_b) a.out_real[rbase + a.V + o] = v[m].y * a.out_scale;
+        } else {
+            zl[o] = v[m];
+        }
     }
 }
 
@@ -360,9 +387,10 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
     alloc((void **)&p->chibar, T * sizeof(float));
     alloc((void **)&p->kp, T * sizeof(float));
     alloc((void **)&p->q, 3 * T * sizeof(float));
-    alloc((void **)&p->z, T * sizeof(float2));
-    alloc((void **)&p->phihat, T * sizeof(float2));
-    alloc((void **)&p->phat, T * sizeof(float2));
+    const size_t TP = V * (size_t)((nvol + 1) / 2);   // complex volumes: two real volumes ride one complex transform
+    alloc((void **)&p->z, TP * sizeof(float2));
+    alloc((void **)&p->phihat, TP * sizeof(float2));
+    alloc((void **)&p->phat, TP * sizeof(float2));
     for (int k = 0; k < 3; ++k) alloc((void **)&p->tw[k], (size_t)dims[k] * sizeof(float2));
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); pd_destroy3d(p); return PD_ENOMEM; }
     if (e != cudaSuccess) { pd_destroy3d(p); return pd_cuda_fail_((int)e, "cudaMalloc"); }
@@ -402,7 +430,8 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int nx = p->nx, ny = p->ny, nz = p->nz, nvol = p->nvol;
     const long long V = (long long)nx * ny * nz, T = V * nvol;
-    cudaError_t e = cudaMemsetAsync(p->phat, 0, T * sizeof(float2), st);
+    const int npairs = (nvol + 1) / 2;
+    cudaError_t e = cudaMemsetAsync(p->phat, 0, V * npairs * sizeof(float2), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(p->q, 0, 3 * T * sizeof(float), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(p->chibar, 0, T * sizeof(float), st);
     if (e == cudaSuccess) e = cudaMemsetAsync(chi_out, 0, T * sizeof(float), st);
@@ -412,9 +441,10 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     std::memset(&f, 0, sizeof(f));
     f.z = p->z; f.phihat = p->phihat; f.phat = p->phat; f.D = p->D;
     f.sigma = p->sigma; f.inv1ps = 1.0f / (1.0f + p->sigma); f.out_scale = (float)(1.0 / (double)V);
-    const long long xlines = (long long)nvol * nz * ny;
-    const dim3 gx((unsigned)((xlines + kTL - 1) / kTL)), gy((unsigned)(nx / kTL), (unsigned)(nvol * nz)),
-        gz((unsigned)((long long)nx * ny / kTL), (unsigned)nvol);
+    f.V = V; f.lines_per_vol = nz * ny; f.nvol = nvol;
+    const long long xlines = (long long)npairs * nz * ny;
+    const dim3 gx((unsigned)((xlines + kTL - 1) / kTL)), gy((unsigned)(nx / kTL), (unsigned)(npairs * nz)),
+        gz((unsigned)((long long)nx * ny / kTL), (unsigned)npairs);
     int launches = 0;
     auto pass_x = [&](const float *in_real, float *out_real, bool inverse) {
         FftArgs a = f;

@@ -86,6 +86,20 @@ def test_automatic_steps_alpha_zero_and_max_iters_zero(torch, pd, o3):
     assert not g.any() and n == 3
 
 
+def test_pair_partners_of_unequal_magnitude(torch, pd, o3):
+    """Volumes 2k and 2k+1 share one complex transform: the weak partner inherits the absolute rounding error of the
+    strong one.  Measured bound: ratio 1e-2 keeps the weak volume within 1e-3 after 10 iterations (and the strong one
+    within 2e-5); documented in include/pd.h -- there is no per-volume normalisation in the 3-D path yet."""
+    case = synth.volume_case(64, 32, 16, nvol=3, seed=5, b0_axis=2)
+    f = case["field"].copy()
+    f[1] *= 1e-2
+    lam = 0.02 * float(np.abs(case["field"]).max())
+    g, _ = gpu_solve3(torch, pd, f, case["mask"], 10, lam=lam, b0=2)
+    o = o3.solve3(f, case["mask"], lambda_=lam, sigma=0.25, tau=0.25, max_iters=10, b0_dir=2)
+    r = vol_rel(g, o)
+    assert r[0] < 2e-5 and r[2] < 2e-5 and r[1] < 1e-3, r
+
+
 def test_full_size_volume(torch, pd, o3):
     """The size bench.py --volume times per coil: 256 x 256 x 64, 10 iterations against the oracle."""
     case = synth.volume_case(256, 256, 64, nvol=1, seed=9, b0_axis=2)

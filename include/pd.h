@@ -212,8 +212,8 @@ int pd_destroy(pd_plan_t p);
  * pd_plan3d: nx in {16..256}, ny, nz in {8..256}, powers of two (else PD_ESIZE); nvol independent volumes (coils);
  *   B0_axis 0 = x, 1 = y, 2 = z; sigma <= 0 or tau <= 0: automatic steps 1/sqrt(4/9 + 12); explicit steps with
  *   sigma*tau*(4/9 + 12) >= 1 give PD_ESTEP.  Allocates 32 bytes per voxel of workspace + the D3 table.  Volumes 2k and
- *   2k+1 ride one complex transform: their rounding errors mix at the 1e-7 level of the LARGER one, so the volumes of a
- *   call should be of comparable magnitude (the coils of one scan are); there is no per-volume normalisation yet.
+ *   2k+1 ride one complex transform, each in its own power-of-two normalisation 2^-floor(log2 rms(field_v)) (exact; the
+ *   iteration is invariant under it), so partners of very different magnitude do not disturb each other.
  * pd_solve3d: field, mask (NULL = ones), chi_out: DEVICE, [nvol][nz][ny][nx] fp32, x fastest; chi_out is the primal
  *   state during the call.  Enqueues everything on cuda_stream; does not synchronise.
  * Errors: PD_EINVAL, PD_ESIZE, PD_ESTEP, PD_ENOMEM, PD_ECUDA. */

@@ -26,7 +26,7 @@ namespace {
 constexpr int kTL = 16;         // lines per CTA
 constexpr int kThreads = 256;
 
-enum { kModePlain = 0, kModeInReal = 1, kModeOutReal = 2, kModeStoreSpectrum = 3, kModeDual = 4 };
+enum { kModePlain = 0, kModeInReal = 1, kModeOutReal = 2, kModeStoreSpectrum = 3, kModeDual = 4, kModeInRealScaled = 5 };
 
 struct FftArgs {
     const float *in_real;     // kModeInReal
@@ -38,6 +38,7 @@ struct FftArgs {
     long long nlines;         // x pass: number of lines (of the PAIRED volumes)
     long long V;              // voxels of one volume
     int lines_per_vol;        // nz * ny
+    const float *cscale;      // kModeInReal: per-volume factor applied on load (NULL: none)
     int nvol;                 // real volumes: the pair pv holds volume 2 pv in its real part and 2 pv + 1 (if any) in its imaginary part
     long long S;              // strided pass: distance between consecutive points of a line (nx, or nx*ny)
     float sigma, inv1ps, out_scale;
@@ -89,9 +90,10 @@ __global__ void __launch_bounds__(kThreads) fft_lines_kernel(const FftArgs a, co
         else { l = idx / N; k = idx % N; g = base + (long long)l * N + k; }
         float2 v = make_float2(0.f, 0.f);
         if (STRIDED || L0 + l < a.nlines) {
-            if (mode == kModeInReal) {
+            if (mode == kModeInReal || mode == kModeInRealScaled) {
                 const long long pv = (L0 + l) / a.lines_per_vol, r = g + pv * a.V;       // volume 2 pv, same line and point
                 v = make_float2(a.in_real[r], 2 * pv + 1 < a.nvol ? a.in_real[r + a.V] : 0.f);
+                if (mode == kModeInRealScaled) { v.x *= a.cscale[2 * pv]; if (2 * pv + 1 < a.nvol) v.y *= a.cscale[2 * pv + 1]; }
             } else {
                 v = a.z[g];
             }
@@ -169,13 +171,20 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
     // real volumes behind the pair (x passes only): volume 2 pv at rbase, volume 2 pv + 1 one volume further
     const long long pv = STRIDED ? 0 : (L0 + l) / a.lines_per_vol, rbase = base + pv * a.V;
     const bool has_b = !STRIDED && 2 * pv + 1 < a.nvol;
+    constexpr bool IN_REAL = mode == kModeInReal || mode == kModeInRealScaled;
+    float ca = 1.f, cb = 1.f;   // per-volume power-of-two normalisation of the field (exact), see vol_scale_kernel
+    if (mode == kModeInRealScaled) { ca = a.cscale[2 * pv]; if (has_b) cb = a.cscale[2 * pv + 1]; }
     float2 v[E];
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int o = (j + T * m) * step;
         if (!live) v[m] = make_float2(0.f, 0.f);
-        else if (mode == kModeInReal) v[m] = make_float2(__ldg(a.in_real + rbase + o), has_b ? __ldg(a.in_real + rbase + a.V + o) : 0.f);
+        else if (IN_REAL) v[m] = make_float2(__ldg(a.in_real + rbase + o), has_b ? __ldg(a.in_real + rbase + a.V + o) : 0.f);
         else v[m] = zl[o];
+    }
+    if (mode == kModeInRealScaled) {   // after all loads have been issued
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = make_float2(ca * v[m].x, cb * v[m].y);
     }
     __syncthreads();   // twiddle table filled
     auto transform = [&](bool inverse) {   // the inverse is the forward transform of the swapped halves (fft_regs.cuh)
@@ -243,7 +252,8 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
 
 struct VoxArgs {
     int nx, ny, nz;           // powers of two; nx a multiple of 4
-    int lx, ly;               // log2 nx, log2 ny
+    int lx, ly, lv;           // log2 nx, log2 ny, log2 (nx ny nz)
+    const float *cscale;      // [nvol] normalisation of every volume: the ball of volume v has radius alpha * cscale[v]
     long long nvox;           // nvol * nz * ny * nx
     const float *mask;        // or NULL (ones)
     float *chi, *chibar, *qx, *qy, *qz;
@@ -269,10 +279,11 @@ __global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
         const float4 gy = y + 1 < a.ny ? sub4(ld4(a.chibar + i + sy), c) : zero;
         const float4 gz = z + 1 < a.nz ? sub4(ld4(a.chibar + i + sz), c) : zero;
         float4 qx = ld4(a.qx + i), qy = ld4(a.qy + i), qz = ld4(a.qz + i);
+        const float alpha = a.alpha * a.cscale[i >> a.lv];
         auto one_voxel = [&](float &px, float &py, float &pz, float mm, float dx, float dy, float dz) {
             const float tx = px + a.sigma * mm * dx, ty = py + a.sigma * mm * dy, tz = pz + a.sigma * mm * dz;
             const float nrm = sqrtf(tx * tx + ty * ty + tz * tz);
-            const float s = nrm > a.alpha ? a.alpha / nrm : 1.f;
+            const float s = nrm > alpha ? alpha / nrm : 1.f;
             px = tx * s; py = ty * s; pz = tz * s;
         };
         one_voxel(qx.x, qy.x, qz.x, m.x, gx.x, gy.x, gz.x);
@@ -310,6 +321,51 @@ __global__ void __launch_bounds__(kThreads) chi_update3_kernel(const VoxArgs a) 
     }
 }
 
+// Per-volume normalisation (the 2-D path's pair_scale): the iteration is exactly invariant under
+// (phi, alpha) -> (c phi, c alpha) with chi -> c chi, and a power of two is exact in floating point, so every volume is
+// iterated at c_v = 2^-floor(log2 rms(phi_v)) and the two volumes of a pair meet at the same magnitude.  Two kernels,
+// fixed summation order: bitwise repeatable.
+constexpr int kScaleParts = 64;
+__global__ void __launch_bounds__(kThreads) vol_sumsq_kernel(const float *__restrict__ field, long long V, float *__restrict__ part) {
+    const long long chunk = V / kScaleParts, b0 = (long long)blockIdx.y * V + (long long)blockIdx.x * chunk;
+    float s = 0.f;
+    for (long long i = threadIdx.x * 4LL; i < chunk; i += kThreads * 4LL) {
+        const float4 f = ld4(field + b0 + i);
+        s += f.x * f.x + f.y * f.y + f.z * f.z + f.w * f.w;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    __shared__ float ws[kThreads / 32];
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float t = 0.f;
+        for (int w = 0; w < kThreads / 32; ++w) t += ws[w];
+        part[blockIdx.y * kScaleParts + blockIdx.x] = t;
+    }
+}
+__global__ void vol_scale_kernel(const float *__restrict__ part, long long V, int nvol, float *__restrict__ cscale) {
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nvol) return;
+    float t = 0.f;
+    for (int k = 0; k < kScaleParts; ++k) t += part[v * kScaleParts + k];
+    const float rms = sqrtf(t / (float)V);
+    const float c = (rms > 0.f && rms < 3.0e38f) ? scalbnf(1.0f, -ilogbf(rms)) : 1.0f;
+    cscale[v] = c;
+    cscale[nvol + v] = t > 0.f ? 1.0f / c : 0.f;   // factor of the final store; a zero field returns chi = 0 exactly (R13b),
+                                                   // whatever rounding noise its pair partner left in its lane
+}
+// chi <- chi / c_v at the end (exact)
+__global__ void __launch_bounds__(kThreads) vol_unscale_kernel(float *__restrict__ chi, long long nvox, int lv, const float *__restrict__ rscale) {
+    for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < (nvox >> 2); i4 += (long long)gridDim.x * kThreads) {
+        const long long i = i4 << 2;
+        const float r = rscale[i >> lv];
+        float4 c = ld4(chi + i);
+        c.x *= r; c.y *= r; c.z *= r; c.w *= r;
+        st4(chi + i, c);
+    }
+}
+
 bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1)) == 0; }
 
 template <int N, bool STRIDED>
@@ -321,6 +377,7 @@ void launch_reg(dim3 grid, const FftArgs &a, int mode, cudaStream_t st) {
         else fft_lines_reg_kernel<N, STRIDED, kModePlain><<<grid, NT, 0, st>>>(a);
     } else {
         if (mode == kModeInReal) fft_lines_reg_kernel<N, STRIDED, kModeInReal><<<grid, NT, 0, st>>>(a);
+        else if (mode == kModeInRealScaled) fft_lines_reg_kernel<N, STRIDED, kModeInRealScaled><<<grid, NT, 0, st>>>(a);
         else if (mode == kModeOutReal) fft_lines_reg_kernel<N, STRIDED, kModeOutReal><<<grid, NT, 0, st>>>(a);
         else fft_lines_reg_kernel<N, STRIDED, kModePlain><<<grid, NT, 0, st>>>(a);
     }
@@ -344,6 +401,7 @@ struct pd_plan3d_s {
     int nx, ny, nz, nvol, b0_axis, num_sms;
     float lambda, sigma, tau, theta;
     float *D, *chibar, *kp, *q;     // q: three volumes
+    float *cscale, *spart;          // [nvol] normalisation, [nvol][kScaleParts] partial sums
     float2 *tw[3], *z, *phihat, *phat;
     int last_launches;
 };
@@ -352,7 +410,7 @@ extern "C" {
 
 int pd_destroy3d(pd_plan3d_t p) {
     if (!p) return PD_EINVAL;
-    void *ptrs[] = {p->D, p->chibar, p->kp, p->q, p->tw[0], p->tw[1], p->tw[2], p->z, p->phihat, p->phat};
+    void *ptrs[] = {p->D, p->chibar, p->kp, p->q, p->tw[0], p->tw[1], p->tw[2], p->z, p->phihat, p->phat, p->cscale, p->spart};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -387,6 +445,8 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
     alloc((void **)&p->chibar, T * sizeof(float));
     alloc((void **)&p->kp, T * sizeof(float));
     alloc((void **)&p->q, 3 * T * sizeof(float));
+    alloc((void **)&p->cscale, 2 * (size_t)nvol * sizeof(float));   // c_v, then the factors of the final store
+    alloc((void **)&p->spart, (size_t)nvol * kScaleParts * sizeof(float));
     const size_t TP = V * (size_t)((nvol + 1) / 2);   // complex volumes: two real volumes ride one complex transform
     alloc((void **)&p->z, TP * sizeof(float2));
     alloc((void **)&p->phihat, TP * sizeof(float2));
@@ -449,7 +509,7 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     auto pass_x = [&](const float *in_real, float *out_real, bool inverse) {
         FftArgs a = f;
         a.tw = p->tw[0]; a.nlines = xlines; a.inverse = inverse ? 1 : 0; a.in_real = in_real; a.out_real = out_real;
-        launch_fft<false>(nx, gx, a, in_real ? kModeInReal : out_real ? kModeOutReal : kModePlain, st);
+        launch_fft<false>(nx, gx, a, in_real ? (a.cscale ? kModeInRealScaled : kModeInReal) : out_real ? kModeOutReal : kModePlain, st);
         ++launches;
     };
     auto pass_y = [&](bool inverse) {
@@ -464,8 +524,13 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
         launch_fft<true>(nz, gz, a, mode, st);
         ++launches;
     };
-    // phi^ = F phi, once (everything else starts at zero)
+    // per-volume normalisation, then phi^ = F (c phi), once (everything else starts at zero)
+    vol_sumsq_kernel<<<dim3(kScaleParts, (unsigned)nvol), kThreads, 0, st>>>(field, V, p->spart);
+    vol_scale_kernel<<<(nvol + 63) / 64, 64, 0, st>>>(p->spart, V, nvol, p->cscale);
+    launches += 2;
+    f.cscale = p->cscale;
     pass_x(field, nullptr, false);
+    f.cscale = nullptr;
     pass_y(false);
     pass_z(kModeStoreSpectrum);
 
@@ -474,6 +539,8 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     v.nx = nx; v.ny = ny; v.nz = nz; v.nvox = T; v.mask = mask;
     for (v.lx = 0; (1 << v.lx) < nx; ++v.lx) {}
     for (v.ly = 0; (1 << v.ly) < ny; ++v.ly) {}
+    for (v.lv = 0; (1LL << v.lv) < V; ++v.lv) {}
+    v.cscale = p->cscale;
     v.chi = chi_out; v.chibar = p->chibar; v.qx = p->q; v.qy = p->q + T; v.qz = p->q + 2 * T; v.kp = p->kp;
     v.sigma = p->sigma; v.tau = p->tau; v.theta = p->theta; v.alpha = p->lambda;
     const long long need = (T / 4 + kThreads - 1) / kThreads, cap = (long long)p->num_sms * 8;
@@ -487,6 +554,10 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
         q_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
         chi_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
         launches += 2;
+    }
+    if (max_iters > 0) {
+        vol_unscale_kernel<<<vgrid, kThreads, 0, st>>>(chi_out, T, v.lv, p->cscale + nvol);
+        ++launches;
     }
     p->last_launches = launches;
     e = cudaGetLastError();

@@ -61,7 +61,7 @@ def test_one_iteration_all_axes(torch, pd, o3, nx, ny, nz, b0):
     g, launches = gpu_solve3(torch, pd, f, m, 1, lam=0.05, b0=b0)
     o = o3.solve3(f, m, lambda_=0.05, sigma=0.25, tau=0.25, max_iters=1, b0_dir=b0)
     assert vol_rel(g, o).max() < 1e-5
-    assert launches == 3 + 7
+    assert launches == 2 + 3 + 7 + 1          # normalisation, phi^, one iteration, un-normalisation
 
 
 @pytest.mark.parametrize("iters,theta,masked", [(2, 1.0, True), (3, 0.5, True), (25, 1.0, True), (25, 1.0, False)])
@@ -83,21 +83,26 @@ def test_automatic_steps_alpha_zero_and_max_iters_zero(torch, pd, o3):
     o = o3.solve3(case["field"], case["mask"], lambda_=0.0, sigma=s, tau=s, max_iters=6, b0_dir=0)
     assert vol_rel(g, o).max() < 1e-5
     g, n = gpu_solve3(torch, pd, case["field"], None, 0, lam=0.1, b0=0)
-    assert not g.any() and n == 3
+    assert not g.any() and n == 5
 
 
-def test_pair_partners_of_unequal_magnitude(torch, pd, o3):
-    """Volumes 2k and 2k+1 share one complex transform: the weak partner inherits the absolute rounding error of the
-    strong one.  Measured bound: ratio 1e-2 keeps the weak volume within 1e-3 after 10 iterations (and the strong one
-    within 2e-5); documented in include/pd.h -- there is no per-volume normalisation in the 3-D path yet."""
+@pytest.mark.parametrize("ratio", [1e-2, 1e-3, 1e4])
+def test_pair_partners_of_unequal_magnitude(torch, pd, o3, ratio):
+    """Volumes 2k and 2k+1 share one complex transform; every volume is iterated in its own power-of-two normalisation
+    (the iteration is invariant under (phi, alpha) -> (c phi, c alpha)), so a weak partner does not inherit the absolute
+    rounding error of a strong one: the one-iteration gate holds for both."""
     case = synth.volume_case(64, 32, 16, nvol=3, seed=5, b0_axis=2)
     f = case["field"].copy()
-    f[1] *= 1e-2
-    lam = 0.02 * float(np.abs(case["field"]).max())
-    g, _ = gpu_solve3(torch, pd, f, case["mask"], 10, lam=lam, b0=2)
-    o = o3.solve3(f, case["mask"], lambda_=lam, sigma=0.25, tau=0.25, max_iters=10, b0_dir=2)
-    r = vol_rel(g, o)
-    assert r[0] < 2e-5 and r[2] < 2e-5 and r[1] < 1e-3, r
+    f[1] *= np.float32(ratio)
+    lam = 0.02 * float(np.abs(case["field"]).max()) * min(1.0, ratio)    # active on the weak volume too
+    for iters, gate in [(1, 1e-5), (10, 2e-5)]:
+        g, _ = gpu_solve3(torch, pd, f, case["mask"], iters, lam=lam, b0=2)
+        o = o3.solve3(f, case["mask"], lambda_=lam, sigma=0.25, tau=0.25, max_iters=iters, b0_dir=2)
+        assert vol_rel(g, o).max() < gate, vol_rel(g, o)
+    z = f.copy()
+    z[0] = 0.0                                                           # a zero volume beside an active partner stays zero
+    g, _ = gpu_solve3(torch, pd, z, case["mask"], 3, lam=lam, b0=2)
+    assert not g[0].any() and g[1].any()
 
 
 def test_full_size_volume(torch, pd, o3):

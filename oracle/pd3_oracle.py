@@ -11,7 +11,7 @@ reduction to the 2-D oracle for nz = 1, hand values and adjointness of the gradi
 Readings (R23): volume [nz][ny][nx], isotropic voxels ("isotropy"): k = (fi/nx, fj/ny, fk/nz)
 with signed fftfreq indices; D3 = 1/3 - k_b^2/|k|^2, D3(0) = 0, B0 along x, y or z; G: forward differences with Neumann
 boundary on all three axes, G^T its exact adjoint; the q-projection is the pointwise Euclidean norm over the three
-components; lambda on the regulariser (R2), r = K chi_bar - phi (W = identity), zero start, chi_N returned (R11).
+components; lambda on the regulariser (R2), r = W (K chi_bar - phi) (R3; W optional), zero start, chi_N returned (R11).
 """
 import numpy as np
 
@@ -54,25 +54,28 @@ def grad3T(qx, qy, qz):
     return out
 
 
-def solve3(field, mask=None, *, lambda_, sigma, tau, theta=1.0, max_iters=10, b0_dir=B0_Z):
-    """PAPER.md:45-49 on one volume [nz][ny][nx] (or a stack of independent volumes [nvol][nz][ny][nx]).  Returns chi_N."""
+def solve3(field, mask=None, weight=None, *, lambda_, sigma, tau, theta=1.0, max_iters=10, b0_dir=B0_Z):
+    """PAPER.md:45-49 on one volume [nz][ny][nx] (or a stack of independent volumes [nvol][nz][ny][nx]).  Returns chi_N.
+    weight: the data weighting W of Eq.(1) (None = identity): r = W (K chi_bar - phi) (R3), chi-update with K (W p)."""
     field = np.asarray(field, np.float64)
     if field.ndim == 4:
-        return np.stack([solve3(field[v], None if mask is None else np.asarray(mask)[v], lambda_=lambda_, sigma=sigma, tau=tau,
+        return np.stack([solve3(field[v], None if mask is None else np.asarray(mask)[v],
+                                None if weight is None else np.asarray(weight)[v], lambda_=lambda_, sigma=sigma, tau=tau,
                                 theta=theta, max_iters=max_iters, b0_dir=b0_dir) for v in range(field.shape[0])])
     M = np.ones_like(field) if mask is None else np.asarray(mask, np.float64)
+    W = np.ones_like(field) if weight is None else np.asarray(weight, np.float64)
     chi = np.zeros_like(field)
     chibar = np.zeros_like(field)
     p = np.zeros_like(field)
     qx, qy, qz = np.zeros_like(field), np.zeros_like(field), np.zeros_like(field)
     for _ in range(max_iters):
-        p = (p + sigma * (apply_K3(chibar, b0_dir) - field)) / (1.0 + sigma)            # PAPER.md:49 line 1
+        p = (p + sigma * W * (apply_K3(chibar, b0_dir) - field)) / (1.0 + sigma)        # PAPER.md:49 line 1
         gx, gy, gz = grad3(chibar)
         tx, ty, tz = qx + sigma * M * gx, qy + sigma * M * gy, qz + sigma * M * gz      # PAPER.md:49 line 2
         nrm = np.sqrt(tx * tx + ty * ty + tz * tz)
         scale = np.where(nrm > lambda_, lambda_ / np.where(nrm > lambda_, nrm, 1.0), 1.0)   # onto the lambda-ball (R13)
         qx, qy, qz = tx * scale, ty * scale, tz * scale
-        new = chi - tau * apply_K3(p, b0_dir) - tau * grad3T(M * qx, M * qy, M * qz)    # PAPER.md:49 line 3
+        new = chi - tau * apply_K3(W * p, b0_dir) - tau * grad3T(M * qx, M * qy, M * qz)   # PAPER.md:49 line 3
         chibar = new + theta * (new - chi)                                              # PAPER.md:49 line 4
         chi = new
     return chi

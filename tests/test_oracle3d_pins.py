@@ -36,6 +36,10 @@ def test_P21_one_slice_volume_is_the_2d_problem(oracle, b0):
     rng = np.random.default_rng(21 + b0)
     f = rng.normal(size=(12, 16))
     m = (rng.uniform(size=f.shape) > 0.3).astype(np.float64)
+    w = rng.uniform(0.2, 1.0, size=f.shape).astype(np.float32)
+    got = o3.solve3(f.astype(np.float32)[None], m[None], w[None], lambda_=0.3, sigma=0.25, tau=0.25, max_iters=6, b0_dir=b0)
+    ref = oracle.solve(f.astype(np.float32), m.astype(np.float32), w, lambda_=0.3, sigma=0.25, tau=0.25, max_iters=6, b0_dir=b0)["chi"][0]
+    assert rel(got[0], ref) < 1e-12                                       # with a data weighting W as well
     for iters, theta in [(1, 1.0), (7, 1.0), (5, 0.5)]:
         got = o3.solve3(f[None], m[None], lambda_=0.3, sigma=0.25, tau=0.25, theta=theta, max_iters=iters, b0_dir=b0)
         ref = oracle.solve(f.astype(np.float32), m.astype(np.float32), lambda_=0.3, sigma=0.25, tau=0.25, theta=theta,
@@ -84,25 +88,27 @@ def dense_ops(nx, ny, nz, b0):
     return K, G
 
 
-@pytest.mark.parametrize("b0,theta", [(2, 1.0), (0, 0.7)])
-def test_P23_dense_matrix_bruteforce_4x4x4(b0, theta):
+@pytest.mark.parametrize("b0,theta,weighted", [(2, 1.0, False), (0, 0.7, False), (1, 0.9, True)])
+def test_P23_dense_matrix_bruteforce_4x4x4(b0, theta, weighted):
     """K from Kronecker DFT matrices, G from stencils, the iteration with mat-vecs (non-cubic 4x3x5 volume, mask)."""
     nx, ny, nz = 4, 3, 5
     K, G = dense_ops(nx, ny, nz, b0)
     rng = np.random.default_rng(23)
     f = rng.normal(size=(nz, ny, nx))
     m = (rng.uniform(size=f.shape) > 0.25).astype(np.float64)
+    w = rng.uniform(0.2, 1.0, size=f.shape) if weighted else np.ones_like(f)
     lam, sig, tau = 0.2, 0.25, 0.25
     chi = np.zeros(f.size); bar = chi.copy(); p = chi.copy(); q = np.zeros((3, f.size))
+    Kw = w.ravel()[:, None] * K                                          # K_full's data block is W K; its transpose K^T W
     for _ in range(6):
-        p = (p + sig * (K @ bar - f.ravel())) / (1 + sig)
+        p = (p + sig * (Kw @ bar - w.ravel() * f.ravel())) / (1 + sig)
         t = q + sig * m.ravel() * (G @ bar)
         nrm = np.sqrt((t * t).sum(0))
         q = t * np.where(nrm > lam, lam / np.maximum(nrm, 1e-300), 1.0)
-        new = chi - tau * (K.T @ p) - tau * sum(G[c].T @ (m.ravel() * q[c]) for c in range(3))
+        new = chi - tau * (Kw.T @ p) - tau * sum(G[c].T @ (m.ravel() * q[c]) for c in range(3))
         bar = new + theta * (new - chi)
         chi = new
-    got = o3.solve3(f, m, lambda_=lam, sigma=sig, tau=tau, theta=theta, max_iters=6, b0_dir=b0)
+    got = o3.solve3(f, m, w if weighted else None, lambda_=lam, sigma=sig, tau=tau, theta=theta, max_iters=6, b0_dir=b0)
     assert rel(got.ravel(), chi) < 1e-12
 
 

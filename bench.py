@@ -286,6 +286,9 @@ def run_volume(args):
     lam = 0.02 * float(np.abs(case["field"]).max())
     out = torch.empty_like(f)
     plan = binding.Plan3D(nx, ny, nz, nvol, 2, lam, 0.25, 0.25, 1.0)
+    if args.weighted:   # W set: the literal iteration, K applied twice (12 launches per iteration)
+        gen = torch.Generator(device="cuda").manual_seed(200609808)
+        plan.set_weight(0.2 + 0.8 * torch.rand(f.shape, device="cuda", generator=gen))
     peak, peak_src = load_peaks()
     for _ in range(args.warmup):
         plan.solve(f, m, out, iters)
@@ -302,7 +305,7 @@ def run_volume(args):
     launches = plan.last_launch_count
     plan.destroy()
     nvox = nvol * nz * ny * nx
-    bytes_per_voxel_it = 118.0
+    bytes_per_voxel_it = 172.0 if args.weighted else 118.0   # literal: 2 x (8 + 8 + 10 + 8 + 8) + 56 (q- and p-update) + 32
     gbs = bytes_per_voxel_it * nvox * iters / (ms * 1e-3) / 1e9
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import pd3_oracle as o3
@@ -311,9 +314,10 @@ def run_volume(args):
     dt = time.perf_counter() - t0
     line = {"metric": "pd3_voxel_iterations_per_s", "value": nvox * iters / (ms * 1e-3), "unit": "voxel-iterations/s", "n_gpus": 1,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "V1: %d coil volumes of %dx%dx%d (synth.volume_case), %d iterations, B0 along z, mask" % (nvol, nx, ny, nz, iters),
+            "config": {"workload": "V1: %d coil volumes of %dx%dx%d (synth.volume_case), %d iterations, B0 along z, mask%s"
+                                   % (nvol, nx, ny, nz, iters, ", random W in [0.2, 1] (literal iteration)" if args.weighted else ""),
                        "l2": "working set (%.1f GB) exceeds the 126 MB L2" % (44.0 * nvox / 1e9)},
-            "roofline": {"kernel": "whole step (7 launches per iteration)", "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
+            "roofline": {"kernel": "whole step (%d launches per iteration)" % (12 if args.weighted else 7), "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
                          "frac": gbs / peak, "algorithmic_bytes_per_voxel_iteration": bytes_per_voxel_it, "peak_source": peak_src, "traffic": None},
             "cpu_baseline": {"value": nz * ny * nx * 4 / dt, "unit": "voxel-iterations/s", "cores": os.cpu_count(), "kind": "oracle (numpy float64, numpy.fft)",
                              "sample": "1 volume, 4 iterations, %.1f s" % dt},

@@ -206,7 +206,7 @@ int pd_destroy(pd_plan_t p);
  * operator in all three dimensions" -- with the 3-D dipole kernel D3(k) = 1/3 - k_b^2/|k|^2, D3(0) = 0,
  * k = (fi/nx, fj/ny, fk/nz) with signed indices (isotropic voxels; reading R23), one problem per VOLUME:
  * the same iteration with q of three components projected on the lambda-ball by its pointwise Euclidean
- * norm, forward differences with Neumann boundary on all three axes, W = identity, lambda on the regulariser (R2).  The
+ * norm, forward differences with Neumann boundary on all three axes, W optional (pd_set_weight3d), lambda on the regulariser (R2).  The
  * slices of a volume are coupled by the z transform and the z difference: there is no per-slice stop, the call runs
  * exactly max_iters iterations.  A streaming implementation (7 launches per iteration).
  * pd_plan3d: nx in {16..256}, ny, nz in {8..256}, powers of two (else PD_ESIZE); nvol independent volumes (coils);
@@ -220,6 +220,11 @@ int pd_destroy(pd_plan_t p);
 typedef struct pd_plan3d_s *pd_plan3d_t;
 int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, float lambda, float sigma, float tau, float theta);
 int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_out, int max_iters, void *cuda_stream);
+/* Optional data weighting W of Eq.(1) for the 3-D variant (DEVICE, [nvol][nz][ny][nx], 16-byte aligned, caller-owned, must
+ * outlive the solves; |W| <= 1 is assumed by the step bound); NULL = identity.  With W set the dual p stays in the image
+ * domain and K is applied twice per iteration, literally as PAPER.md:49 (12 launches per iteration instead of 7); the
+ * first call with a non-NULL W allocates 8 bytes per voxel.  Errors: PD_EINVAL, PD_ENOMEM, PD_ECUDA. */
+int pd_set_weight3d(pd_plan3d_t p, const float *W);
 int pd_last_launch_count3d(pd_plan3d_t p);   /* kernels enqueued by the last pd_solve3d */
 int pd_destroy3d(pd_plan3d_t p);
 

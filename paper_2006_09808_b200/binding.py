@@ -26,7 +26,7 @@ VARIANT_AUTO, VARIANT_STREAMING, VARIANT_RESIDENT = 0, 1, 2
 # every symbol include/pd.h declares (tests/test_abi.py checks the header against this list and the built library)
 SYMBOLS = ["pd_plan", "pd_solve", "pd_solve_host", "pd_set_weight", "pd_set_steps", "pd_set_option", "pd_get_stats",
            "pd_get_stats_host", "pd_get_kernel_times", "pd_last_launch_count", "pd_get_info", "pd_get_hybrid_tail", "pd_hybrid_tail_rule", "pd_line_factors", "pd_get_hybrid_rho", "pd_set_b0_angle", "pd_set_norm_bounds", "pd_destroy", "pd_strerror",
-           "pd_solve_static", "pd_preprocess", "pd_combine_coils", "pd_plan3d", "pd_solve3d", "pd_last_launch_count3d",
+           "pd_solve_static", "pd_preprocess", "pd_combine_coils", "pd_plan3d", "pd_solve3d", "pd_set_weight3d", "pd_last_launch_count3d",
            "pd_destroy3d"]
 
 _lib = None
@@ -69,6 +69,7 @@ def lib():
         L.pd_combine_coils.argtypes = [vp, vp, ip, ip, ip, ip, vp, vp]
         L.pd_plan3d.argtypes = [C.POINTER(vp), ip, ip, ip, ip, ip, fp, fp, fp, fp]
         L.pd_solve3d.argtypes = [vp, vp, vp, vp, ip, vp]
+        L.pd_set_weight3d.argtypes = [vp, vp]
         L.pd_last_launch_count3d.argtypes = [vp]
         L.pd_destroy3d.argtypes = [vp]
         L.pd_solve_static.argtypes = [ip, ip, ip, ip, fp, fp, fp, fp, vp, vp, vp, ip, fp, vp, vp, vp, vp]
@@ -139,6 +140,13 @@ class Plan3D:
             if t is not None and tuple(t.shape) != self.shape:
                 raise ValueError("expected shape %r" % (self.shape,))
         _check(lib().pd_solve3d(self._h, _ptr(field), _ptr(mask), _ptr(chi_out), int(max_iters), _stream_handle(stream)))
+
+    def set_weight(self, weight):
+        """pd_set_weight3d: W [nvol][nz][ny][nx] (float32 CUDA tensor, kept alive here) or None."""
+        if weight is not None and tuple(weight.shape) != self.shape:
+            raise ValueError("expected shape %r" % (self.shape,))
+        self._keep = weight
+        _check(lib().pd_set_weight3d(self._h, _ptr(weight)))
 
     @property
     def last_launch_count(self):

@@ -26,7 +26,7 @@ namespace {
 constexpr int kTL = 16;         // lines per CTA
 constexpr int kThreads = 256;
 
-enum { kModePlain = 0, kModeInReal = 1, kModeOutReal = 2, kModeStoreSpectrum = 3, kModeDual = 4, kModeInRealScaled = 5 };
+enum { kModePlain = 0, kModeInReal = 1, kModeOutReal = 2, kModeStoreSpectrum = 3, kModeDual = 4, kModeInRealScaled = 5, kModeMulD = 6 };
 
 struct FftArgs {
     const float *in_real;     // kModeInReal
@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(kThreads) fft_lines_kernel(const FftArgs a, co
     }
     __syncthreads();
     fft_tile<N>(buf, tws, a.inverse != 0);
-    if (mode == kModeStoreSpectrum || mode == kModeDual) {
+    if (mode == kModeStoreSpectrum || mode == kModeDual || mode == kModeMulD) {
         // the last forward axis: every coordinate is a frequency now (PAPER.md:49 line 1 in the Fourier domain, W = I)
         for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
             const int l = idx % kTL, k = idx / kTL;
@@ -110,6 +110,7 @@ __global__ void __launch_bounds__(kThreads) fft_lines_kernel(const FftArgs a, co
             const float2 z = buf[l * LD + k];
             if (mode == kModeStoreSpectrum) { a.phihat[g] = z; continue; }
             const float d = a.D[g - (long long)blockIdx.y * N * a.S];
+            if (mode == kModeMulD) { buf[l * LD + k] = make_float2(d * z.x, d * z.y); continue; }   // literal path: K alone
             const float2 f = a.phihat[g];
             float2 p = a.phat[g];
             p.x = (p.x + a.sigma * (d * z.x - f.x)) * a.inv1ps;
@@ -220,6 +221,15 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
         for (int m = 0; m < E; ++m) fl[(j + T * m) * step] = v[m];
         return;
     }
+    if (mode == kModeMulD) {   // literal path (W set): K = F^-1 D3 F alone
+        const float *const dl = a.D + (base - vol);
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const float d = __ldg(dl + (j + T * m) * step);
+            v[m] = make_float2(d * v[m].x, d * v[m].y);
+        }
+        transform(true);
+    }
     if (mode == kModeDual) {   // PAPER.md:49 line 1 in the Fourier domain (W = I), then the spectrum of K p
         const float2 *const fl = a.phihat + base;
         float2 *const pl = a.phat + base;
@@ -254,6 +264,9 @@ struct VoxArgs {
     int nx, ny, nz;           // powers of two; nx a multiple of 4
     int lx, ly, lv;           // log2 nx, log2 ny, log2 (nx ny nz)
     const float *cscale;      // [nvol] normalisation of every volume: the ball of volume v has radius alpha * cscale[v]
+    const float *weight, *field;   // literal path (W set): W, and the caller's phi (normalised on the fly)
+    float *p, *wp;                 // literal path: the dual p in the image domain, and W p (input of the second K)
+    float inv1ps;
     long long nvox;           // nvol * nz * ny * nx
     const float *mask;        // or NULL (ones)
     float *chi, *chibar, *qx, *qy, *qz;
@@ -291,6 +304,17 @@ __global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
         one_voxel(qx.z, qy.z, qz.z, m.z, gx.z, gy.z, gz.z);
         one_voxel(qx.w, qy.w, qz.w, m.w, gx.w, gy.w, gz.w);
         st4(a.qx + i, qx); st4(a.qy + i, qy); st4(a.qz + i, qz);
+        if (a.weight) {   // literal path: p <- (p + sigma W (K chi_bar - phi))/(1 + sigma)  (PAPER.md:49 line 1; R3); a.kp holds K chi_bar
+            const float cs = a.cscale[i >> a.lv];
+            const float4 w = ld4(a.weight + i), u = ld4(a.kp + i), f = ld4(a.field + i);
+            float4 pp = ld4(a.p + i);
+            pp.x = (pp.x + a.sigma * w.x * (u.x - cs * f.x)) * a.inv1ps;
+            pp.y = (pp.y + a.sigma * w.y * (u.y - cs * f.y)) * a.inv1ps;
+            pp.z = (pp.z + a.sigma * w.z * (u.z - cs * f.z)) * a.inv1ps;
+            pp.w = (pp.w + a.sigma * w.w * (u.w - cs * f.w)) * a.inv1ps;
+            st4(a.p + i, pp);
+            st4(a.wp + i, make_float4(w.x * pp.x, w.y * pp.y, w.z * pp.z, w.w * pp.w));
+        }
     }
 }
 
@@ -373,6 +397,7 @@ void launch_reg(dim3 grid, const FftArgs &a, int mode, cudaStream_t st) {
     constexpr int NT = kTL * pdk::FftCfg<N>::T;
     if constexpr (STRIDED) {
         if (mode == kModeDual) fft_lines_reg_kernel<N, STRIDED, kModeDual><<<grid, NT, 0, st>>>(a);
+        else if (mode == kModeMulD) fft_lines_reg_kernel<N, STRIDED, kModeMulD><<<grid, NT, 0, st>>>(a);
         else if (mode == kModeStoreSpectrum) fft_lines_reg_kernel<N, STRIDED, kModeStoreSpectrum><<<grid, NT, 0, st>>>(a);
         else fft_lines_reg_kernel<N, STRIDED, kModePlain><<<grid, NT, 0, st>>>(a);
     } else {
@@ -402,6 +427,8 @@ struct pd_plan3d_s {
     float lambda, sigma, tau, theta;
     float *D, *chibar, *kp, *q;     // q: three volumes
     float *cscale, *spart;          // [nvol] normalisation, [nvol][kScaleParts] partial sums
+    const float *weight;            // caller-owned W or NULL (identity)
+    float *pimg;                    // literal path: p and W p, two volumes (allocated by pd_set_weight3d)
     float2 *tw[3], *z, *phihat, *phat;
     int last_launches;
 };
@@ -410,7 +437,7 @@ extern "C" {
 
 int pd_destroy3d(pd_plan3d_t p) {
     if (!p) return PD_EINVAL;
-    void *ptrs[] = {p->D, p->chibar, p->kp, p->q, p->tw[0], p->tw[1], p->tw[2], p->z, p->phihat, p->phat, p->cscale, p->spart};
+    void *ptrs[] = {p->D, p->chibar, p->kp, p->q, p->tw[0], p->tw[1], p->tw[2], p->z, p->phihat, p->phat, p->cscale, p->spart, p->pimg};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     delete p;
@@ -545,15 +572,35 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     v.sigma = p->sigma; v.tau = p->tau; v.theta = p->theta; v.alpha = p->lambda;
     const long long need = (T / 4 + kThreads - 1) / kThreads, cap = (long long)p->num_sms * 8;
     const int vgrid = (int)(need < cap ? need : cap);
+    const bool literal = p->weight != nullptr;   // W set: p stays in the image domain and K is applied twice (PAPER.md:49 literally)
+    if (literal) {
+        v.weight = p->weight; v.field = field; v.p = p->pimg; v.wp = p->pimg + T; v.inv1ps = 1.0f / (1.0f + p->sigma);
+        e = cudaMemsetAsync(p->pimg, 0, T * sizeof(float), st);
+        if (e != cudaSuccess) return pd_cuda_fail_((int)e, "cudaMemsetAsync (3-D dual)");
+    }
     for (int n = 0; n < max_iters; ++n) {
         pass_x(p->chibar, nullptr, false);     // F chi_bar
         pass_y(false);
-        pass_z(kModeDual);                     // p-update in the Fourier domain, spectrum of K p, z lines back
+        if (!literal) {
+            pass_z(kModeDual);                 // p-update in the Fourier domain, spectrum of K p, z lines back
+        } else {
+            pass_z(kModeMulD);                 // K chi_bar ...
+            pass_y(true);
+            pass_x(nullptr, p->kp, true);
+            q_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);   // ... q-update and p-update, W p ...
+            ++launches;
+            pass_x(v.wp, nullptr, false);      // ... and K (W p)
+            pass_y(false);
+            pass_z(kModeMulD);
+        }
         pass_y(true);
         pass_x(nullptr, p->kp, true);          // K p
-        q_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
+        if (!literal) {
+            q_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
+            ++launches;
+        }
         chi_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
-        launches += 2;
+        ++launches;
     }
     if (max_iters > 0) {
         vol_unscale_kernel<<<vgrid, kThreads, 0, st>>>(chi_out, T, v.lv, p->cscale + nvol);
@@ -562,6 +609,18 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     p->last_launches = launches;
     e = cudaGetLastError();
     return e == cudaSuccess ? PD_OK : pd_cuda_fail_((int)e, "pd_solve3d launch");
+}
+
+int pd_set_weight3d(pd_plan3d_t p, const float *W) {
+    if (!p || ((unsigned long long)W & 15ull)) return PD_EINVAL;
+    if (W && !p->pimg) {   // workspace of the literal path: p and W p
+        const size_t T = (size_t)p->nx * p->ny * p->nz * (size_t)p->nvol;
+        const cudaError_t e = cudaMalloc((void **)&p->pimg, 2 * T * sizeof(float));
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); p->pimg = nullptr; return PD_ENOMEM; }
+        if (e != cudaSuccess) return pd_cuda_fail_((int)e, "cudaMalloc");
+    }
+    p->weight = W;
+    return PD_OK;
 }
 
 int pd_last_launch_count3d(pd_plan3d_t p) { return p ? p->last_launches : PD_EINVAL; }

@@ -40,9 +40,11 @@ def vol_rel(a, b):
     return np.linalg.norm(a - b, axis=1) / np.maximum(np.linalg.norm(b, axis=1), 1e-300)
 
 
-def gpu_solve3(torch, pd, field, mask, iters, *, lam, b0, sigma=0.25, tau=0.25, theta=1.0):
+def gpu_solve3(torch, pd, field, mask, iters, *, lam, b0, sigma=0.25, tau=0.25, theta=1.0, weight=None):
     nvol, nz, ny, nx = field.shape
     plan = pd.Plan3D(nx, ny, nz, nvol, b0, lam, sigma, tau, theta)
+    if weight is not None:
+        plan.set_weight(torch.from_numpy(weight).cuda())
     f = torch.from_numpy(field).cuda()
     m = None if mask is None else torch.from_numpy(mask).cuda()
     out = torch.full_like(f, float("nan"))
@@ -74,6 +76,24 @@ def test_iterations_exercise_q_and_divergence(torch, pd, o3, iters, theta, maske
     assert vol_rel(g, o).max() < (1e-5 if iters <= 3 else 1e-3)
     assert vol_rel(g, o).max() < 2e-5                                  # what fp32 actually achieves
     assert np.abs(g.reshape(3, -1).mean(1)).max() < 1e-5 * np.abs(g).max()   # D3(0) = 0 and sum(G^T v) = 0: zero mean
+
+
+@pytest.mark.parametrize("nx,ny,nz,b0,iters", [(16, 8, 8, 2, 1), (64, 32, 16, 0, 1), (128, 64, 64, 1, 1), (64, 32, 16, 2, 12)])
+def test_data_weighting(torch, pd, o3, nx, ny, nz, b0, iters):
+    """W set: the literal iteration (p in the image domain, K applied twice), three volumes (the last rides alone)."""
+    case = synth.volume_case(nx, ny, nz, nvol=3, seed=nx + iters, b0_axis=b0)
+    rng = np.random.default_rng(nx * nz)
+    w = rng.uniform(0.2, 1.0, size=case["field"].shape).astype(np.float32)
+    lam = 0.02 * float(np.abs(case["field"]).max())
+    g, launches = gpu_solve3(torch, pd, case["field"], case["mask"], iters, lam=lam, b0=b0, weight=w)
+    o = o3.solve3(case["field"], case["mask"], w, lambda_=lam, sigma=0.25, tau=0.25, max_iters=iters, b0_dir=b0)
+    assert vol_rel(g, o).max() < (1e-5 if iters == 1 else 2e-5)
+    assert launches == 2 + 3 + 12 * iters + 1
+    # W = 1 everywhere through the literal path equals the Fourier-domain path up to rounding
+    one = np.ones_like(w)
+    g1, _ = gpu_solve3(torch, pd, case["field"], case["mask"], iters, lam=lam, b0=b0, weight=one)
+    g0, _ = gpu_solve3(torch, pd, case["field"], case["mask"], iters, lam=lam, b0=b0)
+    assert vol_rel(g1, g0).max() < 2e-5
 
 
 def test_automatic_steps_alpha_zero_and_max_iters_zero(torch, pd, o3):

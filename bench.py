@@ -274,7 +274,7 @@ def run_prepost(args):
 def run_volume(args):
     """--volume: the true 3-D variant (NEXT-2) on 8 coil volumes of 256 x 256 x 64 (the voxel count of 512 slices of 256^2),
     100 iterations; voxel-iterations/s, HBM roofline of the whole step from its algorithmic bytes (DESIGN.md 5.7:
-    the bytes its seven passes must move, two volumes per complex transform: 8 + 8 + 22 + 8 + 8 + 32 + 32 = 118 B per voxel and iteration with a mask).  Its own JSON line."""
+    the bytes its seven passes must move, two volumes per complex transform: q-update 32, y 8, z with the p-update 22, y 8, x back + chi-update + x forward 4 + 28 + 4 = 106 B per voxel and iteration with a mask).  Its own JSON line."""
     import torch
     from paper_2006_09808_b200 import binding
     torch.cuda.set_device(0)
@@ -305,7 +305,7 @@ def run_volume(args):
     launches = plan.last_launch_count
     plan.destroy()
     nvox = nvol * nz * ny * nx
-    bytes_per_voxel_it = 172.0 if args.weighted else 118.0   # literal: 2 x (8 + 8 + 10 + 8 + 8) + 56 (q- and p-update) + 32
+    bytes_per_voxel_it = 172.0 if args.weighted else 106.0   # literal: 2 x (8 + 8 + 10 + 8 + 8) + 56 (q- and p-update) + 32
     gbs = bytes_per_voxel_it * nvox * iters / (ms * 1e-3) / 1e9
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import pd3_oracle as o3
@@ -317,7 +317,7 @@ def run_volume(args):
             "config": {"workload": "V1: %d coil volumes of %dx%dx%d (synth.volume_case), %d iterations, B0 along z, mask%s"
                                    % (nvol, nx, ny, nz, iters, ", random W in [0.2, 1] (literal iteration)" if args.weighted else ""),
                        "l2": "working set (%.1f GB) exceeds the 126 MB L2" % (44.0 * nvox / 1e9)},
-            "roofline": {"kernel": "whole step (%d launches per iteration)" % (12 if args.weighted else 7), "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
+            "roofline": {"kernel": "whole step (%d launches per iteration)" % (12 if args.weighted else 5), "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
                          "frac": gbs / peak, "algorithmic_bytes_per_voxel_iteration": bytes_per_voxel_it, "peak_source": peak_src, "traffic": None},
             "cpu_baseline": {"value": nz * ny * nx * 4 / dt, "unit": "voxel-iterations/s", "cores": os.cpu_count(), "kind": "oracle (numpy float64, numpy.fft)",
                              "sample": "1 volume, 4 iterations, %.1f s" % dt},

@@ -2,7 +2,7 @@
 // gradient operator in all three dimensions", with the 3-D dipole kernel, one problem per VOLUME
 // [nz][ny][nx] (slices are coupled: no per-slice stop, the iteration count is the caller's; R23, 5.7).
 //
-// A streaming implementation: W = identity, so the dual p lives in the Fourier domain as in DESIGN.md 5.0 -- ONE 3-D FFT
+// A streaming implementation: W = identity (else the literal path below), so the dual p lives in the Fourier domain as in DESIGN.md 5.0 -- ONE 3-D FFT
 // round trip per iteration -- and two real volumes (coils) ride one complex transform, z = a + i b (D3 is real and even,
 // so F^-1 D3 F z = K a + i K b, and the p-update is linear: it acts on the packed spectrum as it stands):
 //   x lines (chi_bar real -> complex) ; y lines ; z lines + [ p^ <- (p^ + sigma (D Z - phi^))/(1+sigma) ; Z <- D p^ ] + z lines
@@ -320,29 +320,91 @@ __global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
 
 // chi+ = chi - tau (K p + G^T (M q)) ; chi_bar = chi+ + theta (chi+ - chi)   (PAPER.md:49 lines 3, 4)
 // G^T v at a voxel = v_x(x-1) [x >= 1] - v_x(x) [x <= nx-2] + the same along y and z, v = M q.
-__global__ void __launch_bounds__(kThreads) chi_update3_kernel(const VoxArgs a) {
-    const long long sy = a.nx, sz = (long long)a.nx << a.ly, nquad = a.nvox >> 2;
-    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f), one = make_float4(1.f, 1.f, 1.f, 1.f);
+// Four voxels along x starting at voxel i = (.., z, y, x); k = K p there.  Stores chi+ and chi_bar, returns chi_bar.
+__device__ __forceinline__ float4 chi_quad(const VoxArgs &a, long long i, int x, int y, int z, float4 k) {
+    const long long sy = a.nx, sz = (long long)a.nx << a.ly;
+    const float4 one = make_float4(1.f, 1.f, 1.f, 1.f);
     auto mul4 = [](float4 u, float4 w) { return make_float4(u.x * w.x, u.y * w.y, u.z * w.z, u.w * w.w); };
+    const float4 m = a.mask ? ld4(a.mask + i) : one;
+    float4 vx = mul4(m, ld4(a.qx + i));
+    const float4 vy = mul4(m, ld4(a.qy + i)), vz = mul4(m, ld4(a.qz + i));
+    const float vxl = x >= 1 ? (a.mask ? a.mask[i - 1] : 1.f) * a.qx[i - 1] : 0.f;
+    if (x + 4 == a.nx) vx.w = 0.f;                                                 // no difference leaves the last column
+    float4 div = make_float4(vxl - vx.x, vx.x - vx.y, vx.y - vx.z, vx.z - vx.w);
+    if (y >= 1) { const float4 t = mul4(a.mask ? ld4(a.mask + i - sy) : one, ld4(a.qy + i - sy)); div.x += t.x; div.y += t.y; div.z += t.z; div.w += t.w; }
+    if (y + 1 < a.ny) { div.x -= vy.x; div.y -= vy.y; div.z -= vy.z; div.w -= vy.w; }
+    if (z >= 1) { const float4 t = mul4(a.mask ? ld4(a.mask + i - sz) : one, ld4(a.qz + i - sz)); div.x += t.x; div.y += t.y; div.z += t.z; div.w += t.w; }
+    if (z + 1 < a.nz) { div.x -= vz.x; div.y -= vz.y; div.z -= vz.z; div.w -= vz.w; }
+    const float4 c = ld4(a.chi + i);
+    const float4 n = make_float4(c.x - a.tau * (k.x + div.x), c.y - a.tau * (k.y + div.y), c.z - a.tau * (k.z + div.z), c.w - a.tau * (k.w + div.w));
+    const float4 bar = make_float4(n.x + a.theta * (n.x - c.x), n.y + a.theta * (n.y - c.y), n.z + a.theta * (n.z - c.z), n.w + a.theta * (n.w - c.w));
+    st4(a.chi + i, n);
+    st4(a.chibar + i, bar);
+    return bar;
+}
+
+__global__ void __launch_bounds__(kThreads) chi_update3_kernel(const VoxArgs a) {
+    const long long nquad = a.nvox >> 2;
     for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < nquad; i4 += (long long)gridDim.x * kThreads) {
         const long long i = i4 << 2;
         const int x = (int)(i & (a.nx - 1)), y = (int)((i >> a.lx) & (a.ny - 1)), z = (int)((i >> (a.lx + a.ly)) & (a.nz - 1));
-        const float4 m = a.mask ? ld4(a.mask + i) : one;
-        float4 vx = mul4(m, ld4(a.qx + i));
-        const float4 vy = mul4(m, ld4(a.qy + i)), vz = mul4(m, ld4(a.qz + i));
-        const float vxl = x >= 1 ? (a.mask ? a.mask[i - 1] : 1.f) * a.qx[i - 1] : 0.f;
-        if (x + 4 == a.nx) vx.w = 0.f;                                                 // no difference leaves the last column
-        float4 div = make_float4(vxl - vx.x, vx.x - vx.y, vx.y - vx.z, vx.z - vx.w);
-        if (y >= 1) { const float4 t = mul4(a.mask ? ld4(a.mask + i - sy) : one, ld4(a.qy + i - sy)); div.x += t.x; div.y += t.y; div.z += t.z; div.w += t.w; }
-        if (y + 1 < a.ny) { div.x -= vy.x; div.y -= vy.y; div.z -= vy.z; div.w -= vy.w; }
-        if (z >= 1) { const float4 t = mul4(a.mask ? ld4(a.mask + i - sz) : one, ld4(a.qz + i - sz)); div.x += t.x; div.y += t.y; div.z += t.z; div.w += t.w; }
-        if (z + 1 < a.nz) { div.x -= vz.x; div.y -= vz.y; div.z -= vz.z; div.w -= vz.w; }
-        const float4 c = ld4(a.chi + i), k = ld4(a.kp + i);
-        const float4 n = make_float4(c.x - a.tau * (k.x + div.x), c.y - a.tau * (k.y + div.y), c.z - a.tau * (k.z + div.z), c.w - a.tau * (k.w + div.w));
-        st4(a.chi + i, n);
-        st4(a.chibar + i, make_float4(n.x + a.theta * (n.x - c.x), n.y + a.theta * (n.y - c.y), n.z + a.theta * (n.z - c.z), n.w + a.theta * (n.w - c.w)));
-        (void)zero;
+        chi_quad(a, i, x, y, z, ld4(a.kp + i));
     }
+}
+
+// W = identity, nx in {64, 128, 256}: the x lines back, the chi-update and the x lines of the NEXT iteration in one
+// kernel -- K p never goes to memory and chi_bar is not read back (12 of 118 bytes per voxel and iteration).  The 16 lines
+// of the tile come out of the inverse transform in the thread map of fft_regs.cuh; they are laid into shared memory as
+// (K p_a, K p_b) rows, the chi-update runs over the rows with coalesced float4 accesses (both volumes of the pair) and
+// leaves (chi_bar_a, chi_bar_b) in their place, from where the forward transform picks its points up again.
+template <int N>
+__global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, 1024 / (kTL * pdk::FftCfg<N>::T)) fused_x_kernel(const FftArgs a, const VoxArgs va, const int do_fwd) {
+    using Cfg = pdk::FftCfg<N>;
+    constexpr int E = Cfg::E, T = Cfg::T, LD = T + 1, NT = kTL * T, REG = E * LD + 1;
+    static_assert(kTL * REG >= kTL * N, "the exchange buffer doubles as the tile of rows");
+    __shared__ float2 tws[E * T];
+    __shared__ float2 ex[kTL * REG];
+    pdk::TwiddlesSmem<N>::fill(tws, a.tw, threadIdx.x, NT);
+    const int l = threadIdx.x / T, j = threadIdx.x % T;
+    pdk::TwiddlesSmem<N> tw;
+    tw.w = tws + j;
+    float2 *sm = ex + l * REG;
+    const long long L0 = (long long)blockIdx.x * kTL;
+    const bool live = L0 + l < a.nlines;
+    float2 *const zl = a.z + (L0 + l) * N;
+    float2 v[E];
+#pragma unroll
+    for (int m = 0; m < E; ++m) v[m] = live ? zl[j + T * m] : make_float2(0.f, 0.f);
+    __syncthreads();   // twiddle table filled
+#pragma unroll
+    for (int m = 0; m < E; ++m) v[m] = make_float2(v[m].y, v[m].x);   // inverse = forward of the swapped halves
+    pdk::fft_line<N, LD>(v, sm, j, tw, pdk::WarpSync());
+    __syncthreads();   // every line is through its exchange: the buffer becomes the tile of rows
+#pragma unroll
+    for (int m = 0; m < E; ++m) ex[l * N + j + T * m] = make_float2(v[m].y * a.out_scale, v[m].x * a.out_scale);
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < kTL * (N / 4); idx += NT) {
+        const int row = idx / (N / 4), x = (idx % (N / 4)) * 4;
+        const long long L = L0 + row;
+        if (L >= a.nlines) continue;
+        const long long pv = L / a.lines_per_vol;
+        const int r = (int)(L - pv * a.lines_per_vol), y = r & (va.ny - 1), z = r >> va.ly;
+        float2 *t = ex + row * N + x;
+        const long long i = (2 * pv) * a.V + (long long)r * N + x;
+        const float4 ba = chi_quad(va, i, x, y, z, make_float4(t[0].x, t[1].x, t[2].x, t[3].x));
+        float4 bb = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (2 * pv + 1 < a.nvol) bb = chi_quad(va, i + a.V, x, y, z, make_float4(t[0].y, t[1].y, t[2].y, t[3].y));
+        t[0] = make_float2(ba.x, bb.x); t[1] = make_float2(ba.y, bb.y); t[2] = make_float2(ba.z, bb.z); t[3] = make_float2(ba.w, bb.w);
+    }
+    if (!do_fwd) return;
+    __syncthreads();
+#pragma unroll
+    for (int m = 0; m < E; ++m) v[m] = ex[l * N + j + T * m];
+    __syncthreads();   // the rows have been read: the buffer is the exchange region again
+    pdk::fft_line<N, LD>(v, sm, j, tw, pdk::WarpSync());
+    if (!live) return;
+#pragma unroll
+    for (int m = 0; m < E; ++m) zl[j + T * m] = v[m];
 }
 
 // Per-volume normalisation (the 2-D path's pair_scale): the iteration is exactly invariant under
@@ -578,8 +640,13 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
         e = cudaMemsetAsync(p->pimg, 0, T * sizeof(float), st);
         if (e != cudaSuccess) return pd_cuda_fail_((int)e, "cudaMemsetAsync (3-D dual)");
     }
+    const bool fused = !literal && nx >= 64;      // the chi-update rides the x passes (fused_x_kernel)
     for (int n = 0; n < max_iters; ++n) {
-        pass_x(p->chibar, nullptr, false);     // F chi_bar
+        if (fused) {   // the q-update needs chi_bar_n, which the fused kernel at the end of the iteration overwrites
+            q_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);
+            ++launches;
+        }
+        if (!fused || n == 0) pass_x(p->chibar, nullptr, false);     // F chi_bar
         pass_y(false);
         if (!literal) {
             pass_z(kModeDual);                 // p-update in the Fourier domain, spectrum of K p, z lines back
@@ -594,6 +661,16 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
             pass_z(kModeMulD);
         }
         pass_y(true);
+        if (fused) {   // x lines back + chi-update + x lines of the next iteration
+            FftArgs a = f;
+            a.tw = p->tw[0]; a.nlines = xlines;
+            const int fwd = n + 1 < max_iters ? 1 : 0;
+            if (nx == 64) fused_x_kernel<64><<<gx, kTL * pdk::FftCfg<64>::T, 0, st>>>(a, v, fwd);
+            else if (nx == 128) fused_x_kernel<128><<<gx, kTL * pdk::FftCfg<128>::T, 0, st>>>(a, v, fwd);
+            else fused_x_kernel<256><<<gx, kTL * pdk::FftCfg<256>::T, 0, st>>>(a, v, fwd);
+            ++launches;
+            continue;
+        }
         pass_x(nullptr, p->kp, true);          // K p
         if (!literal) {
             q_update3_kernel<<<vgrid, kThreads, 0, st>>>(v);

@@ -63,7 +63,8 @@ def test_one_iteration_all_axes(torch, pd, o3, nx, ny, nz, b0):
     g, launches = gpu_solve3(torch, pd, f, m, 1, lam=0.05, b0=b0)
     o = o3.solve3(f, m, lambda_=0.05, sigma=0.25, tau=0.25, max_iters=1, b0_dir=b0)
     assert vol_rel(g, o).max() < 1e-5
-    assert launches == 2 + 3 + 7 + 1          # normalisation, phi^, one iteration, un-normalisation
+    # normalisation, phi^, one iteration, un-normalisation; nx >= 64: the chi-update rides the x passes (one launch less)
+    assert launches == 2 + 3 + (6 if nx >= 64 else 7) + 1
 
 
 @pytest.mark.parametrize("iters,theta,masked", [(2, 1.0, True), (3, 0.5, True), (25, 1.0, True), (25, 1.0, False)])

@@ -222,7 +222,7 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
 int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_out, int max_iters, void *cuda_stream);
 /* Optional data weighting W of Eq.(1) for the 3-D variant (DEVICE, [nvol][nz][ny][nx], 16-byte aligned, caller-owned, must
  * outlive the solves; |W| <= 1 is assumed by the step bound); NULL = identity.  With W set the dual p stays in the image
- * domain and K is applied twice per iteration, literally as PAPER.md:49 (12 launches per iteration instead of 7); the
+ * domain and K is applied twice per iteration, literally as PAPER.md:49 (12 launches per iteration instead of 5); the
  * first call with a non-NULL W allocates 8 bytes per voxel.  Errors: PD_EINVAL, PD_ENOMEM, PD_ECUDA. */
 int pd_set_weight3d(pd_plan3d_t p, const float *W);
 int pd_last_launch_count3d(pd_plan3d_t p);   /* kernels enqueued by the last pd_solve3d */

@@ -318,7 +318,9 @@ def run_volume(args):
                                    % (nvol, nx, ny, nz, iters, ", random W in [0.2, 1] (literal iteration)" if args.weighted else ""),
                        "l2": "working set (%.1f GB) exceeds the 126 MB L2" % (44.0 * nvox / 1e9)},
             "roofline": {"kernel": "whole step (%d launches per iteration)" % (12 if args.weighted else 5), "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
-                         "frac": gbs / peak, "algorithmic_bytes_per_voxel_iteration": bytes_per_voxel_it, "peak_source": peak_src, "traffic": None},
+                         "frac": gbs / peak, "algorithmic_bytes_per_voxel_iteration": bytes_per_voxel_it, "peak_source": peak_src,
+                         # dram__bytes_read.sum + dram__bytes_write.sum over the five kernels of one iteration (profiles/r02/ncu_volume.md)
+                         "traffic": None if args.weighted else 100.3 * nvox * iters},
             "cpu_baseline": {"value": nz * ny * nx * 4 / dt, "unit": "voxel-iterations/s", "cores": os.cpu_count(), "kind": "oracle (numpy float64, numpy.fft)",
                              "sample": "1 volume, 4 iterations, %.1f s" % dt},
             "gpu_launches": launches * args.steps, "clocks": clocks}

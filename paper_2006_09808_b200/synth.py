@@ -335,3 +335,26 @@ def volume_case(nx, ny, nz, nvol=1, seed=0, b0_axis=2, noise=0.01):
         mask[v] = (((xx - nx / 2.0) / (0.46 * nx)) ** 2 + ((yy - ny / 2.0) / (0.46 * ny)) ** 2 + ((zz - nz / 2.0) / (0.48 * nz)) ** 2 <= 1.0)
         truth[v] = chi
     return {"field": field, "mask": mask, "chi_true": truth}
+
+
+def echo_volumes(nx, ny, nz, ncoils, seed=0, b0_axis=2, phase_span=2.5, noise=0.01):
+    """The two complex acquisitions of ONE object seen by `ncoils` coils, as volumes [ncoils][nz][ny][nx]:
+    volume_case's phantom field (one volume, the same for every coil), per coil a Gaussian sensitivity around a point on a
+    circle in the x-y plane times the tissue magnitude (1 inside the ellipsoidal mask, 0.2 outside), a smooth receive
+    phase, the second echo rotated by pscale x field, complex Gaussian noise.  Returns dict(s0, s1, fscale, field, mask)."""
+    case = volume_case(nx, ny, nz, nvol=1, seed=seed, b0_axis=b0_axis, noise=0.0)
+    f, m = case["field"][0].astype(np.float64), case["mask"][0]
+    pscale = phase_span / float(np.abs(f).max())
+    zz, yy, xx = np.mgrid[0:nz, 0:ny, 0:nx]
+    s0 = np.empty((ncoils, nz, ny, nx), np.complex64)
+    s1 = np.empty((ncoils, nz, ny, nx), np.complex64)
+    for c in range(ncoils):
+        ang = 2.0 * np.pi * (c + 0.25) / ncoils
+        cx, cy = nx * (0.5 + 0.45 * np.cos(ang)), ny * (0.5 + 0.45 * np.sin(ang))
+        A = (0.15 + np.exp(-((xx - cx) ** 2 + (yy - cy) ** 2) / (2.0 * (0.45 * min(nx, ny)) ** 2))) * np.where(m > 0, 1.0, 0.2)
+        u = uniform01(stream_key(950 + seed, c, 0, _ECHO_PHASE), 6)
+        theta0 = 2.0 * np.pi * (u[0] * xx / nx + u[1] * yy / ny + u[2] * zz / nz) + 0.5 * np.sin(2.0 * np.pi * (xx / nx + u[3]))
+        g = normal01(stream_key(950 + seed, c, 0, _ECHO_NOISE), 4 * nx * ny * nz).reshape(4, nz, ny, nx)
+        s0[c] = (A * np.exp(1j * theta0) + noise * (g[0] + 1j * g[1])).astype(np.complex64)
+        s1[c] = (A * np.exp(1j * (theta0 + pscale * f)) + noise * (g[2] + 1j * g[3])).astype(np.complex64)
+    return {"s0": s0, "s1": s1, "fscale": 1.0 / pscale, "field": case["field"][0], "mask": m}

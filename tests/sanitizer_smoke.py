@@ -7,7 +7,8 @@
 
 No oracle, no assertions on values beyond "finite": the parity tests do that; this only drives the kernels (resident with
 the state on chip, resident literal, streaming two-launch and literal, l1 regulariser, general lengths, hybrid schedule,
-tolerance stop, graphed loop and plain launches) at sizes a sanitizer finishes in minutes.  Prints one line per case.
+tolerance stop, graphed loop and plain launches, the static-workspace entry point, pre-processing and coil combination,
+the 3-D variant) at sizes a sanitizer finishes in minutes.  Prints one line per case.
 """
 import os
 import sys
@@ -84,6 +85,35 @@ def main():
     plan.solve_host(case["field"], case["mask"], chi, 3, 0.0)
     print("%-44s finite %s" % ("pd_solve_host 64x64 x200 (chunks)", bool(np.isfinite(chi).all())), flush=True)
     plan.destroy()
+    # the allocation-free entry point (static workspace), the steps either side, the 3-D variant (both line-transform
+    # families, the fused x kernel, the literal path with W)
+    case = synth.random_case(128, 64, 5, seed=7, with_mask=True)
+    f, m = torch.from_numpy(case["field"]).cuda(), torch.from_numpy(case["mask"]).cuda()
+    out = torch.empty_like(f)
+    pd.solve_static(f, m, out, 3, lambda_=0.2)
+    torch.cuda.synchronize()
+    print("%-44s finite %s" % ("pd_solve_static 64x128 x5", bool(torch.isfinite(out).all())), flush=True)
+    e = synth.echo_pair(0, nslices=3)
+    a, b = torch.from_numpy(e["s0"]).cuda(), torch.from_numpy(e["s1"]).cuda()
+    fm, w, mk = (torch.empty(e["s0"].shape, device="cuda") for _ in range(3))
+    wmax = torch.zeros(1, device="cuda")
+    pd.preprocess(a, b, e["fscale"], 0.3, field=fm, weight=w, mask=mk, wmax=wmax)
+    comb = torch.empty((1,) + tuple(fm.shape[1:]), device="cuda")
+    pd.combine_coils(fm, w, 3, comb)
+    torch.cuda.synchronize()
+    print("%-44s finite %s" % ("pd_preprocess / pd_combine_coils", bool(torch.isfinite(fm).all() and torch.isfinite(comb).all())), flush=True)
+    for name, (nx, ny, nz), weighted in [("3-D 16x8x8 (radix-2 lines)", (16, 8, 8), False), ("3-D 64x32x16 (register lines, fused x)", (64, 32, 16), False),
+                                         ("3-D 64x32x16, W (literal)", (64, 32, 16), True)]:
+        case = synth.volume_case(nx, ny, nz, nvol=3, seed=nx)
+        f3, m3 = torch.from_numpy(case["field"]).cuda(), torch.from_numpy(case["mask"]).cuda()
+        plan3 = pd.Plan3D(nx, ny, nz, 3, 2, 0.02, 0.25, 0.25, 1.0)
+        if weighted:
+            plan3.set_weight(0.2 + 0.8 * torch.rand(f3.shape, device="cuda"))
+        out3 = torch.empty_like(f3)
+        plan3.solve(f3, m3, out3, 3)
+        torch.cuda.synchronize()
+        plan3.destroy()
+        print("%-44s finite %s" % (name, bool(torch.isfinite(out3).all())), flush=True)
     print("sanitizer_smoke: done")
 
 

@@ -126,6 +126,38 @@ def test_pair_partners_of_unequal_magnitude(torch, pd, o3, ratio):
     assert not g[0].any() and g[1].any()
 
 
+def test_chain_preprocess_solve3d_combine(torch, pd, o3):
+    """Flow steps (1)-(5) on volumes: the two echo acquisitions of 3 coils -> field map, W, Mask (pd_preprocess) -> one
+    weighted, masked 3-D solve per coil volume (pd_set_weight3d, pd_solve3d) -> pd_combine_coils; the CUDA chain against
+    the oracle chain, every stage fed by its own side's previous stage."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import pd_prepost_oracle as po
+    nx, ny, nz, nc, iters, thr = 64, 32, 16, 3, 10, 0.3
+    e = synth.echo_volumes(nx, ny, nz, nc, seed=4)
+    a, b = torch.from_numpy(e["s0"]).cuda(), torch.from_numpy(e["s1"]).cuda()
+    f = torch.empty((nc, nz, ny, nx), device="cuda")
+    w, m, chi = torch.empty_like(f), torch.empty_like(f), torch.empty_like(f)
+    wmax = torch.zeros(1, device="cuda")
+    pd.preprocess(a.view(nc * nz, ny, nx), b.view(nc * nz, ny, nx), e["fscale"], thr, field=f.view(nc * nz, ny, nx),
+                  weight=w.view(nc * nz, ny, nx), mask=m.view(nc * nz, ny, nx), wmax=wmax)
+    lam = 0.02 * float(np.abs(e["field"]).max())
+    plan = pd.Plan3D(nx, ny, nz, nc, 2, lam, 0.25, 0.25, 1.0)
+    plan.set_weight(w)
+    plan.solve(f, m, chi, iters)
+    out = torch.empty((1, nz * ny, nx), device="cuda")
+    pd.combine_coils(chi.view(nc, nz * ny, nx), w.view(nc, nz * ny, nx), nc, out)      # one "slice" of nz*ny rows, nc coils
+    torch.cuda.synchronize()
+    plan.destroy()
+    of = po.field_map(e["s0"], e["s1"], e["fscale"]).astype(np.float32)
+    ow = po.weight(e["s0"], e["s1"], float(po.wscale_f32(e["s0"], e["s1"])))
+    om = po.mask_f32(e["s0"], e["s1"], thr)
+    assert np.array_equal(m.cpu().numpy(), om) and 0.05 < om.mean() < 0.95
+    ochi = o3.solve3(of, om, ow.astype(np.float32), lambda_=lam, sigma=0.25, tau=0.25, max_iters=iters, b0_dir=2)
+    assert vol_rel(chi.cpu().numpy(), ochi).max() < 1e-3
+    ocomb = po.combine_coils(ochi.reshape(nc, nz * ny, nx), ow.reshape(nc, nz * ny, nx), nc)
+    assert vol_rel(out.cpu().numpy(), ocomb).max() < 1e-3
+
+
 def test_full_size_volume(torch, pd, o3):
     """The size bench.py --volume times per coil: 256 x 256 x 64, 10 iterations against the oracle."""
     case = synth.volume_case(256, 256, 64, nvol=1, seed=9, b0_axis=2)

@@ -371,6 +371,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if (args.prepost or args.volume) and int(os.environ.get("RANK", "0")) != 0:
+        return 0   # single-GPU lines: under torchrun rank 0 alone runs and prints them
     if args.prepost:
         return run_prepost(args)
     if args.volume:

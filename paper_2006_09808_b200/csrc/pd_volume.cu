@@ -511,6 +511,7 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
     *out = nullptr;
     if (nvol < 1 || B0_axis < 0 || B0_axis > 2) return PD_EINVAL;
     if (!pow2_in(nx, 16, 256) || !pow2_in(ny, 8, 256) || !pow2_in(nz, 8, 256)) return PD_ESIZE;
+    if ((long long)((nvol + 1) / 2) * nz > 65535) return PD_ESIZE;   // the y passes put (pair, z) on gridDim.y
     if (!(lambda >= 0.f) || !(theta >= 0.f && theta <= 1.f) || std::isnan(sigma) || std::isnan(tau)) return PD_EINVAL;
     const double bound = 4.0 / 9.0 + 12.0;   // ||K||^2 <= 4/9, ||G||^2 <= 12 in three dimensions (tau = sigma = 1/L)
     if (!(sigma > 0.f) || !(tau > 0.f)) sigma = tau = (float)(1.0 / std::sqrt(bound));

@@ -173,6 +173,7 @@ def test_plan3d_errors(pd):
     assert L.pd_plan3d(C.byref(h), 8, 16, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE       # nx < 16
     assert L.pd_plan3d(C.byref(h), 64, 48, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE      # not a power of two
     assert L.pd_plan3d(C.byref(h), 512, 16, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE
+    assert L.pd_plan3d(C.byref(h), 16, 8, 256, 600, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE     # 300 pairs x 256 planes > 65535
     assert L.pd_plan3d(C.byref(h), 64, 16, 16, 1, 3, 0.01, 0.25, 0.25, 1.0) == pd.EINVAL     # B0 axis
     assert L.pd_plan3d(C.byref(h), 64, 16, 16, 0, 2, 0.01, 0.25, 0.25, 1.0) == pd.EINVAL
     assert L.pd_plan3d(C.byref(h), 64, 16, 16, 1, 2, 0.01, 0.3, 0.3, 1.0) == pd.ESTEP        # 0.09 * 12.44 > 1

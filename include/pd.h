@@ -209,8 +209,9 @@ int pd_destroy(pd_plan_t p);
  * norm, forward differences with Neumann boundary on all three axes, W optional (pd_set_weight3d), lambda on the regulariser (R2).  The
  * slices of a volume are coupled by the z transform and the z difference: there is no per-slice stop, the call runs
  * exactly max_iters iterations.  A streaming implementation (5 launches per iteration).
- * pd_plan3d: nx in {16..256}, ny, nz in {8..256}, powers of two, ceil(nvol/2)*nz <= 65535 (else PD_ESIZE); nvol independent
- *   volumes (coils);
+ * pd_plan3d: nx in {16..256}, ny in {8..256}, powers of two; nz a power of two in {8..256} or ANY slice count in [2, 64]
+ *   (the paper's volumes have 25, 12 and 42 slices: dense z-line transform); ceil(nvol/2)*nz <= 65535
+ *   (else PD_ESIZE); nvol independent volumes (coils);
  *   B0_axis 0 = x, 1 = y, 2 = z; sigma <= 0 or tau <= 0: automatic steps 1/sqrt(4/9 + 12); explicit steps with
  *   sigma*tau*(4/9 + 12) >= 1 give PD_ESTEP.  Allocates 32 bytes per voxel of workspace + the D3 table.  Volumes 2k and
  *   2k+1 ride one complex transform, each in its own power-of-two normalisation 2^-floor(log2 rms(field_v)) (exact; the

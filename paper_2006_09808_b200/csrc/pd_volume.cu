@@ -260,9 +260,70 @@ __global__ void __launch_bounds__(kTL * pdk::FftCfg<N>::T, (mode == kModeDual ? 
     }
 }
 
+// z lines of ANY length up to 64 (the paper's volumes have 25, 12 and 42 slices): a dense DFT per line in
+// shared memory, O(nz^2) -- 2 x 42 complex multiply-adds per voxel pair for nz = 42, still cheaper than the pass's memory
+// traffic is long.  Same tiles (16 adjacent x) and the same modes as the strided kernels above.
+constexpr int kDenseMax = 64;
+__global__ void __launch_bounds__(kThreads) dft_lines_dense_kernel(const FftArgs a, const int mode, const int N) {
+    __shared__ float2 buf[2][kTL * (kDenseMax + 1)];
+    __shared__ float2 tws[kDenseMax];
+    const int LD = N + 1;
+    for (int k = threadIdx.x; k < N; k += kThreads) tws[k] = a.tw[k];
+    const long long vol = (long long)blockIdx.y * N * a.S, base = vol + (long long)blockIdx.x * kTL;
+    for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
+        const int l = idx % kTL, k = idx / kTL;
+        buf[0][l * LD + k] = a.z[base + (long long)k * a.S + l];
+    }
+    __syncthreads();
+    auto dft = [&](const float2 *in, float2 *out, bool inverse) {   // out[k] = sum_n in[n] W^(+-nk)
+        for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
+            const int l = idx % kTL, k = idx / kTL;
+            float2 acc = make_float2(0.f, 0.f);
+            int e = 0;
+            for (int n = 0; n < N; ++n) {
+                float2 w = tws[e];
+                if (inverse) w.y = -w.y;
+                const float2 c = in[l * LD + n];
+                acc.x = fmaf(c.x, w.x, fmaf(-c.y, w.y, acc.x));
+                acc.y = fmaf(c.x, w.y, fmaf(c.y, w.x, acc.y));
+                e += k;
+                if (e >= N) e -= N;
+            }
+            out[l * LD + k] = acc;
+        }
+        __syncthreads();
+    };
+    dft(buf[0], buf[1], a.inverse != 0);
+    float2 *res = buf[1];
+    if (mode == kModeStoreSpectrum || mode == kModeDual || mode == kModeMulD) {
+        for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
+            const int l = idx % kTL, k = idx / kTL;
+            const long long g = base + (long long)k * a.S + l;
+            const float2 z = buf[1][l * LD + k];
+            if (mode == kModeStoreSpectrum) { a.phihat[g] = z; continue; }
+            const float d = a.D[g - vol];
+            if (mode == kModeMulD) { buf[1][l * LD + k] = make_float2(d * z.x, d * z.y); continue; }
+            const float2 f = a.phihat[g];
+            float2 p = a.phat[g];
+            p.x = (p.x + a.sigma * (d * z.x - f.x)) * a.inv1ps;
+            p.y = (p.y + a.sigma * (d * z.y - f.y)) * a.inv1ps;
+            a.phat[g] = p;
+            buf[1][l * LD + k] = make_float2(d * p.x, d * p.y);
+        }
+        if (mode == kModeStoreSpectrum) return;
+        __syncthreads();
+        dft(buf[1], buf[0], true);
+        res = buf[0];
+    }
+    for (int idx = threadIdx.x; idx < kTL * N; idx += kThreads) {
+        const int l = idx % kTL, k = idx / kTL;
+        a.z[base + (long long)k * a.S + l] = res[l * LD + k];
+    }
+}
+
 struct VoxArgs {
     int nx, ny, nz;           // powers of two; nx a multiple of 4
-    int lx, ly, lv;           // log2 nx, log2 ny, log2 (nx ny nz)
+    int lx, ly, lv, lz;       // log2 nx, log2 ny, log2 (nx ny nz) (unused), log2 nz or -1 when nz is not a power of two
     const float *cscale;      // [nvol] normalisation of every volume: the ball of volume v has radius alpha * cscale[v]
     const float *weight, *field;   // literal path (W set): W, and the caller's phi (normalised on the fly)
     float *p, *wp;                 // literal path: the dual p in the image domain, and W p (input of the second K)
@@ -285,14 +346,15 @@ __global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f), one = make_float4(1.f, 1.f, 1.f, 1.f);
     for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < nquad; i4 += (long long)gridDim.x * kThreads) {
         const long long i = i4 << 2;
-        const int x = (int)(i & (a.nx - 1)), y = (int)((i >> a.lx) & (a.ny - 1)), z = (int)((i >> (a.lx + a.ly)) & (a.nz - 1));
+        const int plane = (int)(i >> (a.lx + a.ly)), vol = a.lz >= 0 ? plane >> a.lz : plane / a.nz;   // nz need not be a power of two
+        const int x = (int)(i & (a.nx - 1)), y = (int)((i >> a.lx) & (a.ny - 1)), z = plane - vol * a.nz;
         const float4 c = ld4(a.chibar + i), m = a.mask ? ld4(a.mask + i) : one;
         const float cn = x + 4 < a.nx ? a.chibar[i + 4] : c.w;                         // Neumann: last x difference is 0
         const float4 gx = make_float4(c.y - c.x, c.z - c.y, c.w - c.z, cn - c.w);
         const float4 gy = y + 1 < a.ny ? sub4(ld4(a.chibar + i + sy), c) : zero;
         const float4 gz = z + 1 < a.nz ? sub4(ld4(a.chibar + i + sz), c) : zero;
         float4 qx = ld4(a.qx + i), qy = ld4(a.qy + i), qz = ld4(a.qz + i);
-        const float alpha = a.alpha * a.cscale[i >> a.lv];
+        const float alpha = a.alpha * a.cscale[vol];
         auto one_voxel = [&](float &px, float &py, float &pz, float mm, float dx, float dy, float dz) {
             const float tx = px + a.sigma * mm * dx, ty = py + a.sigma * mm * dy, tz = pz + a.sigma * mm * dz;
             const float nrm = sqrtf(tx * tx + ty * ty + tz * tz);
@@ -305,7 +367,7 @@ __global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
         one_voxel(qx.w, qy.w, qz.w, m.w, gx.w, gy.w, gz.w);
         st4(a.qx + i, qx); st4(a.qy + i, qy); st4(a.qz + i, qz);
         if (a.weight) {   // literal path: p <- (p + sigma W (K chi_bar - phi))/(1 + sigma)  (PAPER.md:49 line 1; R3); a.kp holds K chi_bar
-            const float cs = a.cscale[i >> a.lv];
+            const float cs = a.cscale[vol];
             const float4 w = ld4(a.weight + i), u = ld4(a.kp + i), f = ld4(a.field + i);
             float4 pp = ld4(a.p + i);
             pp.x = (pp.x + a.sigma * w.x * (u.x - cs * f.x)) * a.inv1ps;
@@ -347,7 +409,8 @@ __global__ void __launch_bounds__(kThreads) chi_update3_kernel(const VoxArgs a) 
     const long long nquad = a.nvox >> 2;
     for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < nquad; i4 += (long long)gridDim.x * kThreads) {
         const long long i = i4 << 2;
-        const int x = (int)(i & (a.nx - 1)), y = (int)((i >> a.lx) & (a.ny - 1)), z = (int)((i >> (a.lx + a.ly)) & (a.nz - 1));
+        const int plane = (int)(i >> (a.lx + a.ly)), vol = a.lz >= 0 ? plane >> a.lz : plane / a.nz;   // nz need not be a power of two
+        const int x = (int)(i & (a.nx - 1)), y = (int)((i >> a.lx) & (a.ny - 1)), z = plane - vol * a.nz;
         chi_quad(a, i, x, y, z, ld4(a.kp + i));
     }
 }
@@ -415,9 +478,13 @@ constexpr int kScaleParts = 64;
 __global__ void __launch_bounds__(kThreads) vol_sumsq_kernel(const float *__restrict__ field, long long V, float *__restrict__ part) {
     const long long chunk = V / kScaleParts, b0 = (long long)blockIdx.y * V + (long long)blockIdx.x * chunk;
     float s = 0.f;
-    for (long long i = threadIdx.x * 4LL; i < chunk; i += kThreads * 4LL) {
-        const float4 f = ld4(field + b0 + i);
-        s += f.x * f.x + f.y * f.y + f.z * f.z + f.w * f.w;
+    if ((chunk & 3) == 0) {
+        for (long long i = threadIdx.x * 4LL; i < chunk; i += kThreads * 4LL) {
+            const float4 f = ld4(field + b0 + i);
+            s += f.x * f.x + f.y * f.y + f.z * f.z + f.w * f.w;
+        }
+    } else {   // an odd number of planes: chunks of 2 nz (nx ny / 128) floats are not 16-byte aligned
+        for (long long i = threadIdx.x; i < chunk; i += kThreads) { const float f = field[b0 + i]; s += f * f; }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
@@ -442,10 +509,10 @@ __global__ void vol_scale_kernel(const float *__restrict__ part, long long V, in
                                                    // whatever rounding noise its pair partner left in its lane
 }
 // chi <- chi / c_v at the end (exact)
-__global__ void __launch_bounds__(kThreads) vol_unscale_kernel(float *__restrict__ chi, long long nvox, int lv, const float *__restrict__ rscale) {
+__global__ void __launch_bounds__(kThreads) vol_unscale_kernel(float *__restrict__ chi, long long nvox, int lxy, int nz, const float *__restrict__ rscale) {
     for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < (nvox >> 2); i4 += (long long)gridDim.x * kThreads) {
         const long long i = i4 << 2;
-        const float r = rscale[i >> lv];
+        const float r = rscale[(int)(i >> lxy) / nz];
         float4 c = ld4(chi + i);
         c.x *= r; c.y *= r; c.z *= r; c.w *= r;
         st4(chi + i, c);
@@ -510,7 +577,7 @@ int pd_plan3d(pd_plan3d_t *out, int nx, int ny, int nz, int nvol, int B0_axis, f
     if (!out) return PD_EINVAL;
     *out = nullptr;
     if (nvol < 1 || B0_axis < 0 || B0_axis > 2) return PD_EINVAL;
-    if (!pow2_in(nx, 16, 256) || !pow2_in(ny, 8, 256) || !pow2_in(nz, 8, 256)) return PD_ESIZE;
+    if (!pow2_in(nx, 16, 256) || !pow2_in(ny, 8, 256) || !(pow2_in(nz, 8, 256) || (nz >= 2 && nz <= kDenseMax))) return PD_ESIZE;
     if ((long long)((nvol + 1) / 2) * nz > 65535) return PD_ESIZE;   // the y passes put (pair, z) on gridDim.y
     if (!(lambda >= 0.f) || !(theta >= 0.f && theta <= 1.f) || std::isnan(sigma) || std::isnan(tau)) return PD_EINVAL;
     const double bound = 4.0 / 9.0 + 12.0;   // ||K||^2 <= 4/9, ||G||^2 <= 12 in three dimensions (tau = sigma = 1/L)
@@ -611,7 +678,8 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     auto pass_z = [&](int mode) {
         FftArgs a = f;
         a.tw = p->tw[2]; a.S = (long long)nx * ny; a.inverse = 0;
-        launch_fft<true>(nz, gz, a, mode, st);
+        if (pow2_in(nz, 8, 256)) launch_fft<true>(nz, gz, a, mode, st);
+        else dft_lines_dense_kernel<<<gz, kThreads, 0, st>>>(a, mode, nz);   // any other slice count up to 64
         ++launches;
     };
     // per-volume normalisation, then phi^ = F (c phi), once (everything else starts at zero)
@@ -630,6 +698,8 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
     for (v.lx = 0; (1 << v.lx) < nx; ++v.lx) {}
     for (v.ly = 0; (1 << v.ly) < ny; ++v.ly) {}
     for (v.lv = 0; (1LL << v.lv) < V; ++v.lv) {}
+    v.lz = -1;
+    for (int b = 0; b < 9; ++b) if ((1 << b) == nz) v.lz = b;
     v.cscale = p->cscale;
     v.chi = chi_out; v.chibar = p->chibar; v.qx = p->q; v.qy = p->q + T; v.qz = p->q + 2 * T; v.kp = p->kp;
     v.sigma = p->sigma; v.tau = p->tau; v.theta = p->theta; v.alpha = p->lambda;
@@ -681,7 +751,7 @@ int pd_solve3d(pd_plan3d_t p, const float *field, const float *mask, float *chi_
         ++launches;
     }
     if (max_iters > 0) {
-        vol_unscale_kernel<<<vgrid, kThreads, 0, st>>>(chi_out, T, v.lv, p->cscale + nvol);
+        vol_unscale_kernel<<<vgrid, kThreads, 0, st>>>(chi_out, T, v.lx + v.ly, nz, p->cscale + nvol);
         ++launches;
     }
     p->last_launches = launches;

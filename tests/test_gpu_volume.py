@@ -97,6 +97,21 @@ def test_data_weighting(torch, pd, o3, nx, ny, nz, b0, iters):
     assert vol_rel(g1, g0).max() < 2e-5
 
 
+@pytest.mark.parametrize("nx,ny,nz", [(64, 32, 25), (128, 64, 12), (64, 64, 42), (16, 8, 3), (32, 16, 64)])
+def test_slice_counts_of_the_paper(torch, pd, o3, nx, ny, nz):
+    """Any slice count up to 64 (25, 12 and 42 slices): dense z-line transform; two volumes + one alone."""
+    case = synth.volume_case(nx, ny, nz, nvol=3, seed=nz, b0_axis=2)
+    lam = 0.02 * float(np.abs(case["field"]).max())
+    for iters, gate in [(1, 1e-5), (10, 2e-5)]:
+        g, _ = gpu_solve3(torch, pd, case["field"], case["mask"], iters, lam=lam, b0=2)
+        o = o3.solve3(case["field"], case["mask"], lambda_=lam, sigma=0.25, tau=0.25, max_iters=iters, b0_dir=2)
+        assert vol_rel(g, o).max() < gate
+    w = np.random.default_rng(nz).uniform(0.2, 1.0, size=case["field"].shape).astype(np.float32)
+    g, _ = gpu_solve3(torch, pd, case["field"], case["mask"], 4, lam=lam, b0=0, weight=w)      # literal path, B0 along x
+    o = o3.solve3(case["field"], case["mask"], w, lambda_=lam, sigma=0.25, tau=0.25, max_iters=4, b0_dir=0)
+    assert vol_rel(g, o).max() < 2e-5
+
+
 def test_automatic_steps_alpha_zero_and_max_iters_zero(torch, pd, o3):
     case = synth.volume_case(32, 16, 8, nvol=1, seed=3, b0_axis=0)
     s = 1.0 / np.sqrt(4.0 / 9.0 + 12.0)
@@ -171,7 +186,8 @@ def test_plan3d_errors(pd):
     import ctypes as C
     L, h = pd.lib(), C.c_void_p()
     assert L.pd_plan3d(C.byref(h), 8, 16, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE       # nx < 16
-    assert L.pd_plan3d(C.byref(h), 64, 48, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE      # not a power of two
+    assert L.pd_plan3d(C.byref(h), 64, 48, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE      # ny not a power of two
+    assert L.pd_plan3d(C.byref(h), 64, 32, 100, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE     # nz: a power of two, or <= 64
     assert L.pd_plan3d(C.byref(h), 512, 16, 16, 1, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE
     assert L.pd_plan3d(C.byref(h), 16, 8, 256, 600, 2, 0.01, 0.25, 0.25, 1.0) == pd.ESIZE     # 300 pairs x 256 planes > 65535
     assert L.pd_plan3d(C.byref(h), 64, 16, 16, 1, 3, 0.01, 0.25, 0.25, 1.0) == pd.EINVAL     # B0 axis

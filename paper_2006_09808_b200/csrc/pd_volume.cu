@@ -341,7 +341,7 @@ __device__ __forceinline__ float4 sub4(float4 a, float4 b) { return make_float4(
 
 // q <- proj_alpha(q + sigma M G chi_bar): forward differences, Neumann, pointwise Euclidean norm over the three components
 // (PAPER.md:49 line 2; R4, R7, R13 carried to 3-D by R23).  Four voxels along x per thread and trip.
-__global__ void __launch_bounds__(kThreads) q_update3_kernel(const VoxArgs a) {
+__global__ void __launch_bounds__(kThreads, 4) q_update3_kernel(const VoxArgs a) {
     const long long sy = a.nx, sz = (long long)a.nx << a.ly, nquad = a.nvox >> 2;
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f), one = make_float4(1.f, 1.f, 1.f, 1.f);
     for (long long i4 = (long long)blockIdx.x * kThreads + threadIdx.x; i4 < nquad; i4 += (long long)gridDim.x * kThreads) {
